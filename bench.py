@@ -1,0 +1,349 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the limited-1PN hot path (BASELINE.json: fp64 pair-interactions/s
+and RK4 steps/s at N = 1+16383, % of the B200 FP64 FMA peak).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload config2|config3|...]
+
+One timed "step" = one classical-RK4 step of the whole path (4 force evaluations: star-star pair kernel S1 +
+fused BH/1PN/RK4 epilogue S2-S4); the timed region is bracketed by the 1PN energy S5 at its start and end as in
+the paper's timing runs, and those two evaluations are INSIDE the timed region.
+value = ordered star-star pair interactions of the K steps / timed region (energy pairs not counted).
+Prints ONE JSON line (rank 0).  Multi-GPU = independent replicas: weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+FP64_INSTR_PER_PAIR = 15          # SASS-verified: 3 DADD + 9 DFMA + 3 DMUL per ordered pair (+1 MUFU.RSQ64H)
+FLOPS_PER_PAIR = 2 * FP64_INSTR_PER_PAIR  # issue-slot convention: every FP64-pipe instruction counted as an FMA
+SMS, FP64_LANES_PER_SM = 148, 64
+
+
+def load_peaks() -> dict:
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            return json.loads(p.read_text())
+        except Exception:
+            pass
+    return {}
+
+
+def make_problem(name: str, rank: int = 0):
+    from paper_1801_07986_b200 import inputs
+
+    if name.startswith("config"):
+        p = inputs.config(int(name[6:]))
+    elif name.startswith("ball"):
+        p = inputs.uniform_ball_bh(int(name[4:]))
+        p.dt, p.nsteps = 1e-4, 10
+    else:
+        raise SystemExit(f"unknown workload {name}")
+    if rank:  # replicas: same recipe, different seed per rank
+        seed = p.meta["seed"] + 1000 * rank
+        if p.meta["model"] == "plummer+bh":
+            q = inputs.plummer_bh(p.n_stars, seed, M=float(p.mass[0]), c=p.c, softening=p.softening, dt=p.dt, nsteps=p.nsteps)
+        elif p.meta["model"].startswith("bahcall"):
+            q = inputs.cusp_bh(p.n_stars, seed)
+        else:
+            q = p
+        q.name = p.name
+        p = q
+    return p
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        rows = [l for (t, l) in self.lines if t0 <= t <= t1] or [l for (_, l) in self.lines]
+        for l in rows:
+            f = [x.strip() for x in l.split(",")]
+            try:
+                sm.append(float(f[0])), smax.append(float(f[1])), power.append(float(f[2]))
+            except (ValueError, IndexError):
+                continue
+            for nm, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py executes oracle/)
+# ---------------------------------------------------------------------------------------------------------
+def oracle_step_sample(p, o, rows):
+    """One bounded 'step' of the oracle: a full RK4 step when all rows are taken, else 4 force evaluations
+    (one RK4 step's worth) restricted to `rows`; returns pairs visited."""
+    if rows is None:
+        o.step(p.pos, p.vel, p.dt, 1)
+        return 4 * p.pairs_per_eval
+    for _ in range(4):
+        o.accel_rows(p.pos, p.vel, rows)
+    return 4 * len(rows) * (p.n_stars - 1)
+
+
+def oracle_rows(p, budget_pairs=3.0e9):
+    """All stars if one RK4 step stays under the pair budget (config 2 does), else a seeded subset of i-rows."""
+    if 4 * p.pairs_per_eval <= budget_pairs:
+        return None, "full RK4 steps (all rows)"
+    r = max(64, int(budget_pairs / 4 / (p.n_stars - 1)))
+    rows = np.sort(np.random.default_rng(12345).choice(np.arange(1, p.N), size=r, replace=False))
+    return rows, f"4 force evaluations per step on a seeded subset of {r} of {p.n_stars} i-rows, each against all j"
+
+
+def cpu_baseline(p, target_s=12.0, max_steps=8) -> dict:
+    from oracle.pn_oracle import Oracle
+
+    o = Oracle(p.mass, p.G, p.c, p.softening, kind="fast")
+    rows, what = oracle_rows(p)
+    pairs, t0, n = 0, time.perf_counter(), 0
+    while n < max_steps and (time.perf_counter() - t0 < target_s or n == 0):
+        pairs += oracle_step_sample(p, o, rows)
+        n += 1
+    dt = time.perf_counter() - t0
+    return {"value": pairs / dt, "unit": "pair-interactions/s", "cores": o.max_threads, "kind": "oracle",
+            "build": "oracle/pn_oracle.c -DORACLE_FAST (double, -O3 -march=native, OpenMP over i)",
+            "sample": f"{n} x {what}; {dt:.1f} s", "steps_per_s": (n / dt) if rows is None else None}
+
+
+def run_reference(args) -> None:
+    """--impl reference: the oracle, as it stands, on the host cores; same metric/config keys as our arm."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle.pn_oracle import Oracle
+
+    p = make_problem(args.workload)
+    o = Oracle(p.mass, p.G, p.c, p.softening, kind="fast")
+    # bound the whole run to ~4e10 pair visits (about 1.5 min on 8 cores) whatever K is
+    rows, what = oracle_rows(p, budget_pairs=max(2.0e8, 4.0e10 / max(1, args.steps)))
+    for _ in range(args.warmup):
+        oracle_step_sample(p, o, rows if rows is None else rows[:64])
+    pairs, t0 = 0, time.perf_counter()
+    for _ in range(args.steps):
+        pairs += oracle_step_sample(p, o, rows)
+    dt = time.perf_counter() - t0
+    val = pairs / dt
+    line = {
+        "impl": "reference", "metric": "fp64 pair-interactions/s", "value": val, "unit": "pair-interactions/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(p, args),
+        "cpu_baseline": {"value": val, "unit": "pair-interactions/s", "cores": o.max_threads, "kind": "oracle",
+                         "sample": f"each step = {what}"},
+        "e2e": {"value": val, "unit": "pair-interactions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(p, args) -> dict:
+    return {"workload": p.name, "N": p.N, "n_stars": p.n_stars, "pairs_per_force_eval": p.pairs_per_eval,
+            "force_evals_per_step": 4, "dt": p.dt, "c": p.c, "softening": p.softening, "M": float(p.mass[0]),
+            "integrator": "classical RK4", "energy_evals_in_timed_region": 2,
+            "l2": "flushed (256 MiB write) between timed steps, outside the per-step event pairs",
+            "parallelism": f"replicas x{args.gpus}" if args.gpus > 1 else "single GPU"}
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Our arm: the CUDA path through the C-ABI
+# ---------------------------------------------------------------------------------------------------------
+def run_ours(args) -> None:
+    import torch
+    import torch.distributed as dist
+
+    from paper_1801_07986_b200 import PN, binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    p = make_problem(args.workload, rank)
+    K, W = args.steps, max(3, args.warmup)
+    stream = torch.cuda.current_stream()
+    pn = PN(p.mass, p.G, p.c, p.softening, stream=stream)
+    cfg = pn.pn_get_pair_config()
+    pos_d, vel_d = torch.from_numpy(p.pos).cuda(), torch.from_numpy(p.vel).cuda()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+
+    # ---------------- device-resident timing: energy, K x (RK4 step), energy; per-item CUDA event pairs
+    pn.pn_set_option(binding.PN_OPT_TIME_PAIR, 1)  # plain launches + events around every pair-kernel launch
+    pn.pn_set_state(pos_d, vel_d)
+    for _ in range(W):
+        pn.pn_step(p.dt, 1)
+    pn.pn_energy()
+    pn.pn_set_state(pos_d, vel_d)
+    pn.pn_get_pair_time(reset=True)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K + 2)]
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    barrier()
+    launches0 = pn.pn_get_launch_count()
+    t_wall0 = time.perf_counter()
+    ev[0][0].record(stream)
+    e_start = pn.pn_energy()
+    ev[0][1].record(stream)
+    for k in range(K):
+        flush.zero_()
+        ev[k + 1][0].record(stream)
+        pn.pn_step(p.dt, 1)
+        ev[k + 1][1].record(stream)
+    flush.zero_()
+    ev[K + 1][0].record(stream)
+    e_end = pn.pn_energy()
+    ev[K + 1][1].record(stream)
+    barrier()
+    t_wall1 = time.perf_counter()
+    launches = pn.pn_get_launch_count() - launches0
+    clocks = sampler.stop(t_wall0, t_wall1)
+    ms_items = [a.elapsed_time(b) for a, b in ev]
+    ms_energy = ms_items[0] + ms_items[-1]
+    ms_steps = sum(ms_items[1:-1])
+    ms_total = ms_energy + ms_steps
+    pair_ms, pair_n = pn.pn_get_pair_time(reset=True)
+    pn.pn_set_option(binding.PN_OPT_TIME_PAIR, 0)
+
+    # ---------------- same K steps through the CUDA-graph path (information: what a user gets by default)
+    pn.pn_set_state(pos_d, vel_d)
+    pn.pn_step(p.dt, 16 + 1)
+    barrier()
+    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    g0.record(stream)
+    pn.pn_step(p.dt, K)
+    g1.record(stream)
+    barrier()
+    ms_graph = g0.elapsed_time(g1)
+
+    # ---------------- end to end through the host-buffer entry points: every step copies its inputs H2D from
+    # pinned memory and reads its result (the new state) back D2H
+    hp, hv = torch.from_numpy(p.pos).pin_memory(), torch.from_numpy(p.vel).pin_memory()
+    ho_p, ho_v = torch.empty_like(hp).pin_memory(), torch.empty_like(hv).pin_memory()
+    for _ in range(2):
+        pn.pn_set_state_host(hp, hv)
+        pn.pn_step(p.dt, 1)
+        pn.pn_get_state_host(ho_p, ho_v)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        pn.pn_set_state_host(hp, hv)
+        pn.pn_step(p.dt, 1)
+        pn.pn_get_state_host(ho_p, ho_v)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+
+    # ---------------- max over ranks, whole-job aggregate
+    pairs_per_step = 4 * p.pairs_per_eval
+    t = torch.tensor([ms_total, ms_steps, e2e_s, ms_graph], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total_m, ms_steps_m, e2e_m, ms_graph_m = t.tolist()
+    value = world * K * pairs_per_step / (ms_total_m * 1e-3)
+    e2e_val = world * K * pairs_per_step / e2e_m
+
+    if rank == 0:
+        peaks = load_peaks()
+        sm_max = peaks.get("sm_max_mhz", 1965.0)
+        peak_tflops = SMS * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+        pair_avg_ms = pair_ms / max(1, pair_n)
+        achieved = p.pairs_per_eval * FLOPS_PER_PAIR / (pair_avg_ms * 1e-3) / 1e12 if pair_n else None
+        roof = {
+            "bound": "alu", "kernel": "pair_fp64_kernel", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+            "frac": (achieved / peak_tflops) if achieved else None, "traffic": None,
+            "convention": f"{FP64_INSTR_PER_PAIR} FP64-pipe instructions per ordered pair in the shipped SASS, each counted as an "
+                          f"FMA (2 flops) = FP64-pipe issue-slot utilisation; peak = {SMS} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x "
+                          f"{sm_max:.0f} MHz (clocks.max.sm; no measured fp64 peak in MEASURED_PEAKS.json)",
+            "pairs_per_launch": p.pairs_per_eval, "avg_launch_ms": pair_avg_ms, "launches_timed": pair_n,
+            "pair_kernel_share_of_steps": pair_ms / ms_steps if ms_steps else None,
+            "kernel_pairs_per_s": p.pairs_per_eval / (pair_avg_ms * 1e-3) if pair_n else None,
+            "frac_at_sampled_clock": (achieved / (peak_tflops * clocks["sm_mhz"] / sm_max)) if achieved and clocks.get("sm_mhz") else None,
+            "executed_flops_frac": (achieved * 24.0 / 30.0 / peak_tflops) if achieved else None,
+        }
+        base = cpu_baseline(p) if not args.no_cpu_baseline else None
+        line = {
+            "metric": "fp64 pair-interactions/s", "value": value, "unit": "pair-interactions/s", "n_gpus": world,
+            "steps": K, "warmup": W, "ms_per_step": ms_total_m / K, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(p, args),
+            "steps_per_s": world * K / (ms_total_m * 1e-3), "rk4_only_ms_per_step": ms_steps_m / K,
+            "energy_ms_per_eval": ms_energy / 2, "graph_ms_per_step": ms_graph_m / K,
+            "graph_pairs_per_s": world * K * pairs_per_step / (ms_graph_m * 1e-3),
+            "energy_drift": (e_end - e_start) / abs(e_start), "pair_config": cfg,
+            "clocks": clocks,
+            "e2e": {"value": e2e_val, "unit": "pair-interactions/s", "h2d_bytes_per_step": 2 * p.N * 24,
+                    "d2h_bytes_per_step": 2 * p.N * 24, "ms_per_step": 1e3 * e2e_m / K,
+                    "api": "pn_set_state_host + pn_step + pn_get_state_host per step, pinned host buffers"},
+            "gpu_launches": launches, "roofline": roof, "cpu_baseline": base,
+        }
+        print(json.dumps(line), flush=True)
+    pn.pn_destroy()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config2")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

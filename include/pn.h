@@ -1,0 +1,101 @@
+/*
+ * pn.h -- C-ABI of libpn.so: the limited first-order post-Newtonian (1PN) N-body hot path of
+ * arXiv:1801.07986 (Tatekawa) on one NVIDIA B200 (sm_100a).
+ *
+ * Citations are /root/reference/PAPER.md:<line> (+ equation).  Notation: body 0 is the paper's
+ * massive object "#1" (mass M); bodies 1..N-1 are the low-mass stars i, j.
+ * x_ab = x_a - x_b, r_ab = |x_ab|, n_ab = x_ab / r_ab (reading R1);
+ * rho_ij = sqrt(r_ij^2 + eps^2) between stars only (Eq. 4.2).
+ *
+ * What one force evaluation computes (the "hot path"; the Cross terms, Eqs. 2.3 and 2.6, are
+ * outside it -- DESIGN.md "Scope"):
+ *   a_1 = sum_j (G m_j / r_1j^3) { -x_1j + (1/c^2)[ (5 G M / r_1j - 2 v_j^2 + (3/2)(v_j.n_1j)^2) x_1j
+ *                                                   + 3 (v_j.x_1j) v_j ] }      PAPER.md:43-49, Eqs. 2.1, 2.2
+ *   a_i = - G M x_i1 / r_i1^3 - sum_{j != i} G m_j x_ij / rho_ij^3
+ *         + (1/c^2)(G M / r_i1^3)[ (4 G M / r_i1 - v_i^2) x_i1 + 4 (v_i.x_i1) v_i ]   PAPER.md:63-68, Eq. 2.4
+ *
+ * General rules
+ *   - Every function returns PN_OK (0) or a negative PN_E* code; pn_last_error() gives the text.
+ *   - "dev" pointers are CUDA device pointers on the context's device; "host" pointers are
+ *     ordinary host memory.  All arrays are fp64, row-major [N][3] unless stated.
+ *   - The caller owns every buffer it passes; the library copies what it needs during the call
+ *     (stream-ordered) and never retains or frees caller pointers.
+ *   - All work is enqueued on the context's stream (pn_set_stream; default: the legacy default
+ *     stream).  Calls with only device arguments are asynchronous; calls that take or return host
+ *     data synchronise that stream before returning.
+ *   - There is no CPU fallback: without a CUDA device pn_create fails with PN_ECUDA.
+ *   - Coincident bodies (BH-star distance 0, or two stars at distance 0 with eps = 0) give
+ *     inf/NaN, propagated, not trapped.  With eps = 0 the self term j = i is skipped by index.
+ */
+#ifndef PN_H_
+#define PN_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PN_OK 0
+#define PN_EINVAL (-1) /* bad argument: N < 2, null pointer, non-finite/negative mass, M <= 0, G <= 0, c <= 0 or NaN,
+                          eps < 0 or NaN, non-finite dt, nsteps < 0, unknown option/value */
+#define PN_ECUDA (-2)  /* a CUDA call failed (text in pn_last_error) or no device */
+#define PN_ESTATE (-3) /* pn_step / pn_energy / pn_get_state before any pn_set_state */
+#define PN_ENOMEM (-4) /* host or device allocation failed */
+
+/* pn_set_option keys */
+#define PN_OPT_PAIR_PRECISION 1 /* PN_FP64 (default) | PN_FP32_PAIR: arithmetic of the O(N^2) star-star pair loop */
+#define PN_OPT_USE_GRAPH 2      /* 1 (default): pn_step replays a captured CUDA graph; 0: plain launches */
+#define PN_OPT_TIME_PAIR 3      /* 1: bracket every star-star pair-kernel launch with CUDA events (forces plain
+                                   launches); read with pn_get_pair_time.  0 (default) */
+#define PN_OPT_J_SPLIT 4        /* 0 (default): automatic; > 0: force the number of j-chunks per i-tile */
+
+/* PN_OPT_PAIR_PRECISION values */
+#define PN_FP64 0      /* fp64 pair arithmetic and accumulation (parity 1e-12) */
+#define PN_FP32_PAIR 1 /* fp32 pair arithmetic on two-float positions, fp64 accumulation (parity 1e-5) */
+
+typedef struct pn_ctx pn_ctx; /* opaque; owns all internal device buffers */
+
+/* Problem statement of the paper: one massive object + N-1 stars, constants G, c and
+ * the star-star Plummer softening eps.  masses_host: N host doubles, copied; masses_host[0] = M > 0, stars >= 0.
+ * c may be +inf (pure Newtonian).  Uses the current CUDA device.  *out is set to NULL on failure. */
+int pn_create(pn_ctx** out, int64_t N, const double* masses_host, double G, double c, double softening);
+int pn_destroy(pn_ctx* ctx); /* synchronises, frees everything; NULL is allowed */
+
+int pn_set_stream(pn_ctx* ctx, void* cuda_stream); /* a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) */
+int pn_set_option(pn_ctx* ctx, int key, int value);
+
+/* Integrator state (x, v) of all N bodies.  [N][3] each. */
+int pn_set_state(pn_ctx* ctx, const double* pos_dev, const double* vel_dev);
+int pn_get_state(pn_ctx* ctx, double* pos_dev, double* vel_dev);
+int pn_set_state_host(pn_ctx* ctx, const double* pos_host, const double* vel_host); /* H2D inside; synchronous */
+int pn_get_state_host(pn_ctx* ctx, double* pos_host, double* vel_host);             /* D2H inside; synchronous */
+
+/* One force evaluation (equations above) at the given (pos, vel): acc[0] = a_1, acc[i] = a_i.  Does not read or
+ * modify the integrator state.  pos, vel, acc: [N][3]. */
+int pn_accel(pn_ctx* ctx, const double* pos_dev, const double* vel_dev, double* acc_dev);
+int pn_accel_host(pn_ctx* ctx, const double* pos_host, const double* vel_host, double* acc_host); /* synchronous */
+
+/* nsteps steps of the paper's integrator, the classical fourth-order Runge-Kutta method with
+ * fixed dt, on the internal state: y = (x, v) of all N bodies, f = (v, a(x, v)), 4 force evaluations per step,
+ * weights (1, 2, 2, 1)/6.  The stage update is fused into the kernel that finishes each force evaluation. */
+int pn_step(pn_ctx* ctx, double dt, int64_t nsteps);
+
+/* Total 1PN energy of the internal state, Eq. 2.7 with the star-star distances softened;
+ * O(N^2) pair sum in compensated fp64.  Synchronises the stream; *E_host is a host double. */
+int pn_energy(pn_ctx* ctx, double* E_host);
+
+/* Bookkeeping for benchmarks. */
+int pn_get_launch_count(pn_ctx* ctx, int64_t* n_kernels_host);          /* kernels launched (graph nodes count) */
+int pn_get_pair_time(pn_ctx* ctx, double* ms_total_host, int64_t* n_launches_host, int reset); /* PN_OPT_TIME_PAIR;
+                                                                            synchronises the stream */
+int pn_get_pair_config(pn_ctx* ctx, int32_t* cfg_host); /* 8 ints: threads/block, i per thread, j-tile, j-splits,
+                                                           grid blocks, padded N_s, FP64 instr per pair, variant */
+
+const char* pn_last_error(pn_ctx* ctx); /* ctx may be NULL: last error of a failed pn_create in this thread */
+const char* pn_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PN_H_ */

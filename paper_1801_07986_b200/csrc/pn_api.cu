@@ -1,0 +1,535 @@
+// pn_api.cu -- C-ABI (include/pn.h) of the limited-1PN hot path on B200.  Host-side orchestration only:
+// every step of the path runs in the kernels of pn_kernels.cuh.  No CPU fallback exists.
+#include "../../include/pn.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "pn_kernels.cuh"
+
+using namespace pn;
+
+namespace {
+
+constexpr int kNT = 128;        // threads per block of the pair / energy / epilogue kernels
+constexpr int kTJ = 128;        // j records per shared-memory tile
+constexpr int kGraphBatch = 16; // RK4 steps captured in the batched graph
+constexpr int kSMs = 148;       // B200
+
+thread_local std::string g_create_error;
+
+}  // namespace
+
+struct pn_ctx {
+    int64_t N = 0;
+    int n_stars = 0, np = 0;
+    double G = 0, c = 0, eps = 0, M = 0, GM = 0, inv_c2 = 0, eps2 = 0;
+    cudaStream_t stream = nullptr;
+    cudaStream_t cap_stream = nullptr;
+    std::string err;
+
+    // options
+    int precision = PN_FP64, use_graph = 1, time_pair = 0, j_split_opt = 0;
+
+    // pair-kernel launch configuration
+    int ipt = 1, n_itiles = 0, n_tiles = 0, n_split = 1, tiles_per_split = 0, max_split = 1;
+
+    // device buffers.  Two stage sets: [0] integrator state, [1] scratch for pn_accel.
+    JRec* jrec[2] = {nullptr, nullptr};
+    double* v[2] = {nullptr, nullptr};
+    BhState* bh[2] = {nullptr, nullptr};
+    double *x0 = nullptr, *v0 = nullptr, *sx = nullptr, *sv = nullptr;
+    double* part = nullptr;
+    double* bh_part = nullptr;
+    unsigned int* ticket = nullptr;
+    StepParams* prm = nullptr;
+    double *io_pos = nullptr, *io_vel = nullptr, *io_acc = nullptr;  // staging for the *_host entry points
+    ERec* erec = nullptr;
+    double *blk_prep = nullptr, *blk_pair = nullptr, *d_energy = nullptr;
+    int e_split = 1, e_tiles_per_split = 0;
+
+    bool have_state = false;
+    double dt_dev = NAN;
+
+    cudaGraphExec_t graph1 = nullptr, graphB = nullptr;
+    int graph_split = -1, graph_precision = -1;
+
+    int64_t n_launch = 0;
+    std::vector<cudaEvent_t> ev;  // pairs (start, stop)
+    size_t ev_used = 0;
+};
+
+namespace {
+
+int fail(pn_ctx* ctx, int code, const char* fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (ctx)
+        ctx->err = buf;
+    else
+        g_create_error = buf;
+    return code;
+}
+
+#define PN_CUDA(ctx, call)                                                                                  \
+    do {                                                                                                    \
+        cudaError_t e_ = (call);                                                                            \
+        if (e_ != cudaSuccess)                                                                              \
+            return fail(ctx, PN_ECUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+template <typename T>
+cudaError_t dalloc(T** p, size_t n)
+{
+    return cudaMalloc(reinterpret_cast<void**>(p), n * sizeof(T));
+}
+
+void choose_split(pn_ctx* c)
+{
+    int s = c->j_split_opt;
+    if (s <= 0) {
+        // ~16 blocks per SM keeps the tail of the last wave small; at least one tile per block
+        s = (kSMs * 16 + c->n_itiles - 1) / c->n_itiles;
+    }
+    if (s > c->n_tiles) s = c->n_tiles;
+    if (s > c->max_split) s = c->max_split;
+    if (s < 1) s = 1;
+    c->tiles_per_split = (c->n_tiles + s - 1) / s;
+    c->n_split = (c->n_tiles + c->tiles_per_split - 1) / c->tiles_per_split;
+}
+
+void destroy_graphs(pn_ctx* c)
+{
+    if (c->graph1) cudaGraphExecDestroy(c->graph1), c->graph1 = nullptr;
+    if (c->graphB) cudaGraphExecDestroy(c->graphB), c->graphB = nullptr;
+}
+
+// ---- launches ---------------------------------------------------------------------------------------------
+template <int I, bool MASK>
+void launch_pair_fp64(pn_ctx* c, int set, cudaStream_t st)
+{
+    dim3 grid(c->n_itiles, c->n_split);
+    pair_fp64_kernel<I, kNT, kTJ, MASK><<<grid, kNT, 0, st>>>(c->jrec[set], c->part, c->np, c->tiles_per_split, c->eps2);
+}
+
+int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
+{
+    if (timed) {
+        if (c->ev_used + 2 > c->ev.size()) {
+            for (int q = 0; q < 2; ++q) {
+                cudaEvent_t e;
+                PN_CUDA(c, cudaEventCreate(&e));
+                c->ev.push_back(e);
+            }
+        }
+        PN_CUDA(c, cudaEventRecord(c->ev[c->ev_used], st));
+    }
+    const bool mask = (c->eps2 == 0.0);
+    switch (c->ipt) {
+        case 4: mask ? launch_pair_fp64<4, true>(c, set, st) : launch_pair_fp64<4, false>(c, set, st); break;
+        case 2: mask ? launch_pair_fp64<2, true>(c, set, st) : launch_pair_fp64<2, false>(c, set, st); break;
+        default: mask ? launch_pair_fp64<1, true>(c, set, st) : launch_pair_fp64<1, false>(c, set, st); break;
+    }
+    PN_CUDA(c, cudaGetLastError());
+    if (timed) {
+        PN_CUDA(c, cudaEventRecord(c->ev[c->ev_used + 1], st));
+        c->ev_used += 2;
+    }
+    return PN_OK;
+}
+
+EpiArgs epi_args(pn_ctx* c, int set, double* acc_out)
+{
+    EpiArgs a;
+    a.jrec = c->jrec[set];
+    a.v = c->v[set];
+    a.part = c->part;
+    a.x0 = c->x0, a.v0 = c->v0, a.sx = c->sx, a.sv = c->sv;
+    a.bh = c->bh[set];
+    a.bh_part = c->bh_part;
+    a.ticket = c->ticket;
+    a.acc_out = acc_out;
+    a.prm = c->prm;
+    a.n_stars = c->n_stars, a.np = c->np, a.n_split = c->n_split;
+    a.GM = c->GM, a.inv_c2 = c->inv_c2;
+    return a;
+}
+
+// one classical-RK4 step = 4 x (pair kernel, fused epilogue)
+int enqueue_rk4_step(pn_ctx* c, cudaStream_t st, bool timed)
+{
+    const EpiArgs a = epi_args(c, 0, nullptr);
+    const int grid = c->np / kNT;
+    for (int stage = 0; stage < 4; ++stage) {
+        int rc = launch_pair(c, 0, st, timed);
+        if (rc) return rc;
+        epilogue_kernel<MODE_RK4, kNT><<<grid, kNT, 0, st>>>(a, stage);
+        PN_CUDA(c, cudaGetLastError());
+    }
+    return PN_OK;
+}
+
+int build_graph(pn_ctx* c, int nrep, cudaGraphExec_t* out)
+{
+    cudaGraph_t g = nullptr;
+    PN_CUDA(c, cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+    int rc = PN_OK;
+    for (int r = 0; r < nrep && rc == PN_OK; ++r) rc = enqueue_rk4_step(c, c->cap_stream, false);
+    cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
+    if (rc != PN_OK) {
+        if (g) cudaGraphDestroy(g);
+        return rc;
+    }
+    if (e != cudaSuccess) return fail(c, PN_ECUDA, "cudaStreamEndCapture failed: %s", cudaGetErrorString(e));
+    e = cudaGraphInstantiate(out, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) return fail(c, PN_ECUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e));
+    return PN_OK;
+}
+
+int check_ctx(pn_ctx* c)
+{
+    return c ? PN_OK : fail(nullptr, PN_EINVAL, "null context");
+}
+
+}  // namespace
+
+// =================================================================================================== C-ABI ==
+extern "C" {
+
+const char* pn_version(void) { return "pn-b200 0.1 (sm_100a)"; }
+
+const char* pn_last_error(pn_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c, double softening)
+{
+    if (!out) return fail(nullptr, PN_EINVAL, "pn_create: out is null");
+    *out = nullptr;
+    if (N < 2 || N > (int64_t)1 << 24) return fail(nullptr, PN_EINVAL, "pn_create: N = %lld out of range [2, 2^24]", (long long)N);
+    if (!masses) return fail(nullptr, PN_EINVAL, "pn_create: masses is null");
+    if (!(G > 0) || std::isinf(G)) return fail(nullptr, PN_EINVAL, "pn_create: G must be finite and > 0");
+    if (!(c > 0)) return fail(nullptr, PN_EINVAL, "pn_create: c must be > 0 (+inf allowed)");
+    if (!(softening >= 0) || std::isinf(softening)) return fail(nullptr, PN_EINVAL, "pn_create: softening must be finite and >= 0");
+    if (!(masses[0] > 0) || std::isinf(masses[0])) return fail(nullptr, PN_EINVAL, "pn_create: masses[0] = M must be finite and > 0");
+    for (int64_t i = 1; i < N; ++i)
+        if (!(masses[i] >= 0) || std::isinf(masses[i]))
+            return fail(nullptr, PN_EINVAL, "pn_create: masses[%lld] must be finite and >= 0", (long long)i);
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, PN_ECUDA, "pn_create: no CUDA device (this library has no CPU fallback)");
+    }
+
+    pn_ctx* ctx = new (std::nothrow) pn_ctx;
+    if (!ctx) return fail(nullptr, PN_ENOMEM, "pn_create: out of host memory");
+    ctx->N = N;
+    ctx->n_stars = (int)(N - 1);
+    ctx->G = G, ctx->c = c, ctx->eps = softening, ctx->M = masses[0];
+    ctx->GM = G * masses[0];
+    ctx->inv_c2 = std::isinf(c) ? 0.0 : 1.0 / (c * c);
+    ctx->eps2 = softening * softening;
+
+    // i per thread: larger i-tiles amortise the shared-memory broadcast; small N needs more blocks instead
+    ctx->ipt = ctx->n_stars >= 12288 ? 4 : (ctx->n_stars >= 3072 ? 2 : 1);
+    const int ti = ctx->ipt * kNT;
+    ctx->np = (ctx->n_stars + ti - 1) / ti * ti;
+    ctx->n_itiles = ctx->np / ti;
+    ctx->n_tiles = ctx->np / kTJ;
+    ctx->max_split = std::min(ctx->n_tiles, 64);
+    choose_split(ctx);
+
+#define CREATE_CUDA(call)                                                                   \
+    do {                                                                                    \
+        cudaError_t e_ = (call);                                                            \
+        if (e_ != cudaSuccess) {                                                            \
+            int code_ = (e_ == cudaErrorMemoryAllocation) ? PN_ENOMEM : PN_ECUDA;           \
+            fail(nullptr, code_, "pn_create: %s failed: %s", #call, cudaGetErrorString(e_)); \
+            pn_destroy(ctx);                                                                \
+            return code_;                                                                   \
+        }                                                                                   \
+    } while (0)
+
+    const size_t np = ctx->np;
+    CREATE_CUDA(cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
+    for (int s = 0; s < 2; ++s) {
+        CREATE_CUDA(dalloc(&ctx->jrec[s], np));
+        CREATE_CUDA(dalloc(&ctx->v[s], 3 * np));
+        CREATE_CUDA(dalloc(&ctx->bh[s], 1));
+        CREATE_CUDA(cudaMemset(ctx->v[s], 0, 3 * np * sizeof(double)));
+        CREATE_CUDA(cudaMemset(ctx->bh[s], 0, sizeof(BhState)));
+    }
+    CREATE_CUDA(dalloc(&ctx->x0, 3 * np));
+    CREATE_CUDA(dalloc(&ctx->v0, 3 * np));
+    CREATE_CUDA(dalloc(&ctx->sx, 3 * np));
+    CREATE_CUDA(dalloc(&ctx->sv, 3 * np));
+    CREATE_CUDA(dalloc(&ctx->part, (size_t)ctx->max_split * 3 * np));
+    CREATE_CUDA(dalloc(&ctx->bh_part, 3 * (np / kNT)));
+    CREATE_CUDA(dalloc(&ctx->ticket, 1));
+    CREATE_CUDA(cudaMemset(ctx->ticket, 0, sizeof(unsigned int)));
+    CREATE_CUDA(dalloc(&ctx->prm, 1));
+    CREATE_CUDA(dalloc(&ctx->io_pos, 3 * (size_t)N));
+    CREATE_CUDA(dalloc(&ctx->io_vel, 3 * (size_t)N));
+    CREATE_CUDA(dalloc(&ctx->io_acc, 3 * (size_t)N));
+    CREATE_CUDA(dalloc(&ctx->erec, np));
+    {
+        const int n_it = (int)(np / kNT);
+        int s = (kSMs * 8 + n_it - 1) / n_it;
+        s = std::max(1, std::min(s, std::min(ctx->n_tiles, 64)));
+        ctx->e_tiles_per_split = (ctx->n_tiles + s - 1) / s;
+        ctx->e_split = (ctx->n_tiles + ctx->e_tiles_per_split - 1) / ctx->e_tiles_per_split;
+        CREATE_CUDA(dalloc(&ctx->blk_prep, 4 * (size_t)n_it));
+        CREATE_CUDA(dalloc(&ctx->blk_pair, 2 * (size_t)n_it * ctx->e_split));
+        CREATE_CUDA(dalloc(&ctx->d_energy, 1));
+    }
+
+    // j records: mass constants for real stars; pad stars far away with zero mass
+    {
+        std::vector<JRec> h(np);
+        for (size_t s = 0; s < np; ++s) {
+            JRec r;
+            r.x = r.y = r.z = kPadPos;
+            const double gm = (s < (size_t)ctx->n_stars) ? G * masses[s + 1] : 0.0;
+            r.gm = gm, r.g15 = 1.5 * gm, r.g1875 = 1.875 * gm;
+            h[s] = r;
+        }
+        for (int s = 0; s < 2; ++s)
+            CREATE_CUDA(cudaMemcpy(ctx->jrec[s], h.data(), np * sizeof(JRec), cudaMemcpyHostToDevice));
+    }
+#undef CREATE_CUDA
+    *out = ctx;
+    return PN_OK;
+}
+
+int pn_destroy(pn_ctx* c)
+{
+    if (!c) return PN_OK;
+    cudaDeviceSynchronize();
+    destroy_graphs(c);
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    for (int s = 0; s < 2; ++s) cudaFree(c->jrec[s]), cudaFree(c->v[s]), cudaFree(c->bh[s]);
+    cudaFree(c->x0), cudaFree(c->v0), cudaFree(c->sx), cudaFree(c->sv);
+    cudaFree(c->part), cudaFree(c->bh_part), cudaFree(c->ticket), cudaFree(c->prm);
+    cudaFree(c->io_pos), cudaFree(c->io_vel), cudaFree(c->io_acc);
+    cudaFree(c->erec), cudaFree(c->blk_prep), cudaFree(c->blk_pair), cudaFree(c->d_energy);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+    cudaGetLastError();
+    delete c;
+    return PN_OK;
+}
+
+int pn_set_stream(pn_ctx* c, void* s)
+{
+    if (int rc = check_ctx(c)) return rc;
+    c->stream = static_cast<cudaStream_t>(s);
+    return PN_OK;
+}
+
+int pn_set_option(pn_ctx* c, int key, int value)
+{
+    if (int rc = check_ctx(c)) return rc;
+    switch (key) {
+        case PN_OPT_PAIR_PRECISION:
+            if (value != PN_FP64) return fail(c, PN_EINVAL, "pn_set_option: pair precision %d not available in this build", value);
+            c->precision = value;
+            return PN_OK;
+        case PN_OPT_USE_GRAPH:
+            if (value != 0 && value != 1) return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_USE_GRAPH takes 0 or 1");
+            c->use_graph = value;
+            return PN_OK;
+        case PN_OPT_TIME_PAIR:
+            if (value != 0 && value != 1) return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_TIME_PAIR takes 0 or 1");
+            c->time_pair = value;
+            return PN_OK;
+        case PN_OPT_J_SPLIT:
+            if (value < 0) return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_J_SPLIT must be >= 0");
+            c->j_split_opt = value;
+            choose_split(c);
+            return PN_OK;
+        default:
+            return fail(c, PN_EINVAL, "pn_set_option: unknown key %d", key);
+    }
+}
+
+int pn_set_state(pn_ctx* c, const double* pos, const double* vel)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!pos || !vel) return fail(c, PN_EINVAL, "pn_set_state: null pointer");
+    const int grid = (c->n_stars + 255) / 256;
+    pack_kernel<<<grid, 256, 0, c->stream>>>(pos, vel, c->jrec[0], c->v[0], c->x0, c->v0, c->bh[0], c->n_stars, c->np, 1);
+    PN_CUDA(c, cudaGetLastError());
+    c->n_launch += 1;
+    c->have_state = true;
+    return PN_OK;
+}
+
+int pn_get_state(pn_ctx* c, double* pos, double* vel)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!pos || !vel) return fail(c, PN_EINVAL, "pn_get_state: null pointer");
+    if (!c->have_state) return fail(c, PN_ESTATE, "pn_get_state: no state set");
+    const int grid = (c->n_stars + 255) / 256;
+    unpack_kernel<<<grid, 256, 0, c->stream>>>(c->x0, c->v0, c->bh[0], pos, vel, c->n_stars, c->np);
+    PN_CUDA(c, cudaGetLastError());
+    c->n_launch += 1;
+    return PN_OK;
+}
+
+int pn_set_state_host(pn_ctx* c, const double* pos, const double* vel)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!pos || !vel) return fail(c, PN_EINVAL, "pn_set_state_host: null pointer");
+    const size_t bytes = 3 * (size_t)c->N * sizeof(double);
+    PN_CUDA(c, cudaMemcpyAsync(c->io_pos, pos, bytes, cudaMemcpyHostToDevice, c->stream));
+    PN_CUDA(c, cudaMemcpyAsync(c->io_vel, vel, bytes, cudaMemcpyHostToDevice, c->stream));
+    if (int rc = pn_set_state(c, c->io_pos, c->io_vel)) return rc;
+    PN_CUDA(c, cudaStreamSynchronize(c->stream));
+    return PN_OK;
+}
+
+int pn_get_state_host(pn_ctx* c, double* pos, double* vel)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!pos || !vel) return fail(c, PN_EINVAL, "pn_get_state_host: null pointer");
+    if (int rc = pn_get_state(c, c->io_pos, c->io_vel)) return rc;
+    const size_t bytes = 3 * (size_t)c->N * sizeof(double);
+    PN_CUDA(c, cudaMemcpyAsync(pos, c->io_pos, bytes, cudaMemcpyDeviceToHost, c->stream));
+    PN_CUDA(c, cudaMemcpyAsync(vel, c->io_vel, bytes, cudaMemcpyDeviceToHost, c->stream));
+    PN_CUDA(c, cudaStreamSynchronize(c->stream));
+    return PN_OK;
+}
+
+int pn_accel(pn_ctx* c, const double* pos, const double* vel, double* acc)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!pos || !vel || !acc) return fail(c, PN_EINVAL, "pn_accel: null pointer");
+    const int grid_pack = (c->n_stars + 255) / 256;
+    pack_kernel<<<grid_pack, 256, 0, c->stream>>>(pos, vel, c->jrec[1], c->v[1], nullptr, nullptr, c->bh[1], c->n_stars, c->np, 0);
+    PN_CUDA(c, cudaGetLastError());
+    if (int rc = launch_pair(c, 1, c->stream, c->time_pair != 0)) return rc;
+    const EpiArgs a = epi_args(c, 1, acc);
+    epilogue_kernel<MODE_ACCEL, kNT><<<c->np / kNT, kNT, 0, c->stream>>>(a, 0);
+    PN_CUDA(c, cudaGetLastError());
+    c->n_launch += 3;
+    return PN_OK;
+}
+
+int pn_accel_host(pn_ctx* c, const double* pos, const double* vel, double* acc)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!pos || !vel || !acc) return fail(c, PN_EINVAL, "pn_accel_host: null pointer");
+    const size_t bytes = 3 * (size_t)c->N * sizeof(double);
+    PN_CUDA(c, cudaMemcpyAsync(c->io_pos, pos, bytes, cudaMemcpyHostToDevice, c->stream));
+    PN_CUDA(c, cudaMemcpyAsync(c->io_vel, vel, bytes, cudaMemcpyHostToDevice, c->stream));
+    if (int rc = pn_accel(c, c->io_pos, c->io_vel, c->io_acc)) return rc;
+    PN_CUDA(c, cudaMemcpyAsync(acc, c->io_acc, bytes, cudaMemcpyDeviceToHost, c->stream));
+    PN_CUDA(c, cudaStreamSynchronize(c->stream));
+    return PN_OK;
+}
+
+int pn_step(pn_ctx* c, double dt, int64_t nsteps)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!std::isfinite(dt)) return fail(c, PN_EINVAL, "pn_step: dt must be finite");
+    if (nsteps < 0) return fail(c, PN_EINVAL, "pn_step: nsteps must be >= 0");
+    if (!c->have_state) return fail(c, PN_ESTATE, "pn_step: no state set (call pn_set_state first)");
+    if (nsteps == 0) return PN_OK;
+    if (!(dt == c->dt_dev)) {
+        StepParams p;
+        p.dt = dt;
+        PN_CUDA(c, cudaMemcpyAsync(c->prm, &p, sizeof p, cudaMemcpyHostToDevice, c->stream));
+        PN_CUDA(c, cudaStreamSynchronize(c->stream));  // p lives on this stack frame
+        c->dt_dev = dt;
+    }
+    const bool eager = !c->use_graph || c->time_pair;
+    if (eager) {
+        for (int64_t s = 0; s < nsteps; ++s)
+            if (int rc = enqueue_rk4_step(c, c->stream, c->time_pair != 0)) return rc;
+        c->n_launch += 8 * nsteps;
+        return PN_OK;
+    }
+    if (c->graph_split != c->n_split || c->graph_precision != c->precision) {
+        destroy_graphs(c);
+        c->graph_split = c->n_split, c->graph_precision = c->precision;
+    }
+    int64_t left = nsteps;
+    if (left >= kGraphBatch) {
+        if (!c->graphB)
+            if (int rc = build_graph(c, kGraphBatch, &c->graphB)) return rc;
+        for (; left >= kGraphBatch; left -= kGraphBatch) PN_CUDA(c, cudaGraphLaunch(c->graphB, c->stream));
+    }
+    if (left > 0) {
+        if (!c->graph1)
+            if (int rc = build_graph(c, 1, &c->graph1)) return rc;
+        for (; left > 0; --left) PN_CUDA(c, cudaGraphLaunch(c->graph1, c->stream));
+    }
+    c->n_launch += 8 * nsteps;
+    return PN_OK;
+}
+
+int pn_energy(pn_ctx* c, double* E)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!E) return fail(c, PN_EINVAL, "pn_energy: null pointer");
+    if (!c->have_state) return fail(c, PN_ESTATE, "pn_energy: no state set");
+    const int n_it = c->np / kNT;
+    energy_prep_kernel<kNT><<<n_it, kNT, 0, c->stream>>>(c->jrec[0], c->v[0], c->bh[0], c->erec, c->blk_prep, c->n_stars, c->np,
+                                                        c->GM, c->G, c->inv_c2);
+    PN_CUDA(c, cudaGetLastError());
+    dim3 grid(n_it, c->e_split);
+    energy_pair_kernel<kNT, kTJ><<<grid, kNT, 0, c->stream>>>(c->erec, c->blk_pair, c->n_stars, c->np, c->e_tiles_per_split,
+                                                              c->eps2, c->G, c->inv_c2);
+    PN_CUDA(c, cudaGetLastError());
+    energy_final_kernel<256><<<1, 256, 0, c->stream>>>(c->blk_prep, n_it, c->blk_pair, n_it * c->e_split, c->bh[0], c->M, c->GM,
+                                                       c->G, c->inv_c2, c->d_energy);
+    PN_CUDA(c, cudaGetLastError());
+    c->n_launch += 3;
+    PN_CUDA(c, cudaMemcpyAsync(E, c->d_energy, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    PN_CUDA(c, cudaStreamSynchronize(c->stream));
+    return PN_OK;
+}
+
+int pn_get_launch_count(pn_ctx* c, int64_t* n)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!n) return fail(c, PN_EINVAL, "pn_get_launch_count: null pointer");
+    *n = c->n_launch;
+    return PN_OK;
+}
+
+int pn_get_pair_time(pn_ctx* c, double* ms_total, int64_t* n_launches, int reset)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!ms_total || !n_launches) return fail(c, PN_EINVAL, "pn_get_pair_time: null pointer");
+    PN_CUDA(c, cudaStreamSynchronize(c->stream));
+    double tot = 0;
+    for (size_t q = 0; q + 1 < c->ev_used; q += 2) {
+        float ms = 0;
+        PN_CUDA(c, cudaEventElapsedTime(&ms, c->ev[q], c->ev[q + 1]));
+        tot += ms;
+    }
+    *ms_total = tot;
+    *n_launches = (int64_t)(c->ev_used / 2);
+    if (reset) c->ev_used = 0;
+    return PN_OK;
+}
+
+int pn_get_pair_config(pn_ctx* c, int32_t* cfg)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!cfg) return fail(c, PN_EINVAL, "pn_get_pair_config: null pointer");
+    cfg[0] = kNT, cfg[1] = c->ipt, cfg[2] = kTJ, cfg[3] = c->n_split;
+    cfg[4] = c->n_itiles * c->n_split, cfg[5] = c->np, cfg[6] = 15, cfg[7] = c->precision;
+    return PN_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,542 @@
+// pn_kernels.cuh -- sm_100a kernels of the limited-1PN hot path (arXiv:1801.07986).
+// Product code: shares nothing with oracle/.  Citations: /root/reference/PAPER.md:<line>.
+//
+// Internal data layout (all fp64, star index s = body index - 1, padded to NP):
+//   JRec  jrec[NP]      : stage position + mass constants of star s, 48 B, 16 B aligned.  This is the record the
+//                         O(N^2) pair kernel streams through shared memory; pad records have gm = 0, x = 1e100.
+//   double v[3][NP]     : stage velocity, SoA
+//   double x0/v0[3][NP] : state at the beginning of the RK4 step;  double sx/sv[3][NP] : weighted sum of k's
+//   double part[S][3][NP]: per-j-chunk partial star-star accelerations (deterministic fixed-order reduction)
+//   BhState             : the massive object's stage state, step state, k-sums (a handful of doubles)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace pn {
+
+struct __align__(16) JRec {
+    double x, y, z;  // stage position of star j
+    double gm;       // G m_j
+    double g15;      // 1.5   G m_j
+    double g1875;    // 1.875 G m_j
+};
+static_assert(sizeof(JRec) == 48, "JRec must be 48 bytes");
+
+struct BhState {
+    double xs[3], vs[3];  // stage state
+    double x0[3], v0[3];  // state at step start
+    double sx[3], sv[3];  // weighted k sums
+};
+
+struct StepParams {
+    double dt;
+};
+
+constexpr double kPadPos = 1e100;  // pad stars sit far away with zero mass: they add exactly 0 to every sum
+
+// rsqrt seed: MUFU.RSQ64H (operates on the upper 32 bits; ~2^-21 relative error, low word of the result zero)
+__device__ __forceinline__ double rsqrt_seed(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return y;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// S1: star-star Newtonian all-pairs, fp64.   a_i^SS = sum_{j != i} G m_j (x_j - x_i) / rho_ij^3
+// PAPER.md:63 (Eq. 2.4, second term; exponent 3: reading R4) with rho_ij^2 = r_ij^2 + eps^2.
+//
+// Per ordered pair: 15 FP64-pipe instructions + 1 MUFU:
+//   d = x_j - x_i (3 DADD); r2 = d.d + eps^2 (3 DFMA); y0 = MUFU.RSQ64H(r2);
+//   t = y0*y0 (DMUL, exact: y0 has 21 significant bits); e = 1 - r2*t (DFMA)              [e = O(2^-20)]
+//   rho^-3 = y0^3 (1-e)^(-3/2) = y0^3 (1 + 3/2 e + 15/8 e^2 + O(e^3 ~ 2^-60))
+//   q = G m_j (1 + 3/2 e + 15/8 e^2) = fma(e, fma(e, g1875, g15), gm) (2 DFMA, constants precomputed per j)
+//   u = t*y0 (DMUL); s = u*q (DMUL); a += s*d (3 DFMA)
+// Each thread keeps I i-particles (position + accumulator) in registers; j records are broadcast from shared
+// memory with 3 LDS.128 per j, amortised over I pairs.  grid = (i-tiles, j-splits); block (it, sp) writes the
+// partial sums of its i-tile over j-tiles [sp*tiles_per_split, (sp+1)*tiles_per_split).
+// MASK (eps == 0 only): the self pair j == i is skipped by index (it would be 0 * inf).
+// ---------------------------------------------------------------------------------------------------------
+template <int I, bool MASK>
+__device__ __forceinline__ void pair_fp64(const JRec& r, int jglob, const double (&xi)[I], const double (&yi)[I],
+                                          const double (&zi)[I], const int (&ii)[I], double (&ax)[I], double (&ay)[I],
+                                          double (&az)[I], double eps2)
+{
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        const double dx = r.x - xi[k];
+        const double dy = r.y - yi[k];
+        const double dz = r.z - zi[k];
+        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+        const double y0 = rsqrt_seed(r2);
+        const double t = y0 * y0;
+        const double e = fma(-r2, t, 1.0);
+        const double p = fma(e, r.g1875, r.g15);
+        const double q = fma(e, p, r.gm);
+        const double u = t * y0;
+        double s = u * q;
+        if (MASK) s = (jglob == ii[k]) ? 0.0 : s;
+        ax[k] = fma(s, dx, ax[k]);
+        ay[k] = fma(s, dy, ay[k]);
+        az[k] = fma(s, dz, az[k]);
+    }
+}
+
+template <int I, int NT, int TJ, bool MASK>
+__global__ void __launch_bounds__(NT) pair_fp64_kernel(const JRec* __restrict__ jrec, double* __restrict__ part, int np,
+                                                       int tiles_per_split, double eps2)
+{
+    __shared__ JRec sj[2][TJ];
+    const int tid = threadIdx.x;
+    const int i_base = blockIdx.x * (I * NT) + tid;
+
+    double xi[I], yi[I], zi[I], ax[I], ay[I], az[I];
+    int ii[I];
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        ii[k] = i_base + k * NT;
+        const JRec* p = jrec + ii[k];
+        xi[k] = p->x, yi[k] = p->y, zi[k] = p->z;
+        ax[k] = ay[k] = az[k] = 0.0;
+    }
+
+    const int n_tiles = np / TJ;
+    const int t_begin = blockIdx.y * tiles_per_split;
+    const int t_end = min(n_tiles, t_begin + tiles_per_split);
+
+    constexpr int kVecPerTile = TJ * 3;  // double2 per tile
+    auto fill = [&](int buf, int t) {
+        const double2* src = reinterpret_cast<const double2*>(jrec + (size_t)t * TJ);
+        double2* dst = reinterpret_cast<double2*>(sj[buf]);
+        for (int q = tid; q < kVecPerTile; q += NT) dst[q] = src[q];
+    };
+
+    if (t_begin < t_end) fill(0, t_begin);
+    __syncthreads();
+    for (int t = t_begin; t < t_end; ++t) {
+        const int buf = (t - t_begin) & 1;
+        if (t + 1 < t_end) fill(buf ^ 1, t + 1);  // next tile into the other buffer while this one is consumed
+        const JRec* tile = sj[buf];
+        const int j0 = t * TJ;
+#pragma unroll 4
+        for (int jj = 0; jj < TJ; ++jj) {
+            const JRec r = tile[jj];
+            pair_fp64<I, MASK>(r, j0 + jj, xi, yi, zi, ii, ax, ay, az, eps2);
+        }
+        __syncthreads();
+    }
+
+    double* out = part + (size_t)blockIdx.y * 3 * np;
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        out[ii[k]] = ax[k];
+        out[np + ii[k]] = ay[k];
+        out[2 * np + ii[k]] = az[k];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// block-wide deterministic sum of three doubles (warp shuffle tree, then warp 0 sums the warp results in order)
+// ---------------------------------------------------------------------------------------------------------
+template <int NT>
+__device__ __forceinline__ void block_sum3(double& a, double& b, double& c, double* smem /* 3 * NT/32 */)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, o);
+        b += __shfl_down_sync(0xffffffffu, b, o);
+        c += __shfl_down_sync(0xffffffffu, c, o);
+    }
+    constexpr int NW = NT / 32;
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) smem[w] = a, smem[NW + w] = b, smem[2 * NW + w] = c;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double sa = 0, sb = 0, sc = 0;
+        for (int q = 0; q < NW; ++q) sa += smem[q], sb += smem[NW + q], sc += smem[2 * NW + q];
+        a = sa, b = sb, c = sc;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// S2 + S3 + S4: per-star epilogue of one force evaluation.
+//   a_i  = sum over j-chunk partials (fixed order) + BH -> star Newtonian + 1PN
+//   a_1  = sum_i [star i -> BH, Newtonian + 1PN], block reduction + last-block fixed-order final sum
+//   MODE_ACCEL: write acc[N][3] (acc[0] = a_1).
+//   MODE_RK4 stage st: classical RK4 stage update fused onto the acceleration:
+//       k_x = v_stage, k_v = a;  st 0: s = k;  st 1, 2: s += 2k;  next stage state = y0 + {dt/2, dt/2, dt} k;
+//       st 3: y0 += dt/6 (s + k), next stage state = y0.
+// ---------------------------------------------------------------------------------------------------------
+struct EpiArgs {
+    JRec* jrec;           // stage positions (x, y, z updated in RK4 mode)
+    double* v;            // [3][NP] stage velocity
+    const double* part;   // [S][3][NP]
+    double* x0;           // [3][NP]
+    double* v0;           // [3][NP]
+    double* sx;           // [3][NP]
+    double* sv;           // [3][NP]
+    BhState* bh;          // stage/step state of the massive object
+    double* bh_part;      // [gridDim.x][3] per-block partial of a_1
+    unsigned int* ticket; // last-block detection
+    double* acc_out;      // MODE_ACCEL: [N][3]
+    const StepParams* prm;
+    int n_stars, np, n_split;
+    double GM, inv_c2;
+};
+
+enum { MODE_ACCEL = 0, MODE_RK4 = 1 };
+
+template <int MODE, int NT>
+__global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
+{
+    __shared__ double red[3 * (NT / 32)];
+    __shared__ bool is_last;
+    const int i = blockIdx.x * NT + threadIdx.x;
+    const int np = A.np;
+    const bool live = i < A.n_stars;
+
+    double b0 = 0, b1 = 0, b2 = 0;  // this star's contribution to a_1
+    double a[3] = {0, 0, 0}, vel[3] = {0, 0, 0};
+    if (live) {
+        double ss[3] = {0, 0, 0};
+        for (int s = 0; s < A.n_split; ++s) {
+            const double* p = A.part + (size_t)s * 3 * np + i;
+            ss[0] += p[0], ss[1] += p[np], ss[2] += p[2 * np];
+        }
+        const JRec rec = A.jrec[i];
+        const double x[3] = {rec.x - A.bh->xs[0], rec.y - A.bh->xs[1], rec.z - A.bh->xs[2]};  // x_i1 = x_i - x_1
+        vel[0] = A.v[i], vel[1] = A.v[np + i], vel[2] = A.v[2 * np + i];
+        const double r2 = x[0] * x[0] + x[1] * x[1] + x[2] * x[2];
+        const double r = sqrt(r2);
+        const double inv_r = 1.0 / r;
+        const double inv_r3 = inv_r * inv_r * inv_r;
+        const double v2 = vel[0] * vel[0] + vel[1] * vel[1] + vel[2] * vel[2];
+        const double vx = vel[0] * x[0] + vel[1] * x[1] + vel[2] * x[2];
+        const double GMr = A.GM * inv_r;
+        // star <- BH: -GM x/r^3 + (1/c^2)(GM/r^3)[(4GM/r - v^2) x + 4 (v.x) v]
+        const double cs = A.GM * inv_r3;
+        const double fx = -1.0 + A.inv_c2 * (4.0 * GMr - v2);
+        const double fv = A.inv_c2 * 4.0 * vx;
+        // BH <- star (x_1j = -x): (G m/r^3){ x - (1/c^2)[(5GM/r - 2v^2 + 3/2 (v.x)^2/r^2) x + 3 (v.x) v] }
+        const double cb = rec.gm * inv_r3;
+        const double gx = 1.0 - A.inv_c2 * (5.0 * GMr - 2.0 * v2 + 1.5 * vx * vx * inv_r * inv_r);
+        const double gv = -A.inv_c2 * 3.0 * vx;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) a[k] = ss[k] + cs * (fx * x[k] + fv * vel[k]);
+        b0 = cb * (gx * x[0] + gv * vel[0]);
+        b1 = cb * (gx * x[1] + gv * vel[1]);
+        b2 = cb * (gx * x[2] + gv * vel[2]);
+    }
+
+    double hh = 0, dt = 0;
+    if (MODE == MODE_RK4) {
+        dt = A.prm->dt;
+        hh = (stage == 2) ? dt : 0.5 * dt;
+    }
+    if (live) {
+        if (MODE == MODE_ACCEL) {
+            double* o = A.acc_out + 3 * (size_t)(i + 1);
+            o[0] = a[0], o[1] = a[1], o[2] = a[2];
+        } else {
+            JRec* rec = A.jrec + i;
+            double xn[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const size_t q = (size_t)k * np + i;
+                const double kx = vel[k], kv = a[k];
+                if (stage == 3) {
+                    const double xnew = A.x0[q] + dt / 6.0 * (A.sx[q] + kx);
+                    const double vnew = A.v0[q] + dt / 6.0 * (A.sv[q] + kv);
+                    A.x0[q] = xnew, A.v0[q] = vnew;
+                    xn[k] = xnew, A.v[q] = vnew;
+                } else {
+                    if (stage == 0) {
+                        A.sx[q] = kx, A.sv[q] = kv;
+                    } else {
+                        A.sx[q] += 2.0 * kx, A.sv[q] += 2.0 * kv;
+                    }
+                    xn[k] = A.x0[q] + hh * kx;
+                    A.v[q] = A.v0[q] + hh * kv;
+                }
+            }
+            rec->x = xn[0], rec->y = xn[1], rec->z = xn[2];
+        }
+    }
+
+    // ---- a_1: block partial, then the last block to finish adds the block partials in index order
+    block_sum3<NT>(b0, b1, b2, red);
+    if (threadIdx.x == 0) {
+        double* bp = A.bh_part + 3 * (size_t)blockIdx.x;
+        bp[0] = b0, bp[1] = b1, bp[2] = b2;
+        __threadfence();
+        const unsigned int t = atomicAdd(A.ticket, 1u);
+        is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    double c0 = 0, c1 = 0, c2 = 0;
+    // fixed assignment of block partials to threads, fixed tree afterwards: deterministic
+    for (int q = threadIdx.x; q < (int)gridDim.x; q += NT) {
+        const volatile double* bp = A.bh_part + 3 * (size_t)q;
+        c0 += bp[0], c1 += bp[1], c2 += bp[2];
+    }
+    __syncthreads();
+    block_sum3<NT>(c0, c1, c2, red);
+    if (threadIdx.x == 0) {
+        *A.ticket = 0;
+        const double a1[3] = {c0, c1, c2};
+        BhState* bh = A.bh;
+        if (MODE == MODE_ACCEL) {
+            A.acc_out[0] = a1[0], A.acc_out[1] = a1[1], A.acc_out[2] = a1[2];
+        } else {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const double kx = bh->vs[k], kv = a1[k];
+                if (stage == 3) {
+                    bh->x0[k] += dt / 6.0 * (bh->sx[k] + kx);
+                    bh->v0[k] += dt / 6.0 * (bh->sv[k] + kv);
+                    bh->xs[k] = bh->x0[k], bh->vs[k] = bh->v0[k];
+                } else {
+                    if (stage == 0) {
+                        bh->sx[k] = kx, bh->sv[k] = kv;
+                    } else {
+                        bh->sx[k] += 2.0 * kx, bh->sv[k] += 2.0 * kv;
+                    }
+                    bh->xs[k] = bh->x0[k] + hh * kx;
+                    bh->vs[k] = bh->v0[k] + hh * kv;
+                }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Layout conversion: user AoS [N][3] <-> internal records.  to_state: also initialise x0, v0 and the BH state.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void pack_kernel(const double* __restrict__ pos, const double* __restrict__ vel, JRec* jrec, double* v,
+                            double* x0, double* v0, BhState* bh, int n_stars, int np, int to_state)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n_stars) {
+        const double* p = pos + 3 * (size_t)(i + 1);
+        const double* w = vel + 3 * (size_t)(i + 1);
+        JRec* r = jrec + i;
+        r->x = p[0], r->y = p[1], r->z = p[2];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            v[(size_t)k * np + i] = w[k];
+            if (to_state) x0[(size_t)k * np + i] = p[k], v0[(size_t)k * np + i] = w[k];
+        }
+    }
+    if (i == 0) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            bh->xs[k] = pos[k], bh->vs[k] = vel[k];
+            if (to_state) bh->x0[k] = pos[k], bh->v0[k] = vel[k], bh->sx[k] = 0, bh->sv[k] = 0;
+        }
+    }
+}
+
+__global__ void unpack_kernel(const double* __restrict__ x0, const double* __restrict__ v0, const BhState* bh,
+                              double* __restrict__ pos, double* __restrict__ vel, int n_stars, int np)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n_stars) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            pos[3 * (size_t)(i + 1) + k] = x0[(size_t)k * np + i];
+            vel[3 * (size_t)(i + 1) + k] = v0[(size_t)k * np + i];
+        }
+    }
+    if (i == 0) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) pos[k] = bh->x0[k], vel[k] = bh->v0[k];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// S5: total 1PN energy, Eq. 2.7, regrouped:
+//   E = 1/2 M v_1^2 + sum_i e_i + (1/c^2) 1/2 G^2 M (sum_i m_i/r_1i)^2 + 1/2 sum_{i != j} Epair(i, j)
+//   e_i = 1/2 m v^2 - GMm/r + (1/c^2){3/8 m v^4 + 3/2 (GMm/r) v^2 + 1/2 G^2M^2 m/r^2
+//                                    + 1/2 (GMm/r)[3 v_1^2 - 7 v_1.v_i - (n_1i.v_1)(n_1i.v_i)]}
+//   Epair(i,j) = (G m_i m_j / rho){-1 + (1/c^2)[w_i + w_j - 7/2 v_i.v_j - 1/2 (x_ij.v_i)(x_ij.v_j)/rho^2]},
+//   w_i = 3/2 v_i^2 + G M / r_1i.
+// All sums are compensated (TwoSum): a (hi, lo) pair per thread, per block and in the final reduction.
+// ---------------------------------------------------------------------------------------------------------
+struct __align__(16) ERec {
+    double x, y, z, gm;     // position, G m_j
+    double vx, vy, vz, w;   // velocity, w_j
+};
+static_assert(sizeof(ERec) == 64, "ERec must be 64 bytes");
+
+__device__ __forceinline__ void two_sum_acc(double& hi, double& lo, double t)
+{
+    const double s = hi + t;
+    const double bb = s - hi;
+    lo += (hi - (s - bb)) + (t - bb);
+    hi = s;
+}
+
+template <int NT>
+__device__ __forceinline__ void block_sum_dd(double& hi, double& lo, double* smem /* 2*NT/32 */)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double oh = __shfl_down_sync(0xffffffffu, hi, o);
+        const double ol = __shfl_down_sync(0xffffffffu, lo, o);
+        two_sum_acc(hi, lo, oh);
+        lo += ol;
+    }
+    constexpr int NW = NT / 32;
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) smem[w] = hi, smem[NW + w] = lo;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double h = 0, lw = 0;
+        for (int q = 0; q < NW; ++q) {
+            two_sum_acc(h, lw, smem[q]);
+            lw += smem[NW + q];
+        }
+        hi = h, lo = lw;
+    }
+    __syncthreads();
+}
+
+// O(N) part: builds the ERec stream for the pair kernel and the per-block partials of sum e_i and sum m_i/r_1i.
+template <int NT>
+__global__ void __launch_bounds__(NT) energy_prep_kernel(const JRec* __restrict__ jrec, const double* __restrict__ v,
+                                                         const BhState* __restrict__ bh, ERec* __restrict__ erec,
+                                                         double* __restrict__ blk /* [grid][4]: e hi, lo; mr hi, lo */,
+                                                         int n_stars, int np, double GM, double G, double inv_c2)
+{
+    __shared__ double red[2 * (NT / 32)];
+    const int i = blockIdx.x * NT + threadIdx.x;
+    double e_hi = 0, e_lo = 0, mr = 0;
+    if (i < np) {
+        ERec o;
+        const JRec r = jrec[i];
+        o.x = r.x, o.y = r.y, o.z = r.z, o.gm = r.gm;
+        o.vx = o.vy = o.vz = o.w = 0.0;
+        if (i < n_stars) {
+            const double vv[3] = {v[i], v[np + i], v[2 * np + i]};
+            const double v1[3] = {bh->vs[0], bh->vs[1], bh->vs[2]};
+            const double d[3] = {bh->xs[0] - r.x, bh->xs[1] - r.y, bh->xs[2] - r.z};  // x_1i
+            const double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+            const double inv_r = 1.0 / sqrt(r2);
+            const double m = r.gm / G;
+            const double v2 = vv[0] * vv[0] + vv[1] * vv[1] + vv[2] * vv[2];
+            const double v12 = v1[0] * v1[0] + v1[1] * v1[1] + v1[2] * v1[2];
+            const double v1v = v1[0] * vv[0] + v1[1] * vv[1] + v1[2] * vv[2];
+            const double nv1 = (d[0] * v1[0] + d[1] * v1[1] + d[2] * v1[2]) * inv_r;
+            const double nvi = (d[0] * vv[0] + d[1] * vv[1] + d[2] * vv[2]) * inv_r;
+            const double U = GM * m * inv_r;  // G M m / r
+            o.vx = vv[0], o.vy = vv[1], o.vz = vv[2];
+            o.w = 1.5 * v2 + GM * inv_r;
+            two_sum_acc(e_hi, e_lo, 0.5 * m * v2);
+            two_sum_acc(e_hi, e_lo, -U);
+            const double pn = 0.375 * m * v2 * v2 + 1.5 * U * v2 + 0.5 * U * GM * inv_r +
+                              0.5 * U * (3.0 * v12 - 7.0 * v1v - nv1 * nvi);
+            two_sum_acc(e_hi, e_lo, inv_c2 * pn);
+            mr = m * inv_r;
+        }
+        erec[i] = o;
+    }
+    double m_hi = mr, m_lo = 0;
+    block_sum_dd<NT>(e_hi, e_lo, red);
+    block_sum_dd<NT>(m_hi, m_lo, red);
+    if (threadIdx.x == 0) {
+        double* b = blk + 4 * (size_t)blockIdx.x;
+        b[0] = e_hi, b[1] = e_lo, b[2] = m_hi, b[3] = m_lo;
+    }
+}
+
+// O(N^2) part: ordered pairs (i, j != i), each contributing 1/2 Epair.  grid = (i-tiles, j-splits).
+template <int NT, int TJ>
+__global__ void __launch_bounds__(NT) energy_pair_kernel(const ERec* __restrict__ erec, double* __restrict__ blk /* [grid][2] */,
+                                                         int n_stars, int np, int tiles_per_split, double eps2, double G,
+                                                         double inv_c2)
+{
+    __shared__ ERec sj[TJ];
+    __shared__ double red[2 * (NT / 32)];
+    const int tid = threadIdx.x;
+    const int i = blockIdx.x * NT + tid;
+    const ERec me = erec[i];
+    const double mi = me.gm / G;
+    double hi = 0, lo = 0;
+
+    const int n_tiles = np / TJ;
+    const int t_begin = blockIdx.y * tiles_per_split;
+    const int t_end = min(n_tiles, t_begin + tiles_per_split);
+    for (int t = t_begin; t < t_end; ++t) {
+        __syncthreads();
+        {
+            const double2* src = reinterpret_cast<const double2*>(erec + (size_t)t * TJ);
+            double2* dst = reinterpret_cast<double2*>(sj);
+            for (int q = tid; q < TJ * 4; q += NT) dst[q] = src[q];
+        }
+        __syncthreads();
+        const int j0 = t * TJ;
+#pragma unroll 2
+        for (int jj = 0; jj < TJ; ++jj) {
+            const ERec r = sj[jj];
+            const double dx = me.x - r.x, dy = me.y - r.y, dz = me.z - r.z;  // x_ij
+            const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+            const double y0 = rsqrt_seed(r2);
+            const double t2 = y0 * y0;
+            const double e = fma(-r2, t2, 1.0);
+            const double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1/rho to full fp64 accuracy
+            const double vv = me.vx * r.vx + me.vy * r.vy + me.vz * r.vz;
+            const double xvi = dx * me.vx + dy * me.vy + dz * me.vz;
+            const double xvj = dx * r.vx + dy * r.vy + dz * r.vz;
+            const double br = me.w + r.w - 3.5 * vv - 0.5 * xvi * xvj * (y * y);
+            double term = (mi * r.gm * y) * (-1.0 + inv_c2 * br);
+            term = (j0 + jj == i) ? 0.0 : term;
+            two_sum_acc(hi, lo, term);
+        }
+    }
+    if (i >= n_stars) hi = 0, lo = 0;
+    block_sum_dd<NT>(hi, lo, red);
+    if (tid == 0) {
+        double* b = blk + 2 * ((size_t)blockIdx.y * gridDim.x + blockIdx.x);
+        b[0] = hi, b[1] = lo;
+    }
+}
+
+// Final fixed-order reduction: one block.  out[0] = E.
+template <int NT>
+__global__ void __launch_bounds__(NT) energy_final_kernel(const double* __restrict__ blk_prep, int n_prep,
+                                                          const double* __restrict__ blk_pair, int n_pair,
+                                                          const BhState* __restrict__ bh, double M, double GM, double G,
+                                                          double inv_c2, double* __restrict__ out)
+{
+    __shared__ double red[2 * (NT / 32)];
+    double e_hi = 0, e_lo = 0, m_hi = 0, m_lo = 0, p_hi = 0, p_lo = 0;
+    for (int q = threadIdx.x; q < n_prep; q += NT) {
+        two_sum_acc(e_hi, e_lo, blk_prep[4 * q]);
+        e_lo += blk_prep[4 * q + 1];
+        two_sum_acc(m_hi, m_lo, blk_prep[4 * q + 2]);
+        m_lo += blk_prep[4 * q + 3];
+    }
+    for (int q = threadIdx.x; q < n_pair; q += NT) {
+        two_sum_acc(p_hi, p_lo, blk_pair[2 * q]);
+        p_lo += blk_pair[2 * q + 1];
+    }
+    block_sum_dd<NT>(e_hi, e_lo, red);
+    block_sum_dd<NT>(m_hi, m_lo, red);
+    block_sum_dd<NT>(p_hi, p_lo, red);
+    if (threadIdx.x == 0) {
+        const double v12 = bh->vs[0] * bh->vs[0] + bh->vs[1] * bh->vs[1] + bh->vs[2] * bh->vs[2];
+        const double smr = m_hi + m_lo;  // sum_i m_i / r_1i
+        double hi = 0, lo = 0;
+        two_sum_acc(hi, lo, e_hi);
+        lo += e_lo;
+        two_sum_acc(hi, lo, 0.5 * p_hi);  // ordered pairs were summed: 1/2
+        lo += 0.5 * p_lo;
+        two_sum_acc(hi, lo, 0.5 * M * v12);
+        two_sum_acc(hi, lo, inv_c2 * 0.5 * G * GM * smr * smr);
+        out[0] = hi + lo;
+    }
+}
+
+}  // namespace pn
