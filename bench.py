@@ -131,7 +131,7 @@ def oracle_rows(p, budget_pairs=3.0e9):
     return rows, f"4 force evaluations per step on a seeded subset of {r} of {p.n_stars} i-rows, each against all j"
 
 
-def cpu_baseline(p, target_s=12.0, max_steps=8) -> dict:
+def cpu_baseline(p, target_s=12.0, max_steps=200) -> dict:
     from oracle.pn_oracle import Oracle
 
     o = Oracle(p.mass, p.G, p.c, p.softening, kind="fast")
@@ -253,6 +253,7 @@ def run_ours(args) -> None:
     ms_total = ms_energy + ms_steps
     pair_ms, pair_n = pn.pn_get_pair_time(reset=True)
     pn.pn_set_option(binding.PN_OPT_TIME_PAIR, 0)
+    dfma_peak = pn.pn_measure_fp64_peak()  # register-only DFMA chains on this device, TFLOP/s
 
     # ---------------- same K steps through the CUDA-graph path (information: what a user gets by default)
     pn.pn_set_state(pos_d, vel_d)
@@ -308,6 +309,8 @@ def run_ours(args) -> None:
             "kernel_pairs_per_s": p.pairs_per_eval / (pair_avg_ms * 1e-3) if pair_n else None,
             "frac_at_sampled_clock": (achieved / (peak_tflops * clocks["sm_mhz"] / sm_max)) if achieved and clocks.get("sm_mhz") else None,
             "executed_flops_frac": (achieved * 24.0 / 30.0 / peak_tflops) if achieved else None,
+            "peak_measured_dfma": dfma_peak,
+            "frac_of_measured_dfma": (achieved / dfma_peak) if achieved and dfma_peak else None,
         }
         base = cpu_baseline(p) if not args.no_cpu_baseline else None
         line = {

@@ -92,6 +92,10 @@ int pn_get_pair_time(pn_ctx* ctx, double* ms_total_host, int64_t* n_launches_hos
 int pn_get_pair_config(pn_ctx* ctx, int32_t* cfg_host); /* 8 ints: threads/block, i per thread, j-tile, j-splits,
                                                            grid blocks, padded N_s, FP64 instr per pair, variant */
 
+int pn_measure_fp64_peak(pn_ctx* ctx, double* tflops_host); /* sustained FP64 FMA rate of this device from a register-only
+                                                              DFMA-chain kernel (2 flops per FMA), best of 3: the measured
+                                                              roofline denominator of the pair kernel.  Synchronous. */
+
 const char* pn_last_error(pn_ctx* ctx); /* ctx may be NULL: last error of a failed pn_create in this thread */
 const char* pn_version(void);
 

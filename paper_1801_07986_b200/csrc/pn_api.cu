@@ -97,8 +97,8 @@ void choose_split(pn_ctx* c)
 {
     int s = c->j_split_opt;
     if (s <= 0) {
-        // ~16 blocks per SM keeps the tail of the last wave small; at least one tile per block
-        s = (kSMs * 16 + c->n_itiles - 1) / c->n_itiles;
+        // ~28 blocks per SM (4 resident) keeps the tail of the last wave small; at least one tile per block
+        s = (kSMs * 28 + c->n_itiles - 1) / c->n_itiles;
     }
     if (s > c->n_tiles) s = c->n_tiles;
     if (s > c->max_split) s = c->max_split;
@@ -114,11 +114,11 @@ void destroy_graphs(pn_ctx* c)
 }
 
 // ---- launches ---------------------------------------------------------------------------------------------
-template <int I, bool MASK>
+template <int I, int JU, int MINB, bool MASK>
 void launch_pair_fp64(pn_ctx* c, int set, cudaStream_t st)
 {
     dim3 grid(c->n_itiles, c->n_split);
-    pair_fp64_kernel<I, kNT, kTJ, MASK><<<grid, kNT, 0, st>>>(c->jrec[set], c->part, c->np, c->tiles_per_split, c->eps2);
+    pair_fp64_kernel<I, JU, MINB, kNT, kTJ, MASK><<<grid, kNT, 0, st>>>(c->jrec[set], c->part, c->np, c->tiles_per_split, c->eps2);
 }
 
 int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
@@ -134,11 +134,11 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
         PN_CUDA(c, cudaEventRecord(c->ev[c->ev_used], st));
     }
     const bool mask = (c->eps2 == 0.0);
-    switch (c->ipt) {
-        case 4: mask ? launch_pair_fp64<4, true>(c, set, st) : launch_pair_fp64<4, false>(c, set, st); break;
-        case 2: mask ? launch_pair_fp64<2, true>(c, set, st) : launch_pair_fp64<2, false>(c, set, st); break;
-        default: mask ? launch_pair_fp64<1, true>(c, set, st) : launch_pair_fp64<1, false>(c, set, st); break;
-    }
+    // (i per thread, j unroll, min blocks/SM): 8 pair chains in flight per thread in both variants
+    if (c->ipt == 2)
+        mask ? launch_pair_fp64<2, 4, 4, true>(c, set, st) : launch_pair_fp64<2, 4, 4, false>(c, set, st);
+    else
+        mask ? launch_pair_fp64<1, 8, 4, true>(c, set, st) : launch_pair_fp64<1, 8, 4, false>(c, set, st);
     PN_CUDA(c, cudaGetLastError());
     if (timed) {
         PN_CUDA(c, cudaEventRecord(c->ev[c->ev_used + 1], st));
@@ -240,7 +240,7 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     ctx->eps2 = softening * softening;
 
     // i per thread: larger i-tiles amortise the shared-memory broadcast; small N needs more blocks instead
-    ctx->ipt = ctx->n_stars >= 12288 ? 4 : (ctx->n_stars >= 3072 ? 2 : 1);
+    ctx->ipt = ctx->n_stars >= 3072 ? 2 : 1;
     const int ti = ctx->ipt * kNT;
     ctx->np = (ctx->n_stars + ti - 1) / ti * ti;
     ctx->n_itiles = ctx->np / ti;
@@ -520,6 +520,34 @@ int pn_get_pair_time(pn_ctx* c, double* ms_total, int64_t* n_launches, int reset
     *ms_total = tot;
     *n_launches = (int64_t)(c->ev_used / 2);
     if (reset) c->ev_used = 0;
+    return PN_OK;
+}
+
+int pn_measure_fp64_peak(pn_ctx* c, double* tflops)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!tflops) return fail(c, PN_EINVAL, "pn_measure_fp64_peak: null pointer");
+    const int blocks = kSMs * 8, iters = 8192;
+    double* out = nullptr;
+    PN_CUDA(c, dalloc(&out, (size_t)blocks * 128));
+    cudaEvent_t a, b;
+    PN_CUDA(c, cudaEventCreate(&a));
+    PN_CUDA(c, cudaEventCreate(&b));
+    float best = 0;
+    fp64_peak_kernel<<<blocks, 128, 0, c->stream>>>(out, 64);
+    for (int rep = 0; rep < 3; ++rep) {
+        PN_CUDA(c, cudaEventRecord(a, c->stream));
+        fp64_peak_kernel<<<blocks, 128, 0, c->stream>>>(out, iters);
+        PN_CUDA(c, cudaEventRecord(b, c->stream));
+        PN_CUDA(c, cudaEventSynchronize(b));
+        float ms = 0;
+        PN_CUDA(c, cudaEventElapsedTime(&ms, a, b));
+        const float tf = (float)((double)blocks * 128 * iters * 64 * 2 / (ms * 1e-3) / 1e12);
+        if (tf > best) best = tf;
+    }
+    c->n_launch += 4;
+    cudaEventDestroy(a), cudaEventDestroy(b), cudaFree(out);
+    *tflops = best;
     return PN_OK;
 }
 

@@ -57,35 +57,85 @@ __device__ __forceinline__ double rsqrt_seed(double x)
 // partial sums of its i-tile over j-tiles [sp*tiles_per_split, (sp+1)*tiles_per_split).
 // MASK (eps == 0 only): the self pair j == i is skipped by index (it would be 0 * inf).
 // ---------------------------------------------------------------------------------------------------------
-template <int I, bool MASK>
-__device__ __forceinline__ void pair_fp64(const JRec& r, int jglob, const double (&xi)[I], const double (&yi)[I],
-                                          const double (&zi)[I], const int (&ii)[I], double (&ax)[I], double (&ay)[I],
-                                          double (&az)[I], double eps2)
+// The I x JU pairs of one inner-loop trip are evaluated stage by stage (all subtractions, then all r2, ...), so
+// that dependent FP64 instructions of one pair are separated by the same stage of the other pairs: DFMA latency
+// is hidden inside the warp and consecutive instructions share operands (x_j, g15, g1875, gm, s) in the same
+// slot, which the operand-reuse cache needs (a DFMA with three distinct register operands costs 3 issue cycles
+// on sm_100a instead of 2 -- measured).
+template <int I, int JU, bool MASK>
+__device__ __forceinline__ void pairs_fp64(const JRec* __restrict__ tile, int jj, int jglob, const double (&xi)[I],
+                                           const double (&yi)[I], const double (&zi)[I], const int (&ii)[I],
+                                           double (&ax)[I], double (&ay)[I], double (&az)[I], double eps2)
 {
+    JRec r[JU];
 #pragma unroll
-    for (int k = 0; k < I; ++k) {
-        const double dx = r.x - xi[k];
-        const double dy = r.y - yi[k];
-        const double dz = r.z - zi[k];
-        const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
-        const double y0 = rsqrt_seed(r2);
-        const double t = y0 * y0;
-        const double e = fma(-r2, t, 1.0);
-        const double p = fma(e, r.g1875, r.g15);
-        const double q = fma(e, p, r.gm);
-        const double u = t * y0;
-        double s = u * q;
-        if (MASK) s = (jglob == ii[k]) ? 0.0 : s;
-        ax[k] = fma(s, dx, ax[k]);
-        ay[k] = fma(s, dy, ay[k]);
-        az[k] = fma(s, dz, az[k]);
-    }
+    for (int u = 0; u < JU; ++u) r[u] = tile[jj + u];
+    double dx[JU][I], dy[JU][I], dz[JU][I], r2[JU][I], y0[JU][I], t[JU][I], e[JU][I], s[JU][I];
+#pragma unroll
+    for (int u = 0; u < JU; ++u)
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            dx[u][k] = r[u].x - xi[k];
+            dy[u][k] = r[u].y - yi[k];
+            dz[u][k] = r[u].z - zi[k];
+        }
+#pragma unroll
+    for (int u = 0; u < JU; ++u)
+#pragma unroll
+        for (int k = 0; k < I; ++k) r2[u][k] = fma(dz[u][k], dz[u][k], eps2);
+#pragma unroll
+    for (int u = 0; u < JU; ++u)
+#pragma unroll
+        for (int k = 0; k < I; ++k) r2[u][k] = fma(dy[u][k], dy[u][k], r2[u][k]);
+#pragma unroll
+    for (int u = 0; u < JU; ++u)
+#pragma unroll
+        for (int k = 0; k < I; ++k) r2[u][k] = fma(dx[u][k], dx[u][k], r2[u][k]);
+#pragma unroll
+    for (int u = 0; u < JU; ++u)
+#pragma unroll
+        for (int k = 0; k < I; ++k) y0[u][k] = rsqrt_seed(r2[u][k]);
+#pragma unroll
+    for (int u = 0; u < JU; ++u)
+#pragma unroll
+        for (int k = 0; k < I; ++k) t[u][k] = y0[u][k] * y0[u][k];
+#pragma unroll
+    for (int u = 0; u < JU; ++u)
+#pragma unroll
+        for (int k = 0; k < I; ++k) e[u][k] = fma(-r2[u][k], t[u][k], 1.0);
+#pragma unroll
+    for (int u = 0; u < JU; ++u)
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            t[u][k] = t[u][k] * y0[u][k];                        // y0^3
+            s[u][k] = fma(e[u][k], r[u].g1875, r[u].g15);        // G m_j (3/2 + 15/8 e)
+        }
+#pragma unroll
+    for (int u = 0; u < JU; ++u)
+#pragma unroll
+        for (int k = 0; k < I; ++k) s[u][k] = fma(e[u][k], s[u][k], r[u].gm);  // G m_j (1 + 3/2 e + 15/8 e^2)
+#pragma unroll
+    for (int u = 0; u < JU; ++u)
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            s[u][k] = s[u][k] * t[u][k];  // G m_j / rho^3
+            if (MASK) s[u][k] = (jglob + u == ii[k]) ? 0.0 : s[u][k];
+        }
+#pragma unroll
+    for (int u = 0; u < JU; ++u)
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            ax[k] = fma(s[u][k], dx[u][k], ax[k]);
+            ay[k] = fma(s[u][k], dy[u][k], ay[k]);
+            az[k] = fma(s[u][k], dz[u][k], az[k]);
+        }
 }
 
-template <int I, int NT, int TJ, bool MASK>
-__global__ void __launch_bounds__(NT) pair_fp64_kernel(const JRec* __restrict__ jrec, double* __restrict__ part, int np,
-                                                       int tiles_per_split, double eps2)
+template <int I, int JU, int MINB, int NT, int TJ, bool MASK>
+__global__ void __launch_bounds__(NT, MINB) pair_fp64_kernel(const JRec* __restrict__ jrec, double* __restrict__ part,
+                                                             int np, int tiles_per_split, double eps2)
 {
+    static_assert(TJ % JU == 0, "tile must be a multiple of the j unroll");
     __shared__ JRec sj[2][TJ];
     const int tid = threadIdx.x;
     const int i_base = blockIdx.x * (I * NT) + tid;
@@ -118,11 +168,8 @@ __global__ void __launch_bounds__(NT) pair_fp64_kernel(const JRec* __restrict__ 
         if (t + 1 < t_end) fill(buf ^ 1, t + 1);  // next tile into the other buffer while this one is consumed
         const JRec* tile = sj[buf];
         const int j0 = t * TJ;
-#pragma unroll 4
-        for (int jj = 0; jj < TJ; ++jj) {
-            const JRec r = tile[jj];
-            pair_fp64<I, MASK>(r, j0 + jj, xi, yi, zi, ii, ax, ay, az, eps2);
-        }
+#pragma unroll 1
+        for (int jj = 0; jj < TJ; jj += JU) pairs_fp64<I, JU, MASK>(tile, jj, j0 + jj, xi, yi, zi, ii, ax, ay, az, eps2);
         __syncthreads();
     }
 
@@ -133,6 +180,25 @@ __global__ void __launch_bounds__(NT) pair_fp64_kernel(const JRec* __restrict__ 
         out[np + ii[k]] = ay[k];
         out[2 * np + ii[k]] = az[k];
     }
+}
+
+// Register-only DFMA chains: measures the sustained FP64 FMA rate of the device (roofline denominator).
+__global__ void __launch_bounds__(128) fp64_peak_kernel(double* out, int iters)
+{
+    double a[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) a[q] = threadIdx.x * 1e-9 + q;
+    const double m = 1.0000001, c = 1e-9;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+#pragma unroll
+            for (int q = 0; q < 8; ++q) a[q] = fma(a[q], m, c);
+    }
+    double s = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) s += a[q];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
 // ---------------------------------------------------------------------------------------------------------
