@@ -50,6 +50,7 @@ struct pn_ctx {
     StepParams* prm = nullptr;
     double *io_pos = nullptr, *io_vel = nullptr, *io_acc = nullptr;  // staging for the *_host entry points
     ERec* erec = nullptr;
+    FRec* frec = nullptr;  // two-float records of the fp32-pair variant, rebuilt before every pair launch
     double *blk_prep = nullptr, *blk_pair = nullptr, *d_energy = nullptr;
     int e_split = 1, e_tiles_per_split = 0;
 
@@ -134,8 +135,18 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
         PN_CUDA(c, cudaEventRecord(c->ev[c->ev_used], st));
     }
     const bool mask = (c->eps2 == 0.0);
-    // (i per thread, j unroll, min blocks/SM): 8 pair chains in flight per thread in both variants
-    if (c->ipt == 2)
+    if (c->precision == PN_FP32_PAIR) {
+        split_kernel<<<(c->np + 255) / 256, 256, 0, st>>>(c->jrec[set], c->frec, c->n_stars, c->np);
+        PN_CUDA(c, cudaGetLastError());
+        dim3 grid(c->n_itiles, c->n_split);
+        const float e2 = (float)c->eps2;
+        if (c->ipt == 2)
+            mask ? pair_fp32_kernel<2, kNT, kTJ, 32, true><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2)
+                 : pair_fp32_kernel<2, kNT, kTJ, 32, false><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2);
+        else
+            mask ? pair_fp32_kernel<1, kNT, kTJ, 32, true><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2)
+                 : pair_fp32_kernel<1, kNT, kTJ, 32, false><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2);
+    } else if (c->ipt == 2)
         mask ? launch_pair_fp64<2, 4, 4, true>(c, set, st) : launch_pair_fp64<2, 4, 4, false>(c, set, st);
     else
         mask ? launch_pair_fp64<1, 8, 4, true>(c, set, st) : launch_pair_fp64<1, 8, 4, false>(c, set, st);
@@ -168,7 +179,7 @@ EpiArgs epi_args(pn_ctx* c, int set, double* acc_out)
 int enqueue_rk4_step(pn_ctx* c, cudaStream_t st, bool timed)
 {
     const EpiArgs a = epi_args(c, 0, nullptr);
-    const int grid = c->np / kNT;
+    const int grid = c->np / (kNT / kEpiG);
     for (int stage = 0; stage < 4; ++stage) {
         int rc = launch_pair(c, 0, st, timed);
         if (rc) return rc;
@@ -273,7 +284,7 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA(dalloc(&ctx->sx, 3 * np));
     CREATE_CUDA(dalloc(&ctx->sv, 3 * np));
     CREATE_CUDA(dalloc(&ctx->part, (size_t)ctx->max_split * 3 * np));
-    CREATE_CUDA(dalloc(&ctx->bh_part, 3 * (np / kNT)));
+    CREATE_CUDA(dalloc(&ctx->bh_part, 3 * (np / (kNT / kEpiG))));
     CREATE_CUDA(dalloc(&ctx->ticket, 1));
     CREATE_CUDA(cudaMemset(ctx->ticket, 0, sizeof(unsigned int)));
     CREATE_CUDA(dalloc(&ctx->prm, 1));
@@ -281,6 +292,7 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA(dalloc(&ctx->io_vel, 3 * (size_t)N));
     CREATE_CUDA(dalloc(&ctx->io_acc, 3 * (size_t)N));
     CREATE_CUDA(dalloc(&ctx->erec, np));
+    CREATE_CUDA(dalloc(&ctx->frec, np));
     {
         const int n_it = (int)(np / kNT);
         int s = (kSMs * 8 + n_it - 1) / n_it;
@@ -320,7 +332,7 @@ int pn_destroy(pn_ctx* c)
     cudaFree(c->x0), cudaFree(c->v0), cudaFree(c->sx), cudaFree(c->sv);
     cudaFree(c->part), cudaFree(c->bh_part), cudaFree(c->ticket), cudaFree(c->prm);
     cudaFree(c->io_pos), cudaFree(c->io_vel), cudaFree(c->io_acc);
-    cudaFree(c->erec), cudaFree(c->blk_prep), cudaFree(c->blk_pair), cudaFree(c->d_energy);
+    cudaFree(c->frec), cudaFree(c->erec), cudaFree(c->blk_prep), cudaFree(c->blk_pair), cudaFree(c->d_energy);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     cudaGetLastError();
     delete c;
@@ -339,7 +351,7 @@ int pn_set_option(pn_ctx* c, int key, int value)
     if (int rc = check_ctx(c)) return rc;
     switch (key) {
         case PN_OPT_PAIR_PRECISION:
-            if (value != PN_FP64) return fail(c, PN_EINVAL, "pn_set_option: pair precision %d not available in this build", value);
+            if (value != PN_FP64 && value != PN_FP32_PAIR) return fail(c, PN_EINVAL, "pn_set_option: unknown pair precision %d", value);
             c->precision = value;
             return PN_OK;
         case PN_OPT_USE_GRAPH:
@@ -417,9 +429,9 @@ int pn_accel(pn_ctx* c, const double* pos, const double* vel, double* acc)
     PN_CUDA(c, cudaGetLastError());
     if (int rc = launch_pair(c, 1, c->stream, c->time_pair != 0)) return rc;
     const EpiArgs a = epi_args(c, 1, acc);
-    epilogue_kernel<MODE_ACCEL, kNT><<<c->np / kNT, kNT, 0, c->stream>>>(a, 0);
+    epilogue_kernel<MODE_ACCEL, kNT><<<c->np / (kNT / kEpiG), kNT, 0, c->stream>>>(a, 0);
     PN_CUDA(c, cudaGetLastError());
-    c->n_launch += 3;
+    c->n_launch += (c->precision == PN_FP32_PAIR ? 4 : 3);
     return PN_OK;
 }
 
@@ -454,7 +466,7 @@ int pn_step(pn_ctx* c, double dt, int64_t nsteps)
     if (eager) {
         for (int64_t s = 0; s < nsteps; ++s)
             if (int rc = enqueue_rk4_step(c, c->stream, c->time_pair != 0)) return rc;
-        c->n_launch += 8 * nsteps;
+        c->n_launch += (c->precision == PN_FP32_PAIR ? 12 : 8) * nsteps;
         return PN_OK;
     }
     if (c->graph_split != c->n_split || c->graph_precision != c->precision) {
@@ -472,7 +484,7 @@ int pn_step(pn_ctx* c, double dt, int64_t nsteps)
             if (int rc = build_graph(c, 1, &c->graph1)) return rc;
         for (; left > 0; --left) PN_CUDA(c, cudaGraphLaunch(c->graph1, c->stream));
     }
-    c->n_launch += 8 * nsteps;
+    c->n_launch += (c->precision == PN_FP32_PAIR ? 12 : 8) * nsteps;
     return PN_OK;
 }
 
@@ -556,7 +568,7 @@ int pn_get_pair_config(pn_ctx* c, int32_t* cfg)
     if (int rc = check_ctx(c)) return rc;
     if (!cfg) return fail(c, PN_EINVAL, "pn_get_pair_config: null pointer");
     cfg[0] = kNT, cfg[1] = c->ipt, cfg[2] = kTJ, cfg[3] = c->n_split;
-    cfg[4] = c->n_itiles * c->n_split, cfg[5] = c->np, cfg[6] = 15, cfg[7] = c->precision;
+    cfg[4] = c->n_itiles * c->n_split, cfg[5] = c->np, cfg[6] = (c->precision == PN_FP32_PAIR) ? 18 : 15, cfg[7] = c->precision;
     return PN_OK;
 }
 

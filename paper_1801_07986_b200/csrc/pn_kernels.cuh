@@ -182,6 +182,117 @@ __global__ void __launch_bounds__(NT, MINB) pair_fp64_kernel(const JRec* __restr
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// S1 variant: fp32 pair arithmetic, fp64 accumulation (PN_FP32_PAIR, parity 1e-5).
+// Positions are split into two floats, hi = fl32(x), lo = fl32(x - hi), so that the pair separation
+//   d = (hi_j - hi_i) + (lo_j - lo_i)
+// keeps a relative accuracy of ~1e-7 of |d| even for close pairs (a position ~1 has fp32 spacing 6e-8 while the
+// softening is 1e-3...1e-4).  Per ordered pair: 9 FADD + 6 FFMA + 3 FMUL = 18 FP32-pipe instructions + 1 MUFU.RSQ.
+// fp32 partial sums run over FL consecutive j only and are then flushed into fp64 accumulators.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float rsqrt_seed_f32(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));  // MUFU.RSQ
+    return y;
+}
+
+struct __align__(16) FRec {
+    float xh, yh, zh, gm;  // high parts, G m_j
+    float xl, yl, zl, pad; // low parts
+};
+static_assert(sizeof(FRec) == 32, "FRec must be 32 bytes");
+
+constexpr float kPadPosF = 1e15f;  // pad stars for the fp32 kernel: finite r^2, zero mass
+
+__global__ void split_kernel(const JRec* __restrict__ jrec, FRec* __restrict__ frec, int n_stars, int np)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= np) return;
+    FRec f;
+    if (i < n_stars) {
+        const JRec r = jrec[i];
+        f.xh = (float)r.x, f.yh = (float)r.y, f.zh = (float)r.z;
+        f.xl = (float)(r.x - (double)f.xh), f.yl = (float)(r.y - (double)f.yh), f.zl = (float)(r.z - (double)f.zh);
+        f.gm = (float)r.gm;
+    } else {
+        f.xh = f.yh = f.zh = kPadPosF;
+        f.xl = f.yl = f.zl = 0.f, f.gm = 0.f;
+    }
+    f.pad = 0.f;
+    frec[i] = f;
+}
+
+template <int I, int NT, int TJ, int FL, bool MASK>
+__global__ void __launch_bounds__(NT) pair_fp32_kernel(const FRec* __restrict__ frec, double* __restrict__ part, int np,
+                                                       int tiles_per_split, float eps2)
+{
+    static_assert(TJ % FL == 0, "tile must be a multiple of the flush interval");
+    __shared__ FRec sj[2][TJ];
+    const int tid = threadIdx.x;
+    const int i_base = blockIdx.x * (I * NT) + tid;
+
+    float xh[I], yh[I], zh[I], xl[I], yl[I], zl[I];
+    double ax[I], ay[I], az[I];
+    int ii[I];
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        ii[k] = i_base + k * NT;
+        const FRec f = frec[ii[k]];
+        xh[k] = f.xh, yh[k] = f.yh, zh[k] = f.zh, xl[k] = f.xl, yl[k] = f.yl, zl[k] = f.zl;
+        ax[k] = ay[k] = az[k] = 0.0;
+    }
+    const int n_tiles = np / TJ;
+    const int t_begin = blockIdx.y * tiles_per_split;
+    const int t_end = min(n_tiles, t_begin + tiles_per_split);
+    auto fill = [&](int buf, int t) {
+        const float4* src = reinterpret_cast<const float4*>(frec + (size_t)t * TJ);
+        float4* dst = reinterpret_cast<float4*>(sj[buf]);
+        for (int q = tid; q < TJ * 2; q += NT) dst[q] = src[q];
+    };
+    if (t_begin < t_end) fill(0, t_begin);
+    __syncthreads();
+    for (int t = t_begin; t < t_end; ++t) {
+        const int buf = (t - t_begin) & 1;
+        if (t + 1 < t_end) fill(buf ^ 1, t + 1);
+        const FRec* tile = sj[buf];
+        const int j0 = t * TJ;
+#pragma unroll 1
+        for (int jb = 0; jb < TJ; jb += FL) {
+            float fx[I], fy[I], fz[I];
+#pragma unroll
+            for (int k = 0; k < I; ++k) fx[k] = fy[k] = fz[k] = 0.f;
+#pragma unroll 4
+            for (int jj = jb; jj < jb + FL; ++jj) {
+                const FRec r = tile[jj];
+#pragma unroll
+                for (int k = 0; k < I; ++k) {
+                    const float dx = (r.xh - xh[k]) + (r.xl - xl[k]);
+                    const float dy = (r.yh - yh[k]) + (r.yl - yl[k]);
+                    const float dz = (r.zh - zh[k]) + (r.zl - zl[k]);
+                    const float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, eps2)));
+                    const float y = rsqrt_seed_f32(r2);
+                    float s = (y * y) * (y * r.gm);
+                    if (MASK) s = (j0 + jj == ii[k]) ? 0.f : s;
+                    fx[k] = fmaf(s, dx, fx[k]);
+                    fy[k] = fmaf(s, dy, fy[k]);
+                    fz[k] = fmaf(s, dz, fz[k]);
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < I; ++k) ax[k] += (double)fx[k], ay[k] += (double)fy[k], az[k] += (double)fz[k];
+        }
+        __syncthreads();
+    }
+    double* out = part + (size_t)blockIdx.y * 3 * np;
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        out[ii[k]] = ax[k];
+        out[np + ii[k]] = ay[k];
+        out[2 * np + ii[k]] = az[k];
+    }
+}
+
 // Register-only DFMA chains: measures the sustained FP64 FMA rate of the device (roofline denominator).
 __global__ void __launch_bounds__(128) fp64_peak_kernel(double* out, int iters)
 {
@@ -252,23 +363,36 @@ struct EpiArgs {
 
 enum { MODE_ACCEL = 0, MODE_RK4 = 1 };
 
+constexpr int kEpiG = 8;  // threads per star in the epilogue: each sums every 8th j-chunk partial (memory parallelism)
+
 template <int MODE, int NT>
 __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
 {
     __shared__ double red[3 * (NT / 32)];
     __shared__ bool is_last;
-    const int i = blockIdx.x * NT + threadIdx.x;
+    const int i = blockIdx.x * (NT / kEpiG) + threadIdx.x / kEpiG;
+    const int g = threadIdx.x % kEpiG;
     const int np = A.np;
-    const bool live = i < A.n_stars;
+
+    // fixed-order reduction of the j-chunk partials: sub-lane g takes chunks g, g+8, ...; then a fixed shuffle tree
+    double ss[3] = {0, 0, 0};
+    if (i < A.n_stars) {
+        for (int s = g; s < A.n_split; s += kEpiG) {
+            const double* p = A.part + (size_t)s * 3 * np + i;
+            ss[0] += p[0], ss[1] += p[np], ss[2] += p[2 * np];
+        }
+    }
+#pragma unroll
+    for (int o = kEpiG / 2; o > 0; o >>= 1) {
+        ss[0] += __shfl_down_sync(0xffffffffu, ss[0], o, kEpiG);
+        ss[1] += __shfl_down_sync(0xffffffffu, ss[1], o, kEpiG);
+        ss[2] += __shfl_down_sync(0xffffffffu, ss[2], o, kEpiG);
+    }
+    const bool live = (g == 0) && (i < A.n_stars);
 
     double b0 = 0, b1 = 0, b2 = 0;  // this star's contribution to a_1
     double a[3] = {0, 0, 0}, vel[3] = {0, 0, 0};
     if (live) {
-        double ss[3] = {0, 0, 0};
-        for (int s = 0; s < A.n_split; ++s) {
-            const double* p = A.part + (size_t)s * 3 * np + i;
-            ss[0] += p[0], ss[1] += p[np], ss[2] += p[2 * np];
-        }
         const JRec rec = A.jrec[i];
         const double x[3] = {rec.x - A.bh->xs[0], rec.y - A.bh->xs[1], rec.z - A.bh->xs[2]};  // x_i1 = x_i - x_1
         vel[0] = A.v[i], vel[1] = A.v[np + i], vel[2] = A.v[2 * np + i];

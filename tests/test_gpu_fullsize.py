@@ -1,0 +1,165 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (automatic j-split),
+on sampled outputs the oracle can compute one by one (seeded subsets of i-rows, each against ALL j, plus the
+BH row), and the fp32-pair / fp64-accumulate variant (tolerance 1e-5)."""
+import numpy as np
+import pytest
+
+from oracle.pn_oracle import Oracle
+from paper_1801_07986_b200 import inputs
+from tests.conftest import rel_err_rows
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL_ACC = 1e-12
+TOL_FP32 = 1e-5
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _sample_rows(p, n, seed=4242):
+    rng = np.random.default_rng(seed)
+    rows = rng.choice(np.arange(1, p.N), size=min(n, p.n_stars), replace=False)
+    # always include the BH, the first/last star and the stars closest to the BH and to another star's tile edge
+    r = np.linalg.norm(p.pos[1:] - p.pos[0], axis=1)
+    extra = [0, 1, p.N - 1, 1 + int(np.argmin(r)), 1 + int(np.argmax(r)), 128, 129, 256, 257]
+    return np.unique(np.concatenate([rows, [e for e in extra if e < p.N]])).astype(np.int64)
+
+
+def _check_sampled(p, n_rows, precision=None, tol=TOL_ACC):
+    from paper_1801_07986_b200 import PN, binding
+
+    rows = _sample_rows(p, n_rows)
+    ref = Oracle(p.mass, p.G, p.c, p.softening).accel_rows(p.pos, p.vel, rows)
+    with PN(p.mass, p.G, p.c, p.softening) as pn:
+        if precision is not None:
+            pn.pn_set_option(binding.PN_OPT_PAIR_PRECISION, precision)
+        acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
+        cfg = pn.pn_get_pair_config()
+    assert np.isfinite(acc).all()
+    err = rel_err_rows(acc[rows], ref)
+    assert err.max() <= tol, (cfg, float(err.max()))
+    return acc
+
+
+# ------------------------------------------------------------------ fp64, full sizes
+def test_config2_full_size_sampled_rows():
+    _check_sampled(inputs.config(2), 512)
+
+
+def test_config3_cusp_full_size_sampled_rows():
+    _check_sampled(inputs.config(3), 512)
+
+
+def test_config4_full_size_sampled_rows():
+    _check_sampled(inputs.config(4), 256)
+
+
+@pytest.mark.parametrize("k", [10, 14, 17])
+def test_config5_sweep_sampled_rows(k):
+    _check_sampled(inputs.uniform_ball_bh(k), 256)
+
+
+def test_config2_newton_third_law_property_at_full_size():
+    """Property that holds at any size (no oracle needed): with c = inf, M a_1 + sum m_i a_i = 0 to rounding."""
+    from paper_1801_07986_b200 import PN
+
+    p = inputs.config(2)
+    with PN(p.mass, p.G, float("inf"), p.softening) as pn:
+        acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
+    f = (p.mass[:, None] * acc).sum(0)
+    fabs = (p.mass[:, None] * np.abs(acc)).sum(0)
+    assert np.all(np.abs(f) <= 1e-13 * fabs)
+
+
+def test_config2_energy_and_short_run_drift():
+    """Config 2: full-size energy against the oracle and 3 RK4 steps of drift (the oracle's O(N^2) long-double
+    energy takes a few seconds per call at this size)."""
+    from paper_1801_07986_b200 import PN
+
+    p = inputs.config(2)
+    o = Oracle(p.mass, p.G, p.c, p.softening)
+    with PN(p.mass, p.G, p.c, p.softening) as pn:
+        pn.pn_set_state_host(p.pos, p.vel)
+        e0 = pn.pn_energy()
+        e0_ref = o.energy(p.pos, p.vel)
+        assert e0 == pytest.approx(e0_ref, rel=1e-13)
+        pn.pn_step(p.dt, 3)
+        x, v = pn.pn_get_state_host()
+        e1 = pn.pn_energy()
+    xr, vr = o.step(p.pos, p.vel, p.dt, 3)
+    assert rel_err_rows(x, xr).max() <= 1e-12 and rel_err_rows(v, vr).max() <= 1e-11
+    e1_ref = o.energy(xr, vr)
+    assert abs((e1 - e0) / abs(e0) - (e1_ref - e0_ref) / abs(e0_ref)) <= 1e-10
+
+
+def test_config3_energy_full_size():
+    """Config 3 (4.3e9 ordered pairs): energy against the oracle's double build (same source, -DORACLE_FAST;
+    the long-double build would take minutes)."""
+    from paper_1801_07986_b200 import PN
+
+    p = inputs.config(3)
+    ref = Oracle(p.mass, p.G, p.c, p.softening, kind="fast").energy(p.pos, p.vel)
+    with PN(p.mass, p.G, p.c, p.softening) as pn:
+        pn.pn_set_state_host(p.pos, p.vel)
+        e = pn.pn_energy()
+    assert e == pytest.approx(ref, rel=1e-12)
+
+
+# ------------------------------------------------------------------ fp32-pair / fp64-accumulate variant
+@pytest.mark.parametrize("n_stars", [2, 129, 1023, 4099, 13001])
+def test_fp32_pair_variant_parity(n_stars):
+    from paper_1801_07986_b200 import binding
+
+    if n_stars == 2:  # two equal-mass recentred stars make a_1 pure rounding noise: use unequal masses instead
+        p = inputs.random_small(2, seed=302, M=1.0, m_scale=1e-2, c=10.0, softening=1e-3)
+    else:
+        p = inputs.plummer_bh(n_stars, seed=300 + n_stars)
+    _check_sampled(p, 4096, precision=binding.PN_FP32_PAIR, tol=TOL_FP32)
+
+
+def test_fp32_pair_variant_cusp_and_zero_softening():
+    from paper_1801_07986_b200 import binding
+
+    _check_sampled(inputs.cusp_bh(6000, seed=2), 6000, precision=binding.PN_FP32_PAIR, tol=TOL_FP32)
+    p = inputs.random_small(500, seed=31, M=1.0, m_scale=1e-3, c=20.0, softening=0.0)
+    _check_sampled(p, 500, precision=binding.PN_FP32_PAIR, tol=TOL_FP32)
+
+
+def test_fp32_pair_variant_full_size_config2_and_switching_back():
+    from paper_1801_07986_b200 import PN, binding
+
+    p = inputs.config(2)
+    rows = _sample_rows(p, 512)
+    ref = Oracle(p.mass, p.G, p.c, p.softening).accel_rows(p.pos, p.vel, rows)
+    with PN(p.mass, p.G, p.c, p.softening) as pn:
+        pos, vel = _dev(p.pos), _dev(p.vel)
+        a64 = pn.pn_accel(pos, vel).cpu().numpy()
+        pn.pn_set_option(binding.PN_OPT_PAIR_PRECISION, binding.PN_FP32_PAIR)
+        a32 = pn.pn_accel(pos, vel).cpu().numpy()
+        pn.pn_set_option(binding.PN_OPT_PAIR_PRECISION, binding.PN_FP64)
+        a64b = pn.pn_accel(pos, vel).cpu().numpy()
+    assert np.array_equal(a64, a64b)
+    assert rel_err_rows(a64[rows], ref).max() <= TOL_ACC
+    e32 = rel_err_rows(a32[rows], ref).max()
+    assert 1e-9 < e32 <= TOL_FP32  # it really is the fp32 path, and within its tolerance
+
+
+def test_fp32_pair_variant_rk4_run_tracks_fp64():
+    from paper_1801_07986_b200 import PN, binding
+
+    p = inputs.config(1)
+    out = {}
+    for prec in (binding.PN_FP64, binding.PN_FP32_PAIR):
+        with PN(p.mass, p.G, p.c, p.softening) as pn:
+            pn.pn_set_option(binding.PN_OPT_PAIR_PRECISION, prec)
+            pn.pn_set_state_host(p.pos, p.vel)
+            pn.pn_step(p.dt, 20)
+            out[prec] = pn.pn_get_state_host() + (pn.pn_energy(),)
+    x64, v64, e64 = out[binding.PN_FP64]
+    x32, v32, e32 = out[binding.PN_FP32_PAIR]
+    assert rel_err_rows(x32, x64).max() <= 1e-8  # acceleration error 1e-5 * (20 dt)^2 / 2
+    assert rel_err_rows(v32, v64).max() <= 1e-6
+    assert e32 == pytest.approx(e64, rel=1e-7)
