@@ -30,6 +30,9 @@ if str(ROOT) not in sys.path:
 FP64_INSTR_PER_PAIR = 15          # SASS-verified: 3 DADD + 9 DFMA + 3 DMUL per ordered pair (+1 MUFU.RSQ64H)
 FLOPS_PER_PAIR = 2 * FP64_INSTR_PER_PAIR  # issue-slot convention: every FP64-pipe instruction counted as an FMA
 SMS, FP64_LANES_PER_SM = 148, 64
+# dram__bytes_read.sum + dram__bytes_write.sum of one pair_fp64_kernel launch, from the committed ncu --set full capture
+# (profiles/r1_ncu_summary.md section 2), keyed by N_s; algorithmic bytes are the 48 B j records read once: 16384 * 48 = 786432
+NCU_DRAM_BYTES_PER_PAIR_LAUNCH = {16383: 793344}
 
 
 def load_peaks() -> dict:
@@ -106,6 +109,64 @@ class ClockSampler:
                     reasons.add(nm)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
                 "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+class NvmlSampler:
+    """Same quantities through NVML, polled every ~2 ms from a thread: the timed region of the default run lasts
+    only tens of milliseconds, too short for nvidia-smi's 100 ms loop."""
+
+    def __init__(self, index: int):
+        import pynvml
+
+        self.nv = pynvml
+        pynvml.nvmlInit()
+        try:
+            import torch
+
+            uuid = str(torch.cuda.get_device_properties(index).uuid)
+            self.h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + uuid) if not uuid.startswith("GPU-") else uuid)
+        except Exception:
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+        self.samples, self.run = [], False
+
+    def start(self):
+        self.run = True
+        self.thread = threading.Thread(target=self._poll, daemon=True)
+        self.thread.start()
+
+    def _poll(self):
+        nv = self.nv
+        while self.run:
+            try:
+                sm = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                try:
+                    rs = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    rs = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                pw = nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+                self.samples.append((time.perf_counter(), sm, rs, pw))
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def stop(self, t0: float, t1: float) -> dict:
+        nv = self.nv
+        self.run = False
+        self.thread.join(timeout=1.0)
+        rows = [s for s in self.samples if t0 <= s[0] <= t1] or self.samples
+        smax = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+        bits = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
+        reasons = sorted(nm for nm, b in bits.items() if any(r[2] & b for r in rows))
+        return {"sm_mhz": float(np.median([r[1] for r in rows])) if rows else None, "sm_max_mhz": float(smax),
+                "power_w_max": max((r[3] for r in rows), default=None), "samples": len(rows), "reasons": reasons,
+                "source": "nvml, 2 ms poll during the timed region"}
+
+
+def make_sampler(index: int):
+    try:
+        return NvmlSampler(index)
+    except Exception:
+        return ClockSampler(index)
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -225,7 +286,7 @@ def run_ours(args) -> None:
     pn.pn_set_state(pos_d, vel_d)
     pn.pn_get_pair_time(reset=True)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K + 2)]
-    sampler = ClockSampler(local)
+    sampler = make_sampler(local)
     sampler.start()
     time.sleep(0.25)
     barrier()
@@ -300,7 +361,7 @@ def run_ours(args) -> None:
         achieved = p.pairs_per_eval * FLOPS_PER_PAIR / (pair_avg_ms * 1e-3) / 1e12 if pair_n else None
         roof = {
             "bound": "alu", "kernel": "pair_fp64_kernel", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-            "frac": (achieved / peak_tflops) if achieved else None, "traffic": None,
+            "frac": (achieved / peak_tflops) if achieved else None, "traffic": NCU_DRAM_BYTES_PER_PAIR_LAUNCH.get(p.n_stars),
             "convention": f"{FP64_INSTR_PER_PAIR} FP64-pipe instructions per ordered pair in the shipped SASS, each counted as an "
                           f"FMA (2 flops) = FP64-pipe issue-slot utilisation; peak = {SMS} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x "
                           f"{sm_max:.0f} MHz (clocks.max.sm; no measured fp64 peak in MEASURED_PEAKS.json)",
@@ -333,8 +394,58 @@ def run_ours(args) -> None:
         dist.destroy_process_group()
 
 
+def run_sweep(args) -> None:
+    """--sweep: BASELINE.json config 5 (and configs 2-4 when --sweep-configs): ONE force evaluation per size and per
+    pair precision, pairs/s and % of the FMA roofline versus N.  One JSON line per case (not the default bench line)."""
+    import torch
+
+    from paper_1801_07986_b200 import PN, binding, inputs
+
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream()
+    peaks = load_peaks()
+    sm_max = peaks.get("sm_max_mhz", 1965.0)
+    peak64 = SMS * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    peak32 = SMS * 128 * 2 * sm_max * 1e6 / 1e12
+    cases = [("ball%d" % k, lambda k=k: inputs.uniform_ball_bh(k)) for k in range(args.kmin, args.kmax + 1)]
+    if args.sweep_configs:
+        cases += [("config%d" % i, lambda i=i: inputs.config(i)) for i in (1, 2, 3, 4)]
+    for name, make in cases:
+        p = make()
+        pn = PN(p.mass, p.G, p.c, p.softening, stream=stream)
+        pos, vel = torch.from_numpy(p.pos).cuda(), torch.from_numpy(p.vel).cuda()
+        acc = torch.empty_like(pos)
+        pn.pn_set_option(binding.PN_OPT_TIME_PAIR, 1)
+        for prec, pname, instr, peak in ((binding.PN_FP64, "fp64", 15, peak64), (binding.PN_FP32_PAIR, "fp32pair", 18, peak32)):
+            pn.pn_set_option(binding.PN_OPT_PAIR_PRECISION, prec)
+            reps = 5 if p.n_stars < 200000 else 2
+            for _ in range(2):
+                pn.pn_accel(pos, vel, acc)
+            pn.pn_get_pair_time(reset=True)
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+            for a, b in ev:
+                a.record(stream)
+                pn.pn_accel(pos, vel, acc)
+                b.record(stream)
+            torch.cuda.synchronize()
+            ms = float(np.median([a.elapsed_time(b) for a, b in ev]))
+            pair_ms, n = pn.pn_get_pair_time(reset=True)
+            pair_ms /= max(1, n)
+            tfl = p.pairs_per_eval * 2 * instr / (pair_ms * 1e-3) / 1e12
+            print(json.dumps({
+                "workload": name, "N": p.N, "precision": pname, "pairs": p.pairs_per_eval, "accel_ms": ms,
+                "accel_pairs_per_s": p.pairs_per_eval / (ms * 1e-3), "pair_kernel_ms": pair_ms,
+                "pair_kernel_pairs_per_s": p.pairs_per_eval / (pair_ms * 1e-3), "pipe_instr_per_pair": instr,
+                "roofline_frac": tfl / peak, "peak_tflops": peak, "pair_config": pn.pn_get_pair_config()}), flush=True)
+        pn.pn_destroy()
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--sweep", action="store_true", help="config-5 single-evaluation sweep (one JSON line per case)")
+    ap.add_argument("--sweep-configs", action="store_true")
+    ap.add_argument("--kmin", type=int, default=10)
+    ap.add_argument("--kmax", type=int, default=20)
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
@@ -342,7 +453,9 @@ def main():
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
