@@ -48,11 +48,18 @@ extern "C" {
 #define PN_OPT_USE_GRAPH 2      /* 1 (default): pn_step replays a captured CUDA graph; 0: plain launches */
 #define PN_OPT_TIME_PAIR 3      /* 1: bracket every star-star pair-kernel launch with CUDA events (forces plain
                                    launches); read with pn_get_pair_time.  0 (default) */
-#define PN_OPT_J_SPLIT 4        /* 0 (default): automatic; > 0: force the number of j-chunks per i-tile */
+#define PN_OPT_J_SPLIT 4        /* 0 (default): automatic; > 0: force the number of j-chunks per i-tile (tiled kernel) */
+#define PN_OPT_PAIR_KERNEL 5    /* which fp64 star-star kernel: PN_PAIR_AUTO (default) | PN_PAIR_TILED | PN_PAIR_SYMMETRIC */
 
 /* PN_OPT_PAIR_PRECISION values */
 #define PN_FP64 0      /* fp64 pair arithmetic and accumulation (parity 1e-12) */
 #define PN_FP32_PAIR 1 /* fp32 pair arithmetic on two-float positions, fp64 accumulation (parity 1e-5) */
+
+/* PN_OPT_PAIR_KERNEL values (fp64 pair arithmetic only; PN_FP32_PAIR always uses the tiled form) */
+#define PN_PAIR_AUTO 0      /* symmetric for N - 1 >= 3072 stars, tiled below */
+#define PN_PAIR_TILED 1     /* every ordered pair (i, j): 15 FP64 instructions per ordered pair */
+#define PN_PAIR_SYMMETRIC 2 /* every unordered pair once, applied to both stars (Newton's third law, exact for the
+                               softened Newtonian term of Eq. 2.4): 10 FP64 instructions per ordered pair */
 
 typedef struct pn_ctx pn_ctx; /* opaque; owns all internal device buffers */
 
@@ -89,8 +96,10 @@ int pn_energy(pn_ctx* ctx, double* E_host);
 int pn_get_launch_count(pn_ctx* ctx, int64_t* n_kernels_host);          /* kernels launched (graph nodes count) */
 int pn_get_pair_time(pn_ctx* ctx, double* ms_total_host, int64_t* n_launches_host, int reset); /* PN_OPT_TIME_PAIR;
                                                                             synchronises the stream */
-int pn_get_pair_config(pn_ctx* ctx, int32_t* cfg_host); /* 8 ints: threads/block, i per thread, j-tile, j-splits,
-                                                           grid blocks, padded N_s, FP64 instr per pair, variant */
+int pn_get_pair_config(pn_ctx* ctx, int32_t* cfg_host); /* 8 ints: threads/block, i per thread, j-tile, partial-sum
+                                                           slots (j-splits / groups), grid blocks, padded N_s, pipe
+                                                           instructions per ordered pair, variant (0 fp64 tiled,
+                                                           1 fp32-pair, 2 fp64 symmetric) */
 
 int pn_measure_fp64_peak(pn_ctx* ctx, double* tflops_host); /* sustained FP64 FMA rate of this device from a register-only
                                                               DFMA-chain kernel (2 flops per FMA), best of 3: the measured

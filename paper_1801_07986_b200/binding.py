@@ -16,8 +16,9 @@ PKG = Path(__file__).resolve().parent
 LIB_PATH = PKG / "libpn.so"
 
 PN_OK, PN_EINVAL, PN_ECUDA, PN_ESTATE, PN_ENOMEM = 0, -1, -2, -3, -4
-PN_OPT_PAIR_PRECISION, PN_OPT_USE_GRAPH, PN_OPT_TIME_PAIR, PN_OPT_J_SPLIT = 1, 2, 3, 4
+PN_OPT_PAIR_PRECISION, PN_OPT_USE_GRAPH, PN_OPT_TIME_PAIR, PN_OPT_J_SPLIT, PN_OPT_PAIR_KERNEL = 1, 2, 3, 4, 5
 PN_FP64, PN_FP32_PAIR = 0, 1
+PN_PAIR_AUTO, PN_PAIR_TILED, PN_PAIR_SYMMETRIC = 0, 1, 2
 
 # every symbol include/pn.h declares (tests check that the library exports all of them)
 EXPORTS = (

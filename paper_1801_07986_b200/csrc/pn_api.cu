@@ -34,10 +34,12 @@ struct pn_ctx {
     std::string err;
 
     // options
-    int precision = PN_FP64, use_graph = 1, time_pair = 0, j_split_opt = 0;
+    int precision = PN_FP64, use_graph = 1, time_pair = 0, j_split_opt = 0, kernel_opt = PN_PAIR_AUTO;
 
     // pair-kernel launch configuration
     int ipt = 1, n_itiles = 0, n_tiles = 0, n_split = 1, tiles_per_split = 0, max_split = 1;
+    // symmetric pair kernel: unit tile U = 32 W I stars, T unit tiles in G groups of m
+    int sym_I = 0, sym_W = 0, sym_U = 0, sym_T = 0, sym_m = 0, sym_G = 0;
 
     // device buffers.  Two stage sets: [0] integrator state, [1] scratch for pn_accel.
     JRec* jrec[2] = {nullptr, nullptr};
@@ -58,7 +60,7 @@ struct pn_ctx {
     double dt_dev = NAN;
 
     cudaGraphExec_t graph1 = nullptr, graphB = nullptr;
-    int graph_split = -1, graph_precision = -1;
+    int graph_split = -1, graph_precision = -1, graph_sym = -1;
 
     int64_t n_launch = 0;
     std::vector<cudaEvent_t> ev;  // pairs (start, stop)
@@ -108,6 +110,38 @@ void choose_split(pn_ctx* c)
     c->n_split = (c->n_tiles + c->tiles_per_split - 1) / c->tiles_per_split;
 }
 
+constexpr int kSymMaxGroups = 128;  // partial-sum slots of the symmetric kernel (tail granularity vs epilogue traffic)
+
+// Symmetric (Newton's third law) kernel variants, by problem size: smaller unit tiles give enough blocks and a
+// fine-grained tail at small N, larger ones amortise the tile prologue at large N (pair kernel).
+void choose_sym(pn_ctx* c)
+{
+    if (c->n_stars < 12288)
+        c->sym_I = 2, c->sym_W = 1;
+    else if (c->n_stars < 49152)
+        c->sym_I = 4, c->sym_W = 1;
+    else
+        c->sym_I = 4, c->sym_W = 4;
+    c->sym_U = 32 * c->sym_W * c->sym_I;
+}
+
+void choose_sym_groups(pn_ctx* c)
+{
+    c->sym_T = c->np / c->sym_U;
+    c->sym_m = (c->sym_T + kSymMaxGroups - 1) / kSymMaxGroups;
+    c->sym_G = (c->sym_T + c->sym_m - 1) / c->sym_m;
+}
+
+bool use_sym(const pn_ctx* c)
+{
+    if (c->precision != PN_FP64) return false;
+    if (c->kernel_opt == PN_PAIR_SYMMETRIC) return true;
+    if (c->kernel_opt == PN_PAIR_TILED) return false;
+    return c->n_stars >= 3072;
+}
+
+int active_split(const pn_ctx* c) { return use_sym(c) ? c->sym_G : c->n_split; }
+
 void destroy_graphs(pn_ctx* c)
 {
     if (c->graph1) cudaGraphExecDestroy(c->graph1), c->graph1 = nullptr;
@@ -120,6 +154,28 @@ void launch_pair_fp64(pn_ctx* c, int set, cudaStream_t st)
 {
     dim3 grid(c->n_itiles, c->n_split);
     pair_fp64_kernel<I, JU, MINB, kNT, kTJ, MASK><<<grid, kNT, 0, st>>>(c->jrec[set], c->part, c->np, c->tiles_per_split, c->eps2);
+}
+
+template <int I, int W, int MINB>
+cudaError_t prepare_sym()
+{
+    cudaError_t e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         kSymSmemBytes<I, W>);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                kSymSmemBytes<I, W>);
+}
+
+template <int I, int W, int MINB>
+void launch_pair_sym(pn_ctx* c, int set, cudaStream_t st)
+{
+    const int blocks = c->sym_G * (c->sym_G + 1) / 2;
+    if (c->eps2 == 0.0)
+        pair_sym_fp64_kernel<I, W, MINB, true><<<blocks, 32 * W, kSymSmemBytes<I, W>, st>>>(c->jrec[set], c->part, c->np, c->sym_T,
+                                                                                           c->sym_m, c->eps2);
+    else
+        pair_sym_fp64_kernel<I, W, MINB, false><<<blocks, 32 * W, kSymSmemBytes<I, W>, st>>>(c->jrec[set], c->part, c->np, c->sym_T,
+                                                                                            c->sym_m, c->eps2);
 }
 
 int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
@@ -146,6 +202,13 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
         else
             mask ? pair_fp32_kernel<1, kNT, kTJ, 32, true><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2)
                  : pair_fp32_kernel<1, kNT, kTJ, 32, false><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2);
+    } else if (use_sym(c)) {
+        if (c->sym_I == 2)
+            launch_pair_sym<2, 1, 16>(c, set, st);
+        else if (c->sym_W == 1)
+            launch_pair_sym<4, 1, 8>(c, set, st);
+        else
+            launch_pair_sym<4, 4, 3>(c, set, st);
     } else if (c->ipt == 2)
         mask ? launch_pair_fp64<2, 4, 4, true>(c, set, st) : launch_pair_fp64<2, 4, 4, false>(c, set, st);
     else
@@ -170,7 +233,7 @@ EpiArgs epi_args(pn_ctx* c, int set, double* acc_out)
     a.ticket = c->ticket;
     a.acc_out = acc_out;
     a.prm = c->prm;
-    a.n_stars = c->n_stars, a.np = c->np, a.n_split = c->n_split;
+    a.n_stars = c->n_stars, a.np = c->np, a.n_split = active_split(c);
     a.GM = c->GM, a.inv_c2 = c->inv_c2;
     return a;
 }
@@ -252,8 +315,10 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
 
     // i per thread: larger i-tiles amortise the shared-memory broadcast; small N needs more blocks instead
     ctx->ipt = ctx->n_stars >= 3072 ? 2 : 1;
-    const int ti = ctx->ipt * kNT;
+    choose_sym(ctx);
+    const int ti = std::max(ctx->ipt * kNT, ctx->sym_U);  // both are powers of two: np suits every pair kernel
     ctx->np = (ctx->n_stars + ti - 1) / ti * ti;
+    choose_sym_groups(ctx);
     ctx->n_itiles = ctx->np / ti;
     ctx->n_tiles = ctx->np / kTJ;
     ctx->max_split = std::min(ctx->n_tiles, 64);
@@ -283,7 +348,10 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA(dalloc(&ctx->v0, 3 * np));
     CREATE_CUDA(dalloc(&ctx->sx, 3 * np));
     CREATE_CUDA(dalloc(&ctx->sv, 3 * np));
-    CREATE_CUDA(dalloc(&ctx->part, (size_t)ctx->max_split * 3 * np));
+    CREATE_CUDA((prepare_sym<2, 1, 16>()));
+    CREATE_CUDA((prepare_sym<4, 1, 8>()));
+    CREATE_CUDA((prepare_sym<4, 4, 3>()));
+    CREATE_CUDA(dalloc(&ctx->part, (size_t)std::max(ctx->max_split, ctx->sym_G) * 3 * np));
     CREATE_CUDA(dalloc(&ctx->bh_part, 3 * (np / (kNT / kEpiG))));
     CREATE_CUDA(dalloc(&ctx->ticket, 1));
     CREATE_CUDA(cudaMemset(ctx->ticket, 0, sizeof(unsigned int)));
@@ -361,6 +429,11 @@ int pn_set_option(pn_ctx* c, int key, int value)
         case PN_OPT_TIME_PAIR:
             if (value != 0 && value != 1) return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_TIME_PAIR takes 0 or 1");
             c->time_pair = value;
+            return PN_OK;
+        case PN_OPT_PAIR_KERNEL:
+            if (value != PN_PAIR_AUTO && value != PN_PAIR_TILED && value != PN_PAIR_SYMMETRIC)
+                return fail(c, PN_EINVAL, "pn_set_option: unknown pair kernel %d", value);
+            c->kernel_opt = value;
             return PN_OK;
         case PN_OPT_J_SPLIT:
             if (value < 0) return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_J_SPLIT must be >= 0");
@@ -469,9 +542,9 @@ int pn_step(pn_ctx* c, double dt, int64_t nsteps)
         c->n_launch += (c->precision == PN_FP32_PAIR ? 12 : 8) * nsteps;
         return PN_OK;
     }
-    if (c->graph_split != c->n_split || c->graph_precision != c->precision) {
+    if (c->graph_split != c->n_split || c->graph_precision != c->precision || c->graph_sym != (int)use_sym(c)) {
         destroy_graphs(c);
-        c->graph_split = c->n_split, c->graph_precision = c->precision;
+        c->graph_split = c->n_split, c->graph_precision = c->precision, c->graph_sym = (int)use_sym(c);
     }
     int64_t left = nsteps;
     if (left >= kGraphBatch) {
@@ -567,6 +640,11 @@ int pn_get_pair_config(pn_ctx* c, int32_t* cfg)
 {
     if (int rc = check_ctx(c)) return rc;
     if (!cfg) return fail(c, PN_EINVAL, "pn_get_pair_config: null pointer");
+    if (use_sym(c)) {
+        cfg[0] = 32 * c->sym_W, cfg[1] = c->sym_I, cfg[2] = c->sym_U, cfg[3] = c->sym_G;
+        cfg[4] = c->sym_G * (c->sym_G + 1) / 2, cfg[5] = c->np, cfg[6] = 10, cfg[7] = 2;
+        return PN_OK;
+    }
     cfg[0] = kNT, cfg[1] = c->ipt, cfg[2] = kTJ, cfg[3] = c->n_split;
     cfg[4] = c->n_itiles * c->n_split, cfg[5] = c->np, cfg[6] = (c->precision == PN_FP32_PAIR) ? 18 : 15, cfg[7] = c->precision;
     return PN_OK;

@@ -183,6 +183,194 @@ __global__ void __launch_bounds__(NT, MINB) pair_fp64_kernel(const JRec* __restr
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// S1, symmetric form: every unordered star pair {i, j} is evaluated once and applied to both stars (Newton's
+// third law holds exactly for the softened Newtonian star-star term of Eq. 2.4):
+//     a_i += G m_j K d,   a_j -= G m_i K d,   d = x_j - x_i,   K = rho_ij^-3.
+// Per unordered pair: 20 FP64-pipe instructions + 1 MUFU (= 10 per ordered pair instead of 15):
+//   d (3 DADD); r2 = d.d + eps^2 (3 DFMA); y0 = MUFU.RSQ64H(r2); t = y0^2; e = 1 - r2 t;
+//   p = 1 + 3/2 e + 15/8 e^2 (2 DFMA); u = t y0; K = u p; s_j = K Gm_j; s_i = -K Gm_i; 6 DFMA accumulate.
+//
+// Work decomposition.  Stars are cut into unit tiles of U = 32 W I stars and the tiles into G groups of m tiles.
+// Block (A <= B) owns the group pair: it walks the unit-tile pairs (ta in A, tb in B; tb >= ta when A == B).
+// Inside a unit-tile pair each warp keeps I i-stars per lane in registers (position, accumulator, -G m_i) and
+// sweeps the tile's j-stars in sub-groups of 32: lane l starts with j-star l of the sub-group and in 32 rotation
+// steps meets all 32 (positions come from shared memory at a rotating index; the three j-side accumulators
+// travel from lane to lane with SHFL), so after 32 steps the j-side sums are complete and back in their home
+// lane without any reduction across lanes.  The diagonal unit tile (ta == tb) is evaluated as ordered pairs,
+// i-side only.
+//
+// Output: slot P of part[P][3][np] receives, for every star, the sum over the j-stars of group P -- written by
+// exactly one block in a fixed order (row sums of block (A,B) go to slot B, column sums to slot A), so the
+// epilogue's fixed-order sum over the G slots is bit-reproducible and nothing has to be zeroed between launches.
+// ---------------------------------------------------------------------------------------------------------
+template <int I, bool SYM, bool MASK>
+__device__ __forceinline__ void sym_step(const double2 xy, const double2 zm, const double (&xi)[I],
+                                         const double (&yi)[I], const double (&zi)[I], const double (&ngi)[I],
+                                         double (&ax)[I], double (&ay)[I], double (&az)[I], double& bx, double& by,
+                                         double& bz, double eps2, int self_k)
+{
+    double dx[I], dy[I], dz[I], r2[I], y0[I], t[I], e[I], p[I], sj[I];
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        dx[k] = xy.x - xi[k];
+        dy[k] = xy.y - yi[k];
+        dz[k] = zm.x - zi[k];
+    }
+#pragma unroll
+    for (int k = 0; k < I; ++k) r2[k] = fma(dz[k], dz[k], eps2);
+#pragma unroll
+    for (int k = 0; k < I; ++k) r2[k] = fma(dy[k], dy[k], r2[k]);
+#pragma unroll
+    for (int k = 0; k < I; ++k) r2[k] = fma(dx[k], dx[k], r2[k]);
+#pragma unroll
+    for (int k = 0; k < I; ++k) y0[k] = rsqrt_seed(r2[k]);
+#pragma unroll
+    for (int k = 0; k < I; ++k) t[k] = y0[k] * y0[k];
+#pragma unroll
+    for (int k = 0; k < I; ++k) e[k] = fma(-r2[k], t[k], 1.0);
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        t[k] = t[k] * y0[k];             // y0^3
+        p[k] = fma(e[k], 1.875, 1.5);
+    }
+#pragma unroll
+    for (int k = 0; k < I; ++k) p[k] = fma(e[k], p[k], 1.0);  // (1 - e)^(-3/2) to O(e^3)
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        t[k] = t[k] * p[k];              // K = rho^-3
+        if (MASK) t[k] = (k == self_k) ? 0.0 : t[k];
+    }
+#pragma unroll
+    for (int k = 0; k < I; ++k) sj[k] = t[k] * zm.y;  // G m_j K
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        ax[k] = fma(sj[k], dx[k], ax[k]);
+        ay[k] = fma(sj[k], dy[k], ay[k]);
+        az[k] = fma(sj[k], dz[k], az[k]);
+    }
+    if (SYM) {
+#pragma unroll
+        for (int k = 0; k < I; ++k) t[k] = t[k] * ngi[k];  // -G m_i K
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            bx = fma(t[k], dx[k], bx);
+            by = fma(t[k], dy[k], by);
+            bz = fma(t[k], dz[k], bz);
+        }
+    }
+}
+
+template <int I, int W, bool SYM, bool MASK>
+__device__ __forceinline__ void sym_unit_tile(const double2* __restrict__ sxy, const double2* __restrict__ szm,
+                                              double* __restrict__ cw /* this warp's [3][U] column sums */,
+                                              const double (&xi)[I], const double (&yi)[I], const double (&zi)[I],
+                                              const double (&ngi)[I], double (&ax)[I], double (&ay)[I],
+                                              double (&az)[I], double eps2, int lane, int i_local0)
+{
+    constexpr int U = W * 32 * I;
+#pragma unroll 1
+    for (int jb = 0; jb < U; jb += 32) {
+        double bx = 0.0, by = 0.0, bz = 0.0;
+        constexpr int kUnr = (I >= 4) ? 2 : 8 / I;  // about 8 independent pairs in flight per warp
+#pragma unroll kUnr
+        for (int r = 0; r < 32; ++r) {
+            const int jj = jb + ((lane + r) & 31);
+            int self_k = -1;
+            if (MASK) {  // diagonal unit tile with eps == 0: the self pair would be 0 * inf
+                const int q = jj - i_local0;
+                self_k = (q >= 0 && (q & 31) == 0) ? (q >> 5) : -1;
+            }
+            sym_step<I, SYM, MASK>(sxy[jj], szm[jj], xi, yi, zi, ngi, ax, ay, az, bx, by, bz, eps2, self_k);
+            if (SYM) {  // the j-star moves on to the next lane together with its partial sums
+                const int src = (lane + 1) & 31;
+                bx = __shfl_sync(0xffffffffu, bx, src);
+                by = __shfl_sync(0xffffffffu, by, src);
+                bz = __shfl_sync(0xffffffffu, bz, src);
+            }
+        }
+        if (SYM) {  // after 32 rotations lane l holds the complete sums of j-star jb + l again
+            cw[jb + lane] = bx;
+            cw[U + jb + lane] = by;
+            cw[2 * U + jb + lane] = bz;
+        }
+    }
+}
+
+template <int I, int W>
+constexpr int kSymSmemBytes = (W * 32 * I) * (2 * 16 + W * 3 * 8);
+
+template <int I, int W, int MINB, bool MASK>
+__global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp64_kernel(const JRec* __restrict__ jrec,
+                                                                     double* __restrict__ part, int np, int n_tiles,
+                                                                     int m, double eps2)
+{
+    constexpr int U = W * 32 * I;
+    constexpr int NT = W * 32;
+    extern __shared__ double2 sym_smem[];  // kSymSmemBytes<I, W>: dynamic, U = 512 needs more than 48 KB
+    double2* sxy = sym_smem;                                                   // [U] x, y of the j tile
+    double2* szm = sym_smem + U;                                               // [U] z, G m
+    double(*cacc)[3][U] = reinterpret_cast<double(*)[3][U]>(sym_smem + 2 * U);  // [W][3][U] per-warp column sums
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+
+    // triangular decode of the block index: (A <= B), blockIdx.x = B (B + 1) / 2 + A
+    int B = (int)((sqrtf(8.0f * (float)blockIdx.x + 1.0f) - 1.0f) * 0.5f);
+    while ((B + 1) * (B + 2) / 2 <= (int)blockIdx.x) ++B;
+    while (B * (B + 1) / 2 > (int)blockIdx.x) --B;
+    const int A = (int)blockIdx.x - B * (B + 1) / 2;
+
+    const int ta0 = A * m, ta1 = min(ta0 + m, n_tiles);
+    const int tb0 = B * m, tb1 = min(tb0 + m, n_tiles);
+    const int i_local0 = w * 32 * I + lane;  // this lane's k-th i-star is i_local0 + 32 k inside the unit tile
+
+    // sums a block-owned [3][U] tile into slot `slot` of part (same thread <-> same elements on every call)
+    auto flush = [&](int slot, int tile, bool first, int n_src) {
+        double* dst = part + (size_t)slot * 3 * np + (size_t)tile * U;
+        for (int q = tid; q < 3 * U; q += NT) {
+            const int c = q / U, el = q - c * U;
+            double v = cacc[0][c][el];
+            for (int s = 1; s < n_src; ++s) v += cacc[s][c][el];
+            double* d = dst + (size_t)c * np + el;
+            *d = first ? v : *d + v;
+        }
+    };
+
+    for (int ta = ta0; ta < ta1; ++ta) {
+        double xi[I], yi[I], zi[I], ngi[I], ax[I], ay[I], az[I];
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            const JRec* p = jrec + (size_t)ta * U + i_local0 + 32 * k;
+            xi[k] = p->x, yi[k] = p->y, zi[k] = p->z, ngi[k] = -p->gm;
+            ax[k] = ay[k] = az[k] = 0.0;
+        }
+        for (int tb = (A == B) ? ta : tb0; tb < tb1; ++tb) {
+            __syncthreads();  // everyone is done with the previous tile's shared memory
+            for (int q = tid; q < U; q += NT) {
+                const double2* src = reinterpret_cast<const double2*>(jrec + (size_t)tb * U + q);
+                sxy[q] = src[0];  // x, y
+                szm[q] = src[1];  // z, G m
+            }
+            __syncthreads();
+            if (ta == tb) {
+                sym_unit_tile<I, W, false, MASK>(sxy, szm, &cacc[w][0][0], xi, yi, zi, ngi, ax, ay, az, eps2, lane, i_local0);
+            } else {
+                sym_unit_tile<I, W, true, false>(sxy, szm, &cacc[w][0][0], xi, yi, zi, ngi, ax, ay, az, eps2, lane, i_local0);
+                __syncthreads();
+                flush(A, tb, ta == ta0, W);  // column sums: the i-stars of tile ta acting on the j-stars of tile tb
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            cacc[0][0][i_local0 + 32 * k] = ax[k];
+            cacc[0][1][i_local0 + 32 * k] = ay[k];
+            cacc[0][2][i_local0 + 32 * k] = az[k];
+        }
+        __syncthreads();
+        flush(B, ta, (A < B) || (ta == ta0), 1);  // row sums: the j-stars of group B acting on the i-stars of tile ta
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // S1 variant: fp32 pair arithmetic, fp64 accumulation (PN_FP32_PAIR, parity 1e-5).
 // Positions are split into two floats, hi = fl32(x), lo = fl32(x - hi), so that the pair separation
 //   d = (hi_j - hi_i) + (lo_j - lo_i)

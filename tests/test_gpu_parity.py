@@ -78,10 +78,53 @@ def test_accel_parity_other_distributions(gen):
     assert rel_err_rows(acc, ref).max() <= TOL_ACC
 
 
-def test_accel_zero_softening_masks_self_pair():
-    p = inputs.random_small(300, seed=6, M=1.0, m_scale=1e-3, c=20.0, softening=0.0)
+# both fp64 star-star kernels at every size class: the tiled one (ordered pairs) and the symmetric one (unordered
+# pairs applied to both stars) in its three unit-tile variants (U = 64: N_s < 12288, 128: < 49152, 512 above),
+# with one group per tile (m = 1) and several (9000 -> T = 144, m = 2; 20000 -> T = 157, m = 2, ragged last group)
+@pytest.mark.parametrize("kernel", ["tiled", "symmetric"])
+@pytest.mark.parametrize("n_stars", [1, 2, 65, 129, 1023, 3071, 4099, 9000, 13001, 20000])
+def test_accel_parity_both_pair_kernels(n_stars, kernel):
+    from paper_1801_07986_b200 import binding
+
+    if n_stars <= 2:
+        p = inputs.random_small(n_stars, seed=111, M=1.0, m_scale=1e-2, c=10.0, softening=1e-3, bh_moving=True)
+    else:
+        p = inputs.plummer_bh(n_stars, seed=300 + n_stars)
+    ref = Oracle(p.mass, p.G, p.c, p.softening).accel(p.pos, p.vel)
+    with _pn(p) as pn:
+        pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, binding.PN_PAIR_TILED if kernel == "tiled" else binding.PN_PAIR_SYMMETRIC)
+        assert pn.pn_get_pair_config()["variant"] == (0 if kernel == "tiled" else 2)
+        acc = _gpu_accel(pn, p.pos, p.vel)
+        again = _gpu_accel(pn, p.pos, p.vel)
+    assert rel_err_rows(acc, ref).max() <= TOL_ACC
+    assert np.array_equal(acc, again)  # fixed-order partial sums: bit-reproducible
+
+
+def test_pair_kernels_agree_and_auto_selection():
+    from paper_1801_07986_b200 import binding
+
+    for n_stars, want in ((3071, 0), (3072, 2)):
+        p = inputs.plummer_bh(n_stars, seed=12)
+        with _pn(p) as pn:
+            assert pn.pn_get_pair_config()["variant"] == want
+            acc = {}
+            for k in (binding.PN_PAIR_TILED, binding.PN_PAIR_SYMMETRIC):
+                pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, k)
+                acc[k] = _gpu_accel(pn, p.pos, p.vel)
+            assert rel_err_rows(acc[binding.PN_PAIR_SYMMETRIC], acc[binding.PN_PAIR_TILED]).max() <= 1e-13
+            with pytest.raises(binding.PNError):
+                pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, 7)
+
+
+@pytest.mark.parametrize("kernel", ["tiled", "symmetric"])
+@pytest.mark.parametrize("n_stars", [300, 4099])
+def test_accel_zero_softening_masks_self_pair(n_stars, kernel):
+    from paper_1801_07986_b200 import binding
+
+    p = inputs.random_small(n_stars, seed=6, M=1.0, m_scale=1e-3, c=20.0, softening=0.0)
     ref = Oracle(p.mass, p.G, p.c, 0.0).accel(p.pos, p.vel)
     with _pn(p) as pn:
+        pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, binding.PN_PAIR_TILED if kernel == "tiled" else binding.PN_PAIR_SYMMETRIC)
         acc = _gpu_accel(pn, p.pos, p.vel)
     assert np.isfinite(acc).all()
     assert rel_err_rows(acc, ref).max() <= TOL_ACC
@@ -107,6 +150,7 @@ def test_accel_is_deterministic_and_independent_of_j_split():
         a1 = _gpu_accel(pn, p.pos, p.vel)
         a2 = _gpu_accel(pn, p.pos, p.vel)
         assert np.array_equal(a1, a2)  # fixed-order reductions: bit-reproducible
+        pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, binding.PN_PAIR_TILED)  # the j-split belongs to the tiled kernel
         for s in (1, 3, 64):
             pn.pn_set_option(binding.PN_OPT_J_SPLIT, s)
             assert rel_err_rows(_gpu_accel(pn, p.pos, p.vel), ref).max() <= TOL_ACC
