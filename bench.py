@@ -27,12 +27,15 @@ ROOT = Path(__file__).resolve().parent
 if str(ROOT) not in sys.path:
     sys.path.insert(0, str(ROOT))
 
-FP64_INSTR_PER_PAIR = 15          # SASS-verified: 3 DADD + 9 DFMA + 3 DMUL per ordered pair (+1 MUFU.RSQ64H)
-FLOPS_PER_PAIR = 2 * FP64_INSTR_PER_PAIR  # issue-slot convention: every FP64-pipe instruction counted as an FMA
+# fp64 star-star kernels by pn_get_pair_config()["variant"]: name, FP64-pipe instructions per ORDERED pair in the shipped
+# SASS (cuobjdump-verified; the library reports the same number), executed flops per ordered pair (FMA = 2, MUL/ADD = 1):
+#   0 tiled:     3 DADD + 9 DFMA + 3 DMUL = 15 per ordered pair (+1 MUFU.RSQ64H)
+#   2 symmetric: 3 DADD + 12 DFMA + 5 DMUL = 20 per UNORDERED pair (+1 MUFU.RSQ64H) = 10 per ordered pair
+PAIR_KERNELS = {0: ("pair_fp64_kernel", 15, 24.0), 2: ("pair_sym_fp64_kernel", 10, 16.0)}
 SMS, FP64_LANES_PER_SM = 148, 64
-# dram__bytes_read.sum + dram__bytes_write.sum of one pair_fp64_kernel launch, from the committed ncu --set full capture
-# (profiles/r1_ncu_summary.md section 2), keyed by N_s; algorithmic bytes are the 48 B j records read once: 16384 * 48 = 786432
-NCU_DRAM_BYTES_PER_PAIR_LAUNCH = {16383: 793344}
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu --set full
+# captures (profiles/), keyed by (variant, N_s); null when no capture exists for the workload
+NCU_DRAM_BYTES_PER_PAIR_LAUNCH = {(0, 16383): 793344}
 
 
 def load_peaks() -> dict:
@@ -358,18 +361,23 @@ def run_ours(args) -> None:
         sm_max = peaks.get("sm_max_mhz", 1965.0)
         peak_tflops = SMS * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
         pair_avg_ms = pair_ms / max(1, pair_n)
-        achieved = p.pairs_per_eval * FLOPS_PER_PAIR / (pair_avg_ms * 1e-3) / 1e12 if pair_n else None
+        kname, instr, exec_flops = PAIR_KERNELS[cfg["variant"]]
+        assert instr == cfg["fp64_instr_per_pair"]
+        kernel_pairs_per_s = p.pairs_per_eval / (pair_avg_ms * 1e-3) if pair_n else None
+        achieved = kernel_pairs_per_s * 2 * instr / 1e12 if pair_n else None
         roof = {
-            "bound": "alu", "kernel": "pair_fp64_kernel", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-            "frac": (achieved / peak_tflops) if achieved else None, "traffic": NCU_DRAM_BYTES_PER_PAIR_LAUNCH.get(p.n_stars),
-            "convention": f"{FP64_INSTR_PER_PAIR} FP64-pipe instructions per ordered pair in the shipped SASS, each counted as an "
+            "bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+            "frac": (achieved / peak_tflops) if achieved else None,
+            "traffic": NCU_DRAM_BYTES_PER_PAIR_LAUNCH.get((cfg["variant"], p.n_stars)),
+            "convention": f"{instr} FP64-pipe instructions per ordered pair in the shipped SASS, each counted as an "
                           f"FMA (2 flops) = FP64-pipe issue-slot utilisation; peak = {SMS} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x "
                           f"{sm_max:.0f} MHz (clocks.max.sm; no measured fp64 peak in MEASURED_PEAKS.json)",
             "pairs_per_launch": p.pairs_per_eval, "avg_launch_ms": pair_avg_ms, "launches_timed": pair_n,
             "pair_kernel_share_of_steps": pair_ms / ms_steps if ms_steps else None,
-            "kernel_pairs_per_s": p.pairs_per_eval / (pair_avg_ms * 1e-3) if pair_n else None,
+            "kernel_pairs_per_s": kernel_pairs_per_s,
             "frac_at_sampled_clock": (achieved / (peak_tflops * clocks["sm_mhz"] / sm_max)) if achieved and clocks.get("sm_mhz") else None,
-            "executed_flops_frac": (achieved * 24.0 / 30.0 / peak_tflops) if achieved else None,
+            "executed_flops_frac": (kernel_pairs_per_s * exec_flops / 1e12 / peak_tflops) if achieved else None,
+            "classic_20flop_frac": (kernel_pairs_per_s * 20.0 / 1e12 / peak_tflops) if achieved else None,
             "peak_measured_dfma": dfma_peak,
             "frac_of_measured_dfma": (achieved / dfma_peak) if achieved and dfma_peak else None,
         }
@@ -416,8 +424,9 @@ def run_sweep(args) -> None:
         pos, vel = torch.from_numpy(p.pos).cuda(), torch.from_numpy(p.vel).cuda()
         acc = torch.empty_like(pos)
         pn.pn_set_option(binding.PN_OPT_TIME_PAIR, 1)
-        for prec, pname, instr, peak in ((binding.PN_FP64, "fp64", 15, peak64), (binding.PN_FP32_PAIR, "fp32pair", 18, peak32)):
+        for prec, pname, peak in ((binding.PN_FP64, "fp64", peak64), (binding.PN_FP32_PAIR, "fp32pair", peak32)):
             pn.pn_set_option(binding.PN_OPT_PAIR_PRECISION, prec)
+            instr = pn.pn_get_pair_config()["fp64_instr_per_pair"]  # pipe instructions per ordered pair of the kernel in use
             reps = 5 if p.n_stars < 200000 else 2
             for _ in range(2):
                 pn.pn_accel(pos, vel, acc)

@@ -242,7 +242,7 @@ EpiArgs epi_args(pn_ctx* c, int set, double* acc_out)
 int enqueue_rk4_step(pn_ctx* c, cudaStream_t st, bool timed)
 {
     const EpiArgs a = epi_args(c, 0, nullptr);
-    const int grid = c->np / (kNT / kEpiG);
+    const int grid = c->np / kEpiStars;
     for (int stage = 0; stage < 4; ++stage) {
         int rc = launch_pair(c, 0, st, timed);
         if (rc) return rc;
@@ -352,7 +352,7 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA((prepare_sym<4, 1, 8>()));
     CREATE_CUDA((prepare_sym<4, 4, 3>()));
     CREATE_CUDA(dalloc(&ctx->part, (size_t)std::max(ctx->max_split, ctx->sym_G) * 3 * np));
-    CREATE_CUDA(dalloc(&ctx->bh_part, 3 * (np / (kNT / kEpiG))));
+    CREATE_CUDA(dalloc(&ctx->bh_part, 3 * (np / kEpiStars)));
     CREATE_CUDA(dalloc(&ctx->ticket, 1));
     CREATE_CUDA(cudaMemset(ctx->ticket, 0, sizeof(unsigned int)));
     CREATE_CUDA(dalloc(&ctx->prm, 1));
@@ -502,7 +502,7 @@ int pn_accel(pn_ctx* c, const double* pos, const double* vel, double* acc)
     PN_CUDA(c, cudaGetLastError());
     if (int rc = launch_pair(c, 1, c->stream, c->time_pair != 0)) return rc;
     const EpiArgs a = epi_args(c, 1, acc);
-    epilogue_kernel<MODE_ACCEL, kNT><<<c->np / (kNT / kEpiG), kNT, 0, c->stream>>>(a, 0);
+    epilogue_kernel<MODE_ACCEL, kNT><<<c->np / kEpiStars, kNT, 0, c->stream>>>(a, 0);
     PN_CUDA(c, cudaGetLastError());
     c->n_launch += (c->precision == PN_FP32_PAIR ? 4 : 3);
     return PN_OK;
@@ -571,8 +571,8 @@ int pn_energy(pn_ctx* c, double* E)
                                                         c->GM, c->G, c->inv_c2);
     PN_CUDA(c, cudaGetLastError());
     dim3 grid(n_it, c->e_split);
-    energy_pair_kernel<kNT, kTJ><<<grid, kNT, 0, c->stream>>>(c->erec, c->blk_pair, c->n_stars, c->np, c->e_tiles_per_split,
-                                                              c->eps2, c->G, c->inv_c2);
+    energy_pair_kernel<kNT, kTJ><<<grid, kNT, 0, c->stream>>>(c->erec, c->blk_pair, c->n_stars, c->np, c->eps2, c->G,
+                                                              c->inv_c2);
     PN_CUDA(c, cudaGetLastError());
     energy_final_kernel<256><<<1, 256, 0, c->stream>>>(c->blk_prep, n_it, c->blk_pair, n_it * c->e_split, c->bh[0], c->M, c->GM,
                                                        c->G, c->inv_c2, c->d_energy);

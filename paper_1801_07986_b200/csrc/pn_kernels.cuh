@@ -551,32 +551,50 @@ struct EpiArgs {
 
 enum { MODE_ACCEL = 0, MODE_RK4 = 1 };
 
-constexpr int kEpiG = 8;  // threads per star in the epilogue: each sums every 8th j-chunk partial (memory parallelism)
+constexpr int kEpiStars = 32;  // stars per epilogue block: lane = star, warp w sums the partial-sum slots w, w + NW, ...
 
 template <int MODE, int NT>
 __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
 {
-    __shared__ double red[3 * (NT / 32)];
+    constexpr int NW = NT / 32;
+    static_assert(NW == 4, "the fixed-order cross-warp sum below is written for 4 warps");
+    __shared__ double red[3 * NW];
+    __shared__ double wsum[NW][3][kEpiStars];
     __shared__ bool is_last;
-    const int i = blockIdx.x * (NT / kEpiG) + threadIdx.x / kEpiG;
-    const int g = threadIdx.x % kEpiG;
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int i = blockIdx.x * kEpiStars + lane;
     const int np = A.np;
 
-    // fixed-order reduction of the j-chunk partials: sub-lane g takes chunks g, g+8, ...; then a fixed shuffle tree
+    // fixed-order reduction of the partial-sum slots.  Every load is a coalesced 256 B row of one (slot, component);
+    // 4 slots x 3 components are in flight per thread, so the O(S N) read runs at L2/HBM bandwidth, not latency.
     double ss[3] = {0, 0, 0};
     if (i < A.n_stars) {
-        for (int s = g; s < A.n_split; s += kEpiG) {
-            const double* p = A.part + (size_t)s * 3 * np + i;
-            ss[0] += p[0], ss[1] += p[np], ss[2] += p[2 * np];
+        const size_t stride = (size_t)NW * 3 * np;
+        const double* p = A.part + (size_t)w * 3 * np + i;
+        int s = w;
+        for (; s + 3 * NW < A.n_split; s += 4 * NW, p += 4 * stride) {
+            double q[4][3];
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int k = 0; k < 3; ++k) q[u][k] = __ldcg(p + u * stride + (size_t)k * np);
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int k = 0; k < 3; ++k) ss[k] += q[u][k];
         }
+        for (; s < A.n_split; s += NW, p += stride)
+#pragma unroll
+            for (int k = 0; k < 3; ++k) ss[k] += __ldcg(p + (size_t)k * np);
     }
 #pragma unroll
-    for (int o = kEpiG / 2; o > 0; o >>= 1) {
-        ss[0] += __shfl_down_sync(0xffffffffu, ss[0], o, kEpiG);
-        ss[1] += __shfl_down_sync(0xffffffffu, ss[1], o, kEpiG);
-        ss[2] += __shfl_down_sync(0xffffffffu, ss[2], o, kEpiG);
+    for (int k = 0; k < 3; ++k) wsum[w][k][lane] = ss[k];
+    __syncthreads();
+    if (w == 0) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) ss[k] = ((wsum[0][k][lane] + wsum[1][k][lane]) + wsum[2][k][lane]) + wsum[3][k][lane];
     }
-    const bool live = (g == 0) && (i < A.n_stars);
+    const bool live = (w == 0) && (i < A.n_stars);
 
     double b0 = 0, b1 = 0, b2 = 0;  // this star's contribution to a_1
     double a[3] = {0, 0, 0}, vel[3] = {0, 0, 0};
@@ -735,7 +753,7 @@ __global__ void unpack_kernel(const double* __restrict__ x0, const double* __res
 
 // ---------------------------------------------------------------------------------------------------------
 // S5: total 1PN energy, Eq. 2.7, regrouped:
-//   E = 1/2 M v_1^2 + sum_i e_i + (1/c^2) 1/2 G^2 M (sum_i m_i/r_1i)^2 + 1/2 sum_{i != j} Epair(i, j)
+//   E = 1/2 M v_1^2 + sum_i e_i + (1/c^2) 1/2 G^2 M (sum_i m_i/r_1i)^2 + sum_{i < j} Epair(i, j)
 //   e_i = 1/2 m v^2 - GMm/r + (1/c^2){3/8 m v^4 + 3/2 (GMm/r) v^2 + 1/2 G^2M^2 m/r^2
 //                                    + 1/2 (GMm/r)[3 v_1^2 - 7 v_1.v_i - (n_1i.v_1)(n_1i.v_i)]}
 //   Epair(i,j) = (G m_i m_j / rho){-1 + (1/c^2)[w_i + w_j - 7/2 v_i.v_j - 1/2 (x_ij.v_i)(x_ij.v_j)/rho^2]},
@@ -829,11 +847,11 @@ __global__ void __launch_bounds__(NT) energy_prep_kernel(const JRec* __restrict_
     }
 }
 
-// O(N^2) part: ordered pairs (i, j != i), each contributing 1/2 Epair.  grid = (i-tiles, j-splits).
+// O(N^2) part: Epair is symmetric in (i, j), so only the unordered pairs i < j are visited: thread i walks the
+// j-tiles from its own tile upwards and skips j <= i.  grid = (i-tiles, j-splits of that i-tile's own range).
 template <int NT, int TJ>
 __global__ void __launch_bounds__(NT) energy_pair_kernel(const ERec* __restrict__ erec, double* __restrict__ blk /* [grid][2] */,
-                                                         int n_stars, int np, int tiles_per_split, double eps2, double G,
-                                                         double inv_c2)
+                                                         int n_stars, int np, double eps2, double G, double inv_c2)
 {
     __shared__ ERec sj[TJ];
     __shared__ double red[2 * (NT / 32)];
@@ -843,9 +861,11 @@ __global__ void __launch_bounds__(NT) energy_pair_kernel(const ERec* __restrict_
     const double mi = me.gm / G;
     double hi = 0, lo = 0;
 
+    static_assert(NT == TJ, "i-tiles and j-tiles share one index space");
     const int n_tiles = np / TJ;
-    const int t_begin = blockIdx.y * tiles_per_split;
-    const int t_end = min(n_tiles, t_begin + tiles_per_split);
+    const int per = (n_tiles - (int)blockIdx.x + (int)gridDim.y - 1) / (int)gridDim.y;
+    const int t_begin = blockIdx.x + blockIdx.y * per;
+    const int t_end = min(n_tiles, t_begin + per);
     for (int t = t_begin; t < t_end; ++t) {
         __syncthreads();
         {
@@ -869,7 +889,7 @@ __global__ void __launch_bounds__(NT) energy_pair_kernel(const ERec* __restrict_
             const double xvj = dx * r.vx + dy * r.vy + dz * r.vz;
             const double br = me.w + r.w - 3.5 * vv - 0.5 * xvi * xvj * (y * y);
             double term = (mi * r.gm * y) * (-1.0 + inv_c2 * br);
-            term = (j0 + jj == i) ? 0.0 : term;
+            term = (j0 + jj <= i) ? 0.0 : term;  // i < j only (false only inside the diagonal tile)
             two_sum_acc(hi, lo, term);
         }
     }
@@ -909,8 +929,8 @@ __global__ void __launch_bounds__(NT) energy_final_kernel(const double* __restri
         double hi = 0, lo = 0;
         two_sum_acc(hi, lo, e_hi);
         lo += e_lo;
-        two_sum_acc(hi, lo, 0.5 * p_hi);  // ordered pairs were summed: 1/2
-        lo += 0.5 * p_lo;
+        two_sum_acc(hi, lo, p_hi);  // unordered pairs i < j
+        lo += p_lo;
         two_sum_acc(hi, lo, 0.5 * M * v12);
         two_sum_acc(hi, lo, inv_c2 * 0.5 * G * GM * smr * smr);
         out[0] = hi + lo;
