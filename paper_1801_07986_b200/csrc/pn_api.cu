@@ -319,7 +319,7 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     const int ti = std::max(ctx->ipt * kNT, ctx->sym_U);  // both are powers of two: np suits every pair kernel
     ctx->np = (ctx->n_stars + ti - 1) / ti * ti;
     choose_sym_groups(ctx);
-    ctx->n_itiles = ctx->np / ti;
+    ctx->n_itiles = ctx->np / (ctx->ipt * kNT);
     ctx->n_tiles = ctx->np / kTJ;
     ctx->max_split = std::min(ctx->n_tiles, 64);
     choose_split(ctx);

@@ -757,12 +757,12 @@ __global__ void unpack_kernel(const double* __restrict__ x0, const double* __res
 //   e_i = 1/2 m v^2 - GMm/r + (1/c^2){3/8 m v^4 + 3/2 (GMm/r) v^2 + 1/2 G^2M^2 m/r^2
 //                                    + 1/2 (GMm/r)[3 v_1^2 - 7 v_1.v_i - (n_1i.v_1)(n_1i.v_i)]}
 //   Epair(i,j) = (G m_i m_j / rho){-1 + (1/c^2)[w_i + w_j - 7/2 v_i.v_j - 1/2 (x_ij.v_i)(x_ij.v_j)/rho^2]},
-//   w_i = 3/2 v_i^2 + G M / r_1i.
+//   w_i = 3/2 v_i^2 + G M / r_1i (the record stores w_i / c^2).
 // All sums are compensated (TwoSum): a (hi, lo) pair per thread, per block and in the final reduction.
 // ---------------------------------------------------------------------------------------------------------
 struct __align__(16) ERec {
     double x, y, z, gm;     // position, G m_j
-    double vx, vy, vz, w;   // velocity, w_j
+    double vx, vy, vz, w;   // velocity, w_j / c^2
 };
 static_assert(sizeof(ERec) == 64, "ERec must be 64 bytes");
 
@@ -828,7 +828,7 @@ __global__ void __launch_bounds__(NT) energy_prep_kernel(const JRec* __restrict_
             const double nvi = (d[0] * vv[0] + d[1] * vv[1] + d[2] * vv[2]) * inv_r;
             const double U = GM * m * inv_r;  // G M m / r
             o.vx = vv[0], o.vy = vv[1], o.vz = vv[2];
-            o.w = 1.5 * v2 + GM * inv_r;
+            o.w = inv_c2 * (1.5 * v2 + GM * inv_r);
             two_sum_acc(e_hi, e_lo, 0.5 * m * v2);
             two_sum_acc(e_hi, e_lo, -U);
             const double pn = 0.375 * m * v2 * v2 + 1.5 * U * v2 + 0.5 * U * GM * inv_r +
@@ -857,8 +857,11 @@ __global__ void __launch_bounds__(NT) energy_pair_kernel(const ERec* __restrict_
     __shared__ double red[2 * (NT / 32)];
     const int tid = threadIdx.x;
     const int i = blockIdx.x * NT + tid;
+    constexpr int kEGroup = 8;
+    static_assert(TJ % kEGroup == 0, "tile must be a multiple of the summation group");
     const ERec me = erec[i];
     const double mi = me.gm / G;
+    const double wi1 = me.w - 1.0, c35 = 3.5 * inv_c2, c05 = 0.5 * inv_c2;
     double hi = 0, lo = 0;
 
     static_assert(NT == TJ, "i-tiles and j-tiles share one index space");
@@ -875,24 +878,36 @@ __global__ void __launch_bounds__(NT) energy_pair_kernel(const ERec* __restrict_
         }
         __syncthreads();
         const int j0 = t * TJ;
-#pragma unroll 2
-        for (int jj = 0; jj < TJ; ++jj) {
-            const ERec r = sj[jj];
-            const double dx = me.x - r.x, dy = me.y - r.y, dz = me.z - r.z;  // x_ij
-            const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
-            const double y0 = rsqrt_seed(r2);
-            const double t2 = y0 * y0;
-            const double e = fma(-r2, t2, 1.0);
-            const double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1/rho to full fp64 accuracy
-            const double vv = me.vx * r.vx + me.vy * r.vy + me.vz * r.vz;
-            const double xvi = dx * me.vx + dy * me.vy + dz * me.vz;
-            const double xvj = dx * r.vx + dy * r.vy + dz * r.vz;
-            const double br = me.w + r.w - 3.5 * vv - 0.5 * xvi * xvj * (y * y);
-            double term = (mi * r.gm * y) * (-1.0 + inv_c2 * br);
-            term = (j0 + jj <= i) ? 0.0 : term;  // i < j only (false only inside the diagonal tile)
-            two_sum_acc(hi, lo, term);
+#pragma unroll 1
+        for (int jb = 0; jb < TJ; jb += kEGroup) {
+            // kEGroup terms are added plainly (their sum is tiny next to the running total), then the group sum goes
+            // into the compensated accumulator: one TwoSum per kEGroup pairs instead of one per pair
+            double g = 0.0;
+#pragma unroll
+            for (int u = 0; u < kEGroup; ++u) {
+                const int jj = jb + u;
+                const ERec r = sj[jj];
+                const double dx = me.x - r.x, dy = me.y - r.y, dz = me.z - r.z;  // x_ij
+                const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+                const double y0 = rsqrt_seed(r2);
+                const double t2 = y0 * y0;
+                const double e = fma(-r2, t2, 1.0);
+                const double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1/rho to full fp64 accuracy
+                const double vv = fma(me.vx, r.vx, fma(me.vy, r.vy, me.vz * r.vz));
+                const double xvi = fma(dx, me.vx, fma(dy, me.vy, dz * me.vz));
+                const double xvj = fma(dx, r.vx, fma(dy, r.vy, dz * r.vz));
+                // q = -1 + (1/c^2)[w_i + w_j - 7/2 v_i.v_j - 1/2 (x_ij.v_i)(x_ij.v_j)/rho^2]; me.w, r.w carry the 1/c^2
+                double q = wi1 + r.w;
+                q = fma(-c35, vv, q);
+                q = fma(-c05, (xvi * xvj) * (y * y), q);
+                double term = (r.gm * y) * q;
+                term = (j0 + jj <= i) ? 0.0 : term;  // i < j only (false only inside the diagonal tile)
+                g += term;
+            }
+            two_sum_acc(hi, lo, g);
         }
     }
+    hi *= mi, lo *= mi;  // the factor m_i is common to all of thread i's pairs
     if (i >= n_stars) hi = 0, lo = 0;
     block_sum_dd<NT>(hi, lo, red);
     if (tid == 0) {

@@ -28,7 +28,7 @@ def _sample_rows(p, n, seed=4242):
     return np.unique(np.concatenate([rows, [e for e in extra if e < p.N]])).astype(np.int64)
 
 
-def _check_sampled(p, n_rows, precision=None, tol=TOL_ACC):
+def _check_sampled(p, n_rows, precision=None, tol=TOL_ACC, kernel=None):
     from paper_1801_07986_b200 import PN, binding
 
     rows = _sample_rows(p, n_rows)
@@ -36,6 +36,8 @@ def _check_sampled(p, n_rows, precision=None, tol=TOL_ACC):
     with PN(p.mass, p.G, p.c, p.softening) as pn:
         if precision is not None:
             pn.pn_set_option(binding.PN_OPT_PAIR_PRECISION, precision)
+        if kernel is not None:
+            pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, kernel)
         acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
         cfg = pn.pn_get_pair_config()
     assert np.isfinite(acc).all()
@@ -55,6 +57,24 @@ def test_config3_cusp_full_size_sampled_rows():
 
 def test_config4_full_size_sampled_rows():
     _check_sampled(inputs.config(4), 256)
+
+
+def test_config3_full_size_tiled_kernel_and_fp32_variant():
+    """The kernels the automatic choice does not pick at this size (N_s >= 49152: symmetric, U = 512)."""
+    from paper_1801_07986_b200 import binding
+
+    p = inputs.config(3)
+    a_tiled = _check_sampled(p, 256, kernel=binding.PN_PAIR_TILED)
+    a_sym = _check_sampled(p, 256, kernel=binding.PN_PAIR_SYMMETRIC)
+    assert rel_err_rows(a_sym[1:], a_tiled[1:]).max() <= 1e-12  # every row, not only the sampled ones
+    a32 = _check_sampled(p, 256, precision=binding.PN_FP32_PAIR, tol=TOL_FP32)
+    assert rel_err_rows(a32[1:], a_tiled[1:]).max() <= TOL_FP32
+
+
+def test_config4_full_size_fp32_variant():
+    from paper_1801_07986_b200 import binding
+
+    _check_sampled(inputs.config(4), 128, precision=binding.PN_FP32_PAIR, tol=TOL_FP32)
 
 
 @pytest.mark.parametrize("k", [10, 14, 17])
