@@ -55,11 +55,11 @@ extern "C" {
 #define PN_FP64 0      /* fp64 pair arithmetic and accumulation (parity 1e-12) */
 #define PN_FP32_PAIR 1 /* fp32 pair arithmetic on two-float positions, fp64 accumulation (parity 1e-5) */
 
-/* PN_OPT_PAIR_KERNEL values (fp64 pair arithmetic only; PN_FP32_PAIR always uses the tiled form) */
+/* PN_OPT_PAIR_KERNEL values (either pair precision) */
 #define PN_PAIR_AUTO 0      /* symmetric for N - 1 >= 3072 stars, tiled below */
-#define PN_PAIR_TILED 1     /* every ordered pair (i, j): 15 FP64 instructions per ordered pair */
+#define PN_PAIR_TILED 1     /* every ordered pair (i, j): 15 FP64 (18 FP32) instructions per ordered pair */
 #define PN_PAIR_SYMMETRIC 2 /* every unordered pair once, applied to both stars (Newton's third law, exact for the
-                               softened Newtonian term of Eq. 2.4): 10 FP64 instructions per ordered pair */
+                               softened Newtonian term of Eq. 2.4): 10 FP64 (11 FP32) instructions per ordered pair */
 
 typedef struct pn_ctx pn_ctx; /* opaque; owns all internal device buffers */
 
@@ -99,7 +99,7 @@ int pn_get_pair_time(pn_ctx* ctx, double* ms_total_host, int64_t* n_launches_hos
 int pn_get_pair_config(pn_ctx* ctx, int32_t* cfg_host); /* 8 ints: threads/block, i per thread, j-tile, partial-sum
                                                            slots (j-splits / groups), grid blocks, padded N_s, pipe
                                                            instructions per ordered pair, variant (0 fp64 tiled,
-                                                           1 fp32-pair, 2 fp64 symmetric) */
+                                                           1 fp32 tiled, 2 fp64 symmetric, 3 fp32 symmetric) */
 
 int pn_measure_fp64_peak(pn_ctx* ctx, double* tflops_host); /* sustained FP64 FMA rate of this device from a register-only
                                                               DFMA-chain kernel (2 flops per FMA), best of 3: the measured

@@ -134,7 +134,6 @@ void choose_sym_groups(pn_ctx* c)
 
 bool use_sym(const pn_ctx* c)
 {
-    if (c->precision != PN_FP64) return false;
     if (c->kernel_opt == PN_PAIR_SYMMETRIC) return true;
     if (c->kernel_opt == PN_PAIR_TILED) return false;
     return c->n_stars >= 3072;
@@ -167,6 +166,27 @@ cudaError_t prepare_sym()
 }
 
 template <int I, int W, int MINB>
+cudaError_t prepare_sym32()
+{
+    cudaError_t e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         kSymSmemBytes<I, W>);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                kSymSmemBytes<I, W>);
+}
+
+template <int I, int W, int MINB>
+void launch_pair_sym32(pn_ctx* c, cudaStream_t st)
+{
+    const int blocks = c->sym_G * (c->sym_G + 1) / 2;
+    const float e2 = (float)c->eps2;
+    if (c->eps2 == 0.0)
+        pair_sym_fp32_kernel<I, W, MINB, true><<<blocks, 32 * W, kSymSmemBytes<I, W>, st>>>(c->frec, c->part, c->np, c->sym_T, c->sym_m, e2);
+    else
+        pair_sym_fp32_kernel<I, W, MINB, false><<<blocks, 32 * W, kSymSmemBytes<I, W>, st>>>(c->frec, c->part, c->np, c->sym_T, c->sym_m, e2);
+}
+
+template <int I, int W, int MINB>
 void launch_pair_sym(pn_ctx* c, int set, cudaStream_t st)
 {
     const int blocks = c->sym_G * (c->sym_G + 1) / 2;
@@ -196,7 +216,14 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
         PN_CUDA(c, cudaGetLastError());
         dim3 grid(c->n_itiles, c->n_split);
         const float e2 = (float)c->eps2;
-        if (c->ipt == 2)
+        if (use_sym(c)) {
+            if (c->sym_I == 2)
+                launch_pair_sym32<2, 1, 16>(c, st);
+            else if (c->sym_W == 1)
+                launch_pair_sym32<4, 1, 12>(c, st);
+            else
+                launch_pair_sym32<4, 4, 4>(c, st);
+        } else if (c->ipt == 2)
             mask ? pair_fp32_kernel<2, kNT, kTJ, 32, true><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2)
                  : pair_fp32_kernel<2, kNT, kTJ, 32, false><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2);
         else
@@ -351,6 +378,9 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA((prepare_sym<2, 1, 16>()));
     CREATE_CUDA((prepare_sym<4, 1, 8>()));
     CREATE_CUDA((prepare_sym<4, 4, 3>()));
+    CREATE_CUDA((prepare_sym32<2, 1, 16>()));
+    CREATE_CUDA((prepare_sym32<4, 1, 12>()));
+    CREATE_CUDA((prepare_sym32<4, 4, 4>()));
     CREATE_CUDA(dalloc(&ctx->part, (size_t)std::max(ctx->max_split, ctx->sym_G) * 3 * np));
     CREATE_CUDA(dalloc(&ctx->bh_part, 3 * (np / kEpiStars)));
     CREATE_CUDA(dalloc(&ctx->ticket, 1));
@@ -642,7 +672,8 @@ int pn_get_pair_config(pn_ctx* c, int32_t* cfg)
     if (!cfg) return fail(c, PN_EINVAL, "pn_get_pair_config: null pointer");
     if (use_sym(c)) {
         cfg[0] = 32 * c->sym_W, cfg[1] = c->sym_I, cfg[2] = c->sym_U, cfg[3] = c->sym_G;
-        cfg[4] = c->sym_G * (c->sym_G + 1) / 2, cfg[5] = c->np, cfg[6] = 10, cfg[7] = 2;
+        cfg[4] = c->sym_G * (c->sym_G + 1) / 2, cfg[5] = c->np;
+        cfg[6] = (c->precision == PN_FP32_PAIR) ? 11 : 10, cfg[7] = (c->precision == PN_FP32_PAIR) ? 3 : 2;
         return PN_OK;
     }
     cfg[0] = kNT, cfg[1] = c->ipt, cfg[2] = kTJ, cfg[3] = c->n_split;

@@ -296,6 +296,30 @@ __device__ __forceinline__ void sym_unit_tile(const double2* __restrict__ sxy, c
     }
 }
 
+// triangular decode of the block index: (A <= B), blockIdx.x = B (B + 1) / 2 + A
+__device__ __forceinline__ void sym_decode_block(int& A, int& B)
+{
+    B = (int)((sqrtf(8.0f * (float)blockIdx.x + 1.0f) - 1.0f) * 0.5f);
+    while ((B + 1) * (B + 2) / 2 <= (int)blockIdx.x) ++B;
+    while (B * (B + 1) / 2 > (int)blockIdx.x) --B;
+    A = (int)blockIdx.x - B * (B + 1) / 2;
+}
+
+// adds n_src block-owned [3][U] tiles (consecutive in shared memory) into one (slot, tile) of part; the same thread
+// handles the same elements on every call, so read-modify-write sequences of one block need no fence
+template <int U, int NT>
+__device__ __forceinline__ void sym_flush(const double* __restrict__ cacc, double* __restrict__ dst, int np, bool first,
+                                          int n_src)
+{
+    for (int q = threadIdx.x; q < 3 * U; q += NT) {
+        const int c = q / U, el = q - c * U;
+        double v = cacc[q];
+        for (int s = 1; s < n_src; ++s) v += cacc[s * 3 * U + q];
+        double* d = dst + (size_t)c * np + el;
+        *d = first ? v : *d + v;
+    }
+}
+
 template <int I, int W>
 constexpr int kSymSmemBytes = (W * 32 * I) * (2 * 16 + W * 3 * 8);
 
@@ -312,26 +336,15 @@ __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp64_kernel(const JRec*
     double(*cacc)[3][U] = reinterpret_cast<double(*)[3][U]>(sym_smem + 2 * U);  // [W][3][U] per-warp column sums
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
 
-    // triangular decode of the block index: (A <= B), blockIdx.x = B (B + 1) / 2 + A
-    int B = (int)((sqrtf(8.0f * (float)blockIdx.x + 1.0f) - 1.0f) * 0.5f);
-    while ((B + 1) * (B + 2) / 2 <= (int)blockIdx.x) ++B;
-    while (B * (B + 1) / 2 > (int)blockIdx.x) --B;
-    const int A = (int)blockIdx.x - B * (B + 1) / 2;
+    int A, B;
+    sym_decode_block(A, B);
 
     const int ta0 = A * m, ta1 = min(ta0 + m, n_tiles);
     const int tb0 = B * m, tb1 = min(tb0 + m, n_tiles);
     const int i_local0 = w * 32 * I + lane;  // this lane's k-th i-star is i_local0 + 32 k inside the unit tile
 
-    // sums a block-owned [3][U] tile into slot `slot` of part (same thread <-> same elements on every call)
     auto flush = [&](int slot, int tile, bool first, int n_src) {
-        double* dst = part + (size_t)slot * 3 * np + (size_t)tile * U;
-        for (int q = tid; q < 3 * U; q += NT) {
-            const int c = q / U, el = q - c * U;
-            double v = cacc[0][c][el];
-            for (int s = 1; s < n_src; ++s) v += cacc[s][c][el];
-            double* d = dst + (size_t)c * np + el;
-            *d = first ? v : *d + v;
-        }
+        sym_flush<U, NT>(&cacc[0][0][0], part + (size_t)slot * 3 * np + (size_t)tile * U, np, first, n_src);
     };
 
     for (int ta = ta0; ta < ta1; ++ta) {
@@ -478,6 +491,126 @@ __global__ void __launch_bounds__(NT) pair_fp32_kernel(const FRec* __restrict__ 
         out[ii[k]] = ax[k];
         out[np + ii[k]] = ay[k];
         out[2 * np + ii[k]] = az[k];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// S1 variant, symmetric form: fp32 pair arithmetic on two-float positions, every unordered pair once (same
+// decomposition, rotation and slot scheme as pair_sym_fp64_kernel).  Per unordered pair: 9 FADD + 9 FFMA + 4 FMUL =
+// 22 FP32-pipe instructions + 1 MUFU.RSQ (11 per ordered pair; the tiled form needs 18).  The i-side fp32 sums run
+// over the 32 steps of one rotation, the j-side sums over its 32 I terms; both are then added in fp64.
+// ---------------------------------------------------------------------------------------------------------
+template <int I, int W, bool SYM, bool MASK>
+__device__ __forceinline__ void sym32_unit_tile(const float4* __restrict__ shi, const float4* __restrict__ slo,
+                                                double* __restrict__ cw, const float (&xh)[I], const float (&yh)[I],
+                                                const float (&zh)[I], const float (&xl)[I], const float (&yl)[I],
+                                                const float (&zl)[I], const float (&ngi)[I], double (&ax)[I],
+                                                double (&ay)[I], double (&az)[I], float eps2, int lane, int i_local0)
+{
+    constexpr int U = W * 32 * I;
+#pragma unroll 1
+    for (int jb = 0; jb < U; jb += 32) {
+        float fx[I], fy[I], fz[I];
+#pragma unroll
+        for (int k = 0; k < I; ++k) fx[k] = fy[k] = fz[k] = 0.f;
+        float bx = 0.f, by = 0.f, bz = 0.f;
+        constexpr int kUnr = (I >= 4) ? 4 : 16 / I;
+#pragma unroll kUnr
+        for (int r = 0; r < 32; ++r) {
+            const int jj = jb + ((lane + r) & 31);
+            const float4 h = shi[jj], l = slo[jj];
+#pragma unroll
+            for (int k = 0; k < I; ++k) {
+                const float dx = (h.x - xh[k]) + (l.x - xl[k]);
+                const float dy = (h.y - yh[k]) + (l.y - yl[k]);
+                const float dz = (h.z - zh[k]) + (l.z - zl[k]);
+                const float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, eps2)));
+                const float y = rsqrt_seed_f32(r2);
+                float K = (y * y) * y;
+                if (MASK) K = (jj == i_local0 + 32 * k) ? 0.f : K;
+                const float sj = K * h.w;
+                fx[k] = fmaf(sj, dx, fx[k]);
+                fy[k] = fmaf(sj, dy, fy[k]);
+                fz[k] = fmaf(sj, dz, fz[k]);
+                if (SYM) {
+                    const float si = K * ngi[k];
+                    bx = fmaf(si, dx, bx);
+                    by = fmaf(si, dy, by);
+                    bz = fmaf(si, dz, bz);
+                }
+            }
+            if (SYM) {
+                const int src = (lane + 1) & 31;
+                bx = __shfl_sync(0xffffffffu, bx, src);
+                by = __shfl_sync(0xffffffffu, by, src);
+                bz = __shfl_sync(0xffffffffu, bz, src);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < I; ++k) ax[k] += (double)fx[k], ay[k] += (double)fy[k], az[k] += (double)fz[k];
+        if (SYM) {
+            cw[jb + lane] = (double)bx;
+            cw[U + jb + lane] = (double)by;
+            cw[2 * U + jb + lane] = (double)bz;
+        }
+    }
+}
+
+template <int I, int W, int MINB, bool MASK>
+__global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp32_kernel(const FRec* __restrict__ frec,
+                                                                     double* __restrict__ part, int np, int n_tiles,
+                                                                     int m, float eps2)
+{
+    constexpr int U = W * 32 * I;
+    constexpr int NT = W * 32;
+    extern __shared__ double2 sym_smem[];  // kSymSmemBytes<I, W>
+    float4* shi = reinterpret_cast<float4*>(sym_smem);      // [U] high parts, G m
+    float4* slo = reinterpret_cast<float4*>(sym_smem + U);  // [U] low parts
+    double(*cacc)[3][U] = reinterpret_cast<double(*)[3][U]>(sym_smem + 2 * U);
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    int A, B;
+    sym_decode_block(A, B);
+    const int ta0 = A * m, ta1 = min(ta0 + m, n_tiles);
+    const int tb0 = B * m, tb1 = min(tb0 + m, n_tiles);
+    const int i_local0 = w * 32 * I + lane;
+    auto flush = [&](int slot, int tile, bool first, int n_src) {
+        sym_flush<U, NT>(&cacc[0][0][0], part + (size_t)slot * 3 * np + (size_t)tile * U, np, first, n_src);
+    };
+
+    for (int ta = ta0; ta < ta1; ++ta) {
+        float xh[I], yh[I], zh[I], xl[I], yl[I], zl[I], ngi[I];
+        double ax[I], ay[I], az[I];
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            const FRec f = frec[(size_t)ta * U + i_local0 + 32 * k];
+            xh[k] = f.xh, yh[k] = f.yh, zh[k] = f.zh, xl[k] = f.xl, yl[k] = f.yl, zl[k] = f.zl, ngi[k] = -f.gm;
+            ax[k] = ay[k] = az[k] = 0.0;
+        }
+        for (int tb = (A == B) ? ta : tb0; tb < tb1; ++tb) {
+            __syncthreads();
+            for (int q = tid; q < U; q += NT) {
+                const float4* src = reinterpret_cast<const float4*>(frec + (size_t)tb * U + q);
+                shi[q] = src[0];
+                slo[q] = src[1];
+            }
+            __syncthreads();
+            if (ta == tb) {
+                sym32_unit_tile<I, W, false, MASK>(shi, slo, &cacc[w][0][0], xh, yh, zh, xl, yl, zl, ngi, ax, ay, az, eps2, lane, i_local0);
+            } else {
+                sym32_unit_tile<I, W, true, false>(shi, slo, &cacc[w][0][0], xh, yh, zh, xl, yl, zl, ngi, ax, ay, az, eps2, lane, i_local0);
+                __syncthreads();
+                flush(A, tb, ta == ta0, W);
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            cacc[0][0][i_local0 + 32 * k] = ax[k];
+            cacc[0][1][i_local0 + 32 * k] = ay[k];
+            cacc[0][2][i_local0 + 32 * k] = az[k];
+        }
+        __syncthreads();
+        flush(B, ta, (A < B) || (ta == ta0), 1);
     }
 }
 

@@ -67,8 +67,9 @@ def test_config3_full_size_tiled_kernel_and_fp32_variant():
     a_tiled = _check_sampled(p, 256, kernel=binding.PN_PAIR_TILED)
     a_sym = _check_sampled(p, 256, kernel=binding.PN_PAIR_SYMMETRIC)
     assert rel_err_rows(a_sym[1:], a_tiled[1:]).max() <= 1e-12  # every row, not only the sampled ones
-    a32 = _check_sampled(p, 256, precision=binding.PN_FP32_PAIR, tol=TOL_FP32)
-    assert rel_err_rows(a32[1:], a_tiled[1:]).max() <= TOL_FP32
+    for kernel in (binding.PN_PAIR_TILED, binding.PN_PAIR_SYMMETRIC):
+        a32 = _check_sampled(p, 256, precision=binding.PN_FP32_PAIR, tol=TOL_FP32, kernel=kernel)
+        assert rel_err_rows(a32[1:], a_tiled[1:]).max() <= TOL_FP32
 
 
 def test_config4_full_size_fp32_variant():
@@ -129,23 +130,27 @@ def test_config3_energy_full_size():
 
 
 # ------------------------------------------------------------------ fp32-pair / fp64-accumulate variant
+@pytest.mark.parametrize("kernel", ["tiled", "symmetric"])
 @pytest.mark.parametrize("n_stars", [2, 129, 1023, 4099, 13001])
-def test_fp32_pair_variant_parity(n_stars):
+def test_fp32_pair_variant_parity(n_stars, kernel):
     from paper_1801_07986_b200 import binding
+
+    kernel = binding.PN_PAIR_TILED if kernel == "tiled" else binding.PN_PAIR_SYMMETRIC
 
     if n_stars == 2:  # two equal-mass recentred stars make a_1 pure rounding noise: use unequal masses instead
         p = inputs.random_small(2, seed=302, M=1.0, m_scale=1e-2, c=10.0, softening=1e-3)
     else:
         p = inputs.plummer_bh(n_stars, seed=300 + n_stars)
-    _check_sampled(p, 4096, precision=binding.PN_FP32_PAIR, tol=TOL_FP32)
+    _check_sampled(p, 4096, precision=binding.PN_FP32_PAIR, tol=TOL_FP32, kernel=kernel)
 
 
 def test_fp32_pair_variant_cusp_and_zero_softening():
     from paper_1801_07986_b200 import binding
 
-    _check_sampled(inputs.cusp_bh(6000, seed=2), 6000, precision=binding.PN_FP32_PAIR, tol=TOL_FP32)
-    p = inputs.random_small(500, seed=31, M=1.0, m_scale=1e-3, c=20.0, softening=0.0)
-    _check_sampled(p, 500, precision=binding.PN_FP32_PAIR, tol=TOL_FP32)
+    for kernel in (binding.PN_PAIR_TILED, binding.PN_PAIR_SYMMETRIC):
+        _check_sampled(inputs.cusp_bh(6000, seed=2), 6000, precision=binding.PN_FP32_PAIR, tol=TOL_FP32, kernel=kernel)
+        p = inputs.random_small(500, seed=31, M=1.0, m_scale=1e-3, c=20.0, softening=0.0)
+        _check_sampled(p, 500, precision=binding.PN_FP32_PAIR, tol=TOL_FP32, kernel=kernel)
 
 
 def test_fp32_pair_variant_full_size_config2_and_switching_back():
