@@ -241,6 +241,24 @@ def run_reference(args) -> None:
     print(json.dumps(line), flush=True)
 
 
+def max_over_ranks(values, world: int, device):
+    """Per-rank timings -> the slowest rank's (the contract's max over ranks); any torch.distributed backend."""
+    import torch
+
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def whole_job_rate(world: int, steps: int, pairs_per_step: int, seconds: float) -> float:
+    """Replicas only: every rank processes the same number of pairs; the job's rate is all of them
+    over the slowest rank's time."""
+    return world * steps * pairs_per_step / seconds
+
+
 def workload_config(p, args) -> dict:
     return {"workload": p.name, "N": p.N, "n_stars": p.n_stars, "pairs_per_force_eval": p.pairs_per_eval,
             "force_evals_per_step": 4, "dt": p.dt, "c": p.c, "softening": p.softening, "M": float(p.mass[0]),
@@ -349,12 +367,9 @@ def run_ours(args) -> None:
 
     # ---------------- max over ranks, whole-job aggregate
     pairs_per_step = 4 * p.pairs_per_eval
-    t = torch.tensor([ms_total, ms_steps, e2e_s, ms_graph], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total_m, ms_steps_m, e2e_m, ms_graph_m = t.tolist()
-    value = world * K * pairs_per_step / (ms_total_m * 1e-3)
-    e2e_val = world * K * pairs_per_step / e2e_m
+    ms_total_m, ms_steps_m, e2e_m, ms_graph_m = max_over_ranks([ms_total, ms_steps, e2e_s, ms_graph], world, "cuda")
+    value = whole_job_rate(world, K, pairs_per_step, ms_total_m * 1e-3)
+    e2e_val = whole_job_rate(world, K, pairs_per_step, e2e_m)
 
     if rank == 0:
         peaks = load_peaks()
@@ -388,7 +403,7 @@ def run_ours(args) -> None:
             "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(p, args),
             "steps_per_s": world * K / (ms_total_m * 1e-3), "rk4_only_ms_per_step": ms_steps_m / K,
             "energy_ms_per_eval": ms_energy / 2, "graph_ms_per_step": ms_graph_m / K,
-            "graph_pairs_per_s": world * K * pairs_per_step / (ms_graph_m * 1e-3),
+            "graph_pairs_per_s": whole_job_rate(world, K, pairs_per_step, ms_graph_m * 1e-3),
             "energy_drift": (e_end - e_start) / abs(e_start), "pair_config": cfg,
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": "pair-interactions/s", "h2d_bytes_per_step": 2 * p.N * 24,
