@@ -31,7 +31,10 @@ if str(ROOT) not in sys.path:
 # SASS (cuobjdump-verified; the library reports the same number), executed flops per ordered pair (FMA = 2, MUL/ADD = 1):
 #   0 tiled:     3 DADD + 9 DFMA + 3 DMUL = 15 per ordered pair (+1 MUFU.RSQ64H)
 #   2 symmetric: 3 DADD + 12 DFMA + 5 DMUL = 20 per UNORDERED pair (+1 MUFU.RSQ64H) = 10 per ordered pair
-PAIR_KERNELS = {0: ("pair_fp64_kernel", 15, 24.0), 2: ("pair_sym_fp64_kernel", 10, 16.0)}
+#   4 symmetric, equal-mass form (every star has the same mass, as in every BASELINE.json config): the two mass
+#     multiplications go: 3 DADD + 12 DFMA + 3 DMUL = 18 per unordered pair = 9 per ordered pair
+PAIR_KERNELS = {0: ("pair_fp64_kernel", 15, 24.0), 2: ("pair_sym_fp64_kernel", 10, 16.0),
+                4: ("pair_sym_fp64_kernel<EQM>", 9, 15.0)}
 SMS, FP64_LANES_PER_SM = 148, 64
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu --set full
 # captures (profiles/), keyed by (variant, N_s); null when no capture exists for the workload

@@ -34,7 +34,9 @@ struct pn_ctx {
     std::string err;
 
     // options
-    int precision = PN_FP64, use_graph = 1, time_pair = 0, j_split_opt = 0, kernel_opt = PN_PAIR_AUTO;
+    int precision = PN_FP64, use_graph = 1, time_pair = 0, j_split_opt = 0, kernel_opt = PN_PAIR_AUTO, eqm_opt = 1;
+    bool equal_mass = false;  // every star has the same mass > 0
+    double gm_eq = 0;
 
     // pair-kernel launch configuration
     int ipt = 1, n_itiles = 0, n_tiles = 0, n_split = 1, tiles_per_split = 0, max_split = 1;
@@ -60,7 +62,7 @@ struct pn_ctx {
     double dt_dev = NAN;
 
     cudaGraphExec_t graph1 = nullptr, graphB = nullptr;
-    int graph_split = -1, graph_precision = -1, graph_sym = -1;
+    int graph_split = -1, graph_precision = -1, graph_sym = -1, graph_eqm = -1;
 
     int64_t n_launch = 0;
     std::vector<cudaEvent_t> ev;  // pairs (start, stop)
@@ -139,6 +141,8 @@ bool use_sym(const pn_ctx* c)
     return c->n_stars >= 3072;
 }
 
+bool use_eqm(const pn_ctx* c) { return c->equal_mass && c->eqm_opt && c->precision == PN_FP64 && use_sym(c); }
+
 int active_split(const pn_ctx* c) { return use_sym(c) ? c->sym_G : c->n_split; }
 
 void destroy_graphs(pn_ctx* c)
@@ -155,47 +159,47 @@ void launch_pair_fp64(pn_ctx* c, int set, cudaStream_t st)
     pair_fp64_kernel<I, JU, MINB, kNT, kTJ, MASK><<<grid, kNT, 0, st>>>(c->jrec[set], c->part, c->np, c->tiles_per_split, c->eps2);
 }
 
+// symmetric kernels <I, W, MINB>: one block per work item (group pair), W warps
 template <int I, int W, int MINB>
 cudaError_t prepare_sym()
 {
-    cudaError_t e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         kSymSmemBytes<I, W>);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                kSymSmemBytes<I, W>);
-}
-
-template <int I, int W, int MINB>
-cudaError_t prepare_sym32()
-{
-    cudaError_t e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         kSymSmemBytes<I, W>);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                kSymSmemBytes<I, W>);
+    const int bytes = kSymSmemBytes<I, W>;
+    cudaError_t e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    return e;
 }
 
 template <int I, int W, int MINB>
 void launch_pair_sym32(pn_ctx* c, cudaStream_t st)
 {
-    const int blocks = c->sym_G * (c->sym_G + 1) / 2;
+    const int items = c->sym_G * (c->sym_G + 1) / 2;
     const float e2 = (float)c->eps2;
     if (c->eps2 == 0.0)
-        pair_sym_fp32_kernel<I, W, MINB, true><<<blocks, 32 * W, kSymSmemBytes<I, W>, st>>>(c->frec, c->part, c->np, c->sym_T, c->sym_m, e2);
+        pair_sym_fp32_kernel<I, W, MINB, true><<<items, 32 * W, kSymSmemBytes<I, W>, st>>>(c->frec, c->part, c->np, c->sym_T, c->sym_m, e2);
     else
-        pair_sym_fp32_kernel<I, W, MINB, false><<<blocks, 32 * W, kSymSmemBytes<I, W>, st>>>(c->frec, c->part, c->np, c->sym_T, c->sym_m, e2);
+        pair_sym_fp32_kernel<I, W, MINB, false><<<items, 32 * W, kSymSmemBytes<I, W>, st>>>(c->frec, c->part, c->np, c->sym_T, c->sym_m, e2);
+}
+
+template <int I, int W, int MINB, bool MASK, bool EQM>
+void launch_pair_sym_v(pn_ctx* c, int set, cudaStream_t st)
+{
+    const int items = c->sym_G * (c->sym_G + 1) / 2;
+    pair_sym_fp64_kernel<I, W, MINB, MASK, EQM><<<items, 32 * W, kSymSmemBytes<I, W>, st>>>(c->jrec[set], c->part, c->np, c->sym_T,
+                                                                                           c->sym_m, c->eps2, c->gm_eq);
 }
 
 template <int I, int W, int MINB>
 void launch_pair_sym(pn_ctx* c, int set, cudaStream_t st)
 {
-    const int blocks = c->sym_G * (c->sym_G + 1) / 2;
-    if (c->eps2 == 0.0)
-        pair_sym_fp64_kernel<I, W, MINB, true><<<blocks, 32 * W, kSymSmemBytes<I, W>, st>>>(c->jrec[set], c->part, c->np, c->sym_T,
-                                                                                           c->sym_m, c->eps2);
+    const bool mask = (c->eps2 == 0.0), eqm = use_eqm(c);
+    if (mask)
+        eqm ? launch_pair_sym_v<I, W, MINB, true, true>(c, set, st) : launch_pair_sym_v<I, W, MINB, true, false>(c, set, st);
     else
-        pair_sym_fp64_kernel<I, W, MINB, false><<<blocks, 32 * W, kSymSmemBytes<I, W>, st>>>(c->jrec[set], c->part, c->np, c->sym_T,
-                                                                                            c->sym_m, c->eps2);
+        eqm ? launch_pair_sym_v<I, W, MINB, false, true>(c, set, st) : launch_pair_sym_v<I, W, MINB, false, false>(c, set, st);
 }
 
 int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
@@ -220,9 +224,9 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
             if (c->sym_I == 2)
                 launch_pair_sym32<2, 1, 16>(c, st);
             else if (c->sym_W == 1)
-                launch_pair_sym32<4, 1, 12>(c, st);
+                launch_pair_sym32<4, 1, 8>(c, st);
             else
-                launch_pair_sym32<4, 4, 4>(c, st);
+                launch_pair_sym32<4, 4, 3>(c, st);
         } else if (c->ipt == 2)
             mask ? pair_fp32_kernel<2, kNT, kTJ, 32, true><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2)
                  : pair_fp32_kernel<2, kNT, kTJ, 32, false><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2);
@@ -235,7 +239,7 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
         else if (c->sym_W == 1)
             launch_pair_sym<4, 1, 8>(c, set, st);
         else
-            launch_pair_sym<4, 4, 3>(c, set, st);
+            launch_pair_sym<4, 4, 2>(c, set, st);
     } else if (c->ipt == 2)
         mask ? launch_pair_fp64<2, 4, 4, true>(c, set, st) : launch_pair_fp64<2, 4, 4, false>(c, set, st);
     else
@@ -339,6 +343,9 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     ctx->GM = G * masses[0];
     ctx->inv_c2 = std::isinf(c) ? 0.0 : 1.0 / (c * c);
     ctx->eps2 = softening * softening;
+    ctx->equal_mass = masses[1] > 0;
+    for (int64_t i = 2; i < N && ctx->equal_mass; ++i) ctx->equal_mass = (masses[i] == masses[1]);
+    ctx->gm_eq = G * masses[1];
 
     // i per thread: larger i-tiles amortise the shared-memory broadcast; small N needs more blocks instead
     ctx->ipt = ctx->n_stars >= 3072 ? 2 : 1;
@@ -377,10 +384,8 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA(dalloc(&ctx->sv, 3 * np));
     CREATE_CUDA((prepare_sym<2, 1, 16>()));
     CREATE_CUDA((prepare_sym<4, 1, 8>()));
+    CREATE_CUDA((prepare_sym<4, 4, 2>()));
     CREATE_CUDA((prepare_sym<4, 4, 3>()));
-    CREATE_CUDA((prepare_sym32<2, 1, 16>()));
-    CREATE_CUDA((prepare_sym32<4, 1, 12>()));
-    CREATE_CUDA((prepare_sym32<4, 4, 4>()));
     CREATE_CUDA(dalloc(&ctx->part, (size_t)std::max(ctx->max_split, ctx->sym_G) * 3 * np));
     CREATE_CUDA(dalloc(&ctx->bh_part, 3 * (np / kEpiStars)));
     CREATE_CUDA(dalloc(&ctx->ticket, 1));
@@ -464,6 +469,10 @@ int pn_set_option(pn_ctx* c, int key, int value)
             if (value != PN_PAIR_AUTO && value != PN_PAIR_TILED && value != PN_PAIR_SYMMETRIC)
                 return fail(c, PN_EINVAL, "pn_set_option: unknown pair kernel %d", value);
             c->kernel_opt = value;
+            return PN_OK;
+        case PN_OPT_EQUAL_MASS:
+            if (value != 0 && value != 1) return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_EQUAL_MASS takes 0 or 1");
+            c->eqm_opt = value;
             return PN_OK;
         case PN_OPT_J_SPLIT:
             if (value < 0) return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_J_SPLIT must be >= 0");
@@ -572,9 +581,10 @@ int pn_step(pn_ctx* c, double dt, int64_t nsteps)
         c->n_launch += (c->precision == PN_FP32_PAIR ? 12 : 8) * nsteps;
         return PN_OK;
     }
-    if (c->graph_split != c->n_split || c->graph_precision != c->precision || c->graph_sym != (int)use_sym(c)) {
+    if (c->graph_split != c->n_split || c->graph_precision != c->precision || c->graph_sym != (int)use_sym(c) ||
+        c->graph_eqm != (int)use_eqm(c)) {
         destroy_graphs(c);
-        c->graph_split = c->n_split, c->graph_precision = c->precision, c->graph_sym = (int)use_sym(c);
+        c->graph_split = c->n_split, c->graph_precision = c->precision, c->graph_sym = (int)use_sym(c), c->graph_eqm = (int)use_eqm(c);
     }
     int64_t left = nsteps;
     if (left >= kGraphBatch) {
@@ -673,7 +683,8 @@ int pn_get_pair_config(pn_ctx* c, int32_t* cfg)
     if (use_sym(c)) {
         cfg[0] = 32 * c->sym_W, cfg[1] = c->sym_I, cfg[2] = c->sym_U, cfg[3] = c->sym_G;
         cfg[4] = c->sym_G * (c->sym_G + 1) / 2, cfg[5] = c->np;
-        cfg[6] = (c->precision == PN_FP32_PAIR) ? 11 : 10, cfg[7] = (c->precision == PN_FP32_PAIR) ? 3 : 2;
+        cfg[6] = (c->precision == PN_FP32_PAIR) ? 11 : (use_eqm(c) ? 9 : 10);
+        cfg[7] = (c->precision == PN_FP32_PAIR) ? 3 : (use_eqm(c) ? 4 : 2);
         return PN_OK;
     }
     cfg[0] = kNT, cfg[1] = c->ipt, cfg[2] = kTJ, cfg[3] = c->n_split;

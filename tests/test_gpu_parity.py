@@ -81,7 +81,9 @@ def test_accel_parity_other_distributions(gen):
 # both fp64 star-star kernels at every size class: the tiled one (ordered pairs) and the symmetric one (unordered
 # pairs applied to both stars) in its three unit-tile variants (U = 64: N_s < 12288, 128: < 49152, 512 above),
 # with one group per tile (m = 1) and several (9000 -> T = 144, m = 2; 20000 -> T = 157, m = 2, ragged last group)
-@pytest.mark.parametrize("kernel", ["tiled", "symmetric"])
+# "symmetric" on equal-mass stars takes the equal-mass form (variant 4: rho^-3 d accumulated, G m applied at the flush);
+# "symmetric_general" switches that off (variant 2), which is also what unequal masses get.
+@pytest.mark.parametrize("kernel", ["tiled", "symmetric", "symmetric_general"])
 @pytest.mark.parametrize("n_stars", [1, 2, 65, 129, 1023, 3071, 4099, 9000, 13001, 20000])
 def test_accel_parity_both_pair_kernels(n_stars, kernel):
     from paper_1801_07986_b200 import binding
@@ -93,7 +95,11 @@ def test_accel_parity_both_pair_kernels(n_stars, kernel):
     ref = Oracle(p.mass, p.G, p.c, p.softening).accel(p.pos, p.vel)
     with _pn(p) as pn:
         pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, binding.PN_PAIR_TILED if kernel == "tiled" else binding.PN_PAIR_SYMMETRIC)
-        assert pn.pn_get_pair_config()["variant"] == (0 if kernel == "tiled" else 2)
+        if kernel == "symmetric_general":
+            pn.pn_set_option(binding.PN_OPT_EQUAL_MASS, 0)
+        equal = n_stars != 2  # plummer_bh: equal masses (one star trivially so); random_small(2): unequal
+        want = 0 if kernel == "tiled" else (4 if (kernel == "symmetric" and equal) else 2)
+        assert pn.pn_get_pair_config()["variant"] == want
         acc = _gpu_accel(pn, p.pos, p.vel)
         again = _gpu_accel(pn, p.pos, p.vel)
     assert rel_err_rows(acc, ref).max() <= TOL_ACC
@@ -103,7 +109,7 @@ def test_accel_parity_both_pair_kernels(n_stars, kernel):
 def test_pair_kernels_agree_and_auto_selection():
     from paper_1801_07986_b200 import binding
 
-    for n_stars, want in ((3071, 0), (3072, 2)):
+    for n_stars, want in ((3071, 0), (3072, 4)):
         p = inputs.plummer_bh(n_stars, seed=12)
         with _pn(p) as pn:
             assert pn.pn_get_pair_config()["variant"] == want
@@ -125,6 +131,19 @@ def test_accel_zero_softening_masks_self_pair(n_stars, kernel):
     ref = Oracle(p.mass, p.G, p.c, 0.0).accel(p.pos, p.vel)
     with _pn(p) as pn:
         pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, binding.PN_PAIR_TILED if kernel == "tiled" else binding.PN_PAIR_SYMMETRIC)
+        acc = _gpu_accel(pn, p.pos, p.vel)
+    assert np.isfinite(acc).all()
+    assert rel_err_rows(acc, ref).max() <= TOL_ACC
+
+
+def test_accel_zero_softening_equal_mass_form():
+    """eps = 0 on equal-mass stars: the self-pair mask inside the equal-mass form of the symmetric kernel."""
+    from paper_1801_07986_b200 import binding
+
+    p = inputs.plummer_bh(4099, seed=61, softening=0.0)
+    ref = Oracle(p.mass, p.G, p.c, 0.0).accel(p.pos, p.vel)
+    with _pn(p) as pn:
+        assert pn.pn_get_pair_config()["variant"] == 4
         acc = _gpu_accel(pn, p.pos, p.vel)
     assert np.isfinite(acc).all()
     assert rel_err_rows(acc, ref).max() <= TOL_ACC
