@@ -15,8 +15,8 @@
  *   rho_ij = sqrt(r_ij^2 + eps^2) for star-star pairs only (Eq. 4.2;
  *   DESIGN.md reading R9).
  *
- * What is computed (hot path only; the "Cross" terms, Eqs. 2.3 and 2.6, are NOT included,
- * see DESIGN.md "Scope"):
+ * What is computed (hot path; the "Cross" terms, Eqs. 2.3 and 2.6, are the NEXT rows of the scope table and are
+ * added only when asked for through the *_terms entry points, see below and DESIGN.md "Scope"):
  *   oracle_accel   a_1 : Eq. 2.1 Newtonian term + (1/c^2)[a_1]_BH, Eq. 2.2
  *                  a_i : Eq. 2.4 first two terms + (1/c^2)[a_i]_BH
  *   oracle_step    classical 4th-order Runge-Kutta on (x, v) of all N bodies
@@ -151,19 +151,128 @@ static void accel_star(int64_t N, const real* m, real G, real inv_c2, real eps2,
     }
 }
 
+/* ---------------------------------------------------------------------------------------
+ * NEXT rows of the scope table, selected by the `terms` bit mask; terms = 0 is the hot path.
+ *
+ * ORACLE_CROSS_STAR: [a_i]_Cross, Eq. 2.6, line by line as printed (x_ab = x_a - x_b,
+ * v_ij = v_i - v_j: reading R1; "sum_i" of the last line -> sum_j: reading A6; j != i in every sum):
+ *   L0  5 G^2 m_i M x_i1 / r_i1^4 - (G m_i / r_i1^3) [ 4 v_i^2 x_i1 - 7 (v_i.x_i1) v_i ]
+ *   L1  sum_j G^2 m_j M x_i1 / r_i1^3 ( 4/r_ij + 5/(4 r_j1) + r_i1^2/(4 r_j1^3) - r_ij^2/(4 r_j1^3) )
+ *   L2  sum_j G^2 m_j M x_ij / r_ij^3 ( 4/r_i1 + 5/(4 r_j1) - r_i1^2/(4 r_j1^3) + r_ij^2/(4 r_j1^3) )
+ *   L3  -(7/2) sum_j G^2 m_j M x_j1 / r_j1^3 ( 1/r_ij - 1/r_i1 )
+ *   L4  - sum_j (G m_j / r_i1^3) [ 4 (v_i.v_j) x_i1 - 3 (v_j.x_i1) v_i - 4 (v_i.x_i1) v_j ]
+ *   L5  + sum_j (G m_j x_ij / r_ij^3) [ v_i^2 - 2 |v_ij|^2 + (3/2)(v_j.n_ij)^2 ]
+ *   L6  + sum_j (G m_j / r_ij^3) [ x_ij.(4 v_i - 3 v_j) ] v_ij
+ * Softening (reading R9, a convention, exact at eps = 0): every star-star r_ij above is rho_ij, including the
+ * r_ij^2 in the numerators and n_ij = x_ij / rho_ij; distances to the massive object are never softened.
+ * ------------------------------------------------------------------------------------- */
+#define ORACLE_CROSS_STAR 1
+#define ORACLE_CROSS_BH 2
+
+static void cross_star(int64_t N, const real* m, real G, real eps2, const real* x, const real* v, int64_t i, real* out)
+{
+    const real M = m[0];
+    real xi1[3];
+    for (int k = 0; k < 3; ++k) xi1[k] = x[3 * i + k] - x[k];
+    const real ri1 = R_SQRT(dot3(xi1, xi1));
+    const real ri1_3 = ri1 * ri1 * ri1;
+    const real* vi = v + 3 * i;
+    const real vi2 = dot3(vi, vi);
+    const real vixi1 = dot3(vi, xi1);
+    real acc[3];
+    for (int k = 0; k < 3; ++k) /* L0 */
+        acc[k] = 5 * G * G * m[i] * M * xi1[k] / (ri1_3 * ri1) - G * m[i] / ri1_3 * (4 * vi2 * xi1[k] - 7 * vixi1 * vi[k]);
+    for (int64_t j = 1; j < N; ++j) {
+        if (j == i) continue;
+        real xij[3], xj1[3], vij[3], w[3];
+        for (int k = 0; k < 3; ++k) {
+            xij[k] = x[3 * i + k] - x[3 * j + k];
+            xj1[k] = x[3 * j + k] - x[k];
+            vij[k] = vi[k] - v[3 * j + k];
+            w[k] = 4 * vi[k] - 3 * v[3 * j + k];
+        }
+        const real* vj = v + 3 * j;
+        const real rij2 = dot3(xij, xij) + eps2; /* rho_ij^2 */
+        const real rij = R_SQRT(rij2);
+        const real rij3 = rij2 * rij;
+        const real rj1 = R_SQRT(dot3(xj1, xj1));
+        const real rj1_3 = rj1 * rj1 * rj1;
+        const real f1 = 4 / rij + 5 / (4 * rj1) + ri1 * ri1 / (4 * rj1_3) - rij2 / (4 * rj1_3);
+        const real f2 = 4 / ri1 + 5 / (4 * rj1) - ri1 * ri1 / (4 * rj1_3) + rij2 / (4 * rj1_3);
+        const real vn = dot3(vj, xij) / rij;
+        const real b5 = vi2 - 2 * dot3(vij, vij) + (real)1.5 * vn * vn;
+        const real xw = dot3(xij, w);
+        for (int k = 0; k < 3; ++k) {
+            acc[k] += G * G * m[j] * M * xi1[k] / ri1_3 * f1;                                              /* L1 */
+            acc[k] += G * G * m[j] * M * xij[k] / rij3 * f2;                                               /* L2 */
+            acc[k] -= (real)3.5 * G * G * m[j] * M * xj1[k] / rj1_3 * (1 / rij - 1 / ri1);                 /* L3 */
+            acc[k] -= G * m[j] / ri1_3 * (4 * dot3(vi, vj) * xi1[k] - 3 * dot3(vj, xi1) * vi[k] - 4 * vixi1 * vj[k]); /* L4 */
+            acc[k] += G * m[j] * xij[k] / rij3 * b5;                                                       /* L5 */
+            acc[k] += G * m[j] / rij3 * xw * vij[k];                                                       /* L6 */
+        }
+    }
+    for (int k = 0; k < 3; ++k) out[k] = acc[k];
+}
+
+/* ---------------------------------------------------------------------------------------
+ * ORACLE_CROSS_BH: [a_1]_Cross, Eq. 2.3 (x_1j = x_1 - x_j, x_jk = x_j - x_k; k != j in the sums
+ * that contain r_jk, k = j INCLUDED in the velocity sum: reading A6; star-star r_jk softened as above):
+ *   4 sum_j G^2 m_j^2 x_1j / r_1j^4
+ *   + sum_{j,k} G^2 m_j m_k x_1j / r_1j^3 ( 4/r_1k + 5/(4 r_jk) - r_1k^2/(4 r_jk^3) + r_1j^2/(4 r_jk^3) )
+ *   - (7/2) sum_{j,k} G^2 m_j m_k x_jk / (r_jk^3 r_1j)
+ *   - sum_{j,k} (G m_j m_k / (M r_1j^3)) [ 4 (v_j.v_k) x_1j - 3 (v_j.x_1j) v_k - 4 (v_k.x_1j) v_j ]
+ * ------------------------------------------------------------------------------------- */
+static void cross_bh(int64_t N, const real* m, real G, real eps2, const real* x, const real* v, real* out)
+{
+    const real M = m[0];
+    real acc[3] = {0, 0, 0};
+    for (int64_t j = 1; j < N; ++j) {
+        real x1j[3];
+        for (int q = 0; q < 3; ++q) x1j[q] = x[q] - x[3 * j + q];
+        const real r1j = R_SQRT(dot3(x1j, x1j));
+        const real r1j3 = r1j * r1j * r1j;
+        const real* vj = v + 3 * j;
+        for (int q = 0; q < 3; ++q) acc[q] += 4 * G * G * m[j] * m[j] * x1j[q] / (r1j3 * r1j);
+        for (int64_t k = 1; k < N; ++k) {
+            const real* vk = v + 3 * k;
+            for (int q = 0; q < 3; ++q)
+                acc[q] -= G * m[j] * m[k] / (M * r1j3) *
+                          (4 * dot3(vj, vk) * x1j[q] - 3 * dot3(vj, x1j) * vk[q] - 4 * dot3(vk, x1j) * vj[q]);
+            if (k == j) continue;
+            real x1k[3], xjk[3];
+            for (int q = 0; q < 3; ++q) x1k[q] = x[q] - x[3 * k + q], xjk[q] = x[3 * j + q] - x[3 * k + q];
+            const real r1k = R_SQRT(dot3(x1k, x1k));
+            const real rjk2 = dot3(xjk, xjk) + eps2;
+            const real rjk = R_SQRT(rjk2);
+            const real rjk3 = rjk2 * rjk;
+            const real f = 4 / r1k + 5 / (4 * rjk) - r1k * r1k / (4 * rjk3) + r1j * r1j / (4 * rjk3);
+            for (int q = 0; q < 3; ++q) {
+                acc[q] += G * G * m[j] * m[k] * x1j[q] / r1j3 * f;
+                acc[q] -= (real)3.5 * G * G * m[j] * m[k] * xjk[q] / (rjk3 * r1j);
+            }
+        }
+    }
+    for (int q = 0; q < 3; ++q) out[q] = acc[q];
+}
+
 /* acc[a] for every body a in rows[0..nrows) (rows == NULL: all bodies, nrows == N). */
 static void accel_real(int64_t N, const real* m, real G, real inv_c2, real eps2, const real* x, const real* v,
-                       int64_t nrows, const int64_t* rows, real* acc)
+                       int64_t nrows, const int64_t* rows, int terms, real* acc)
 {
 #ifdef _OPENMP
 #pragma omp parallel for schedule(dynamic, 16)
 #endif
     for (int64_t q = 0; q < nrows; ++q) {
         const int64_t a = rows ? rows[q] : q;
-        if (a == 0)
+        real cr[3] = {0, 0, 0};
+        if (a == 0) {
             accel_bh(N, m, G, inv_c2, x, v, acc + 3 * q);
-        else
+            if (terms & ORACLE_CROSS_BH) cross_bh(N, m, G, eps2, x, v, cr);
+        } else {
             accel_star(N, m, G, inv_c2, eps2, x, v, a, acc + 3 * q);
+            if (terms & ORACLE_CROSS_STAR) cross_star(N, m, G, eps2, x, v, a, cr);
+        }
+        for (int k = 0; k < 3; ++k) acc[3 * q + k] += inv_c2 * cr[k];
     }
 }
 
@@ -186,11 +295,12 @@ static real* to_real(const double* src, int64_t n)
 }
 
 /* pos, vel, acc: host, row-major [N][3] doubles; mass: N doubles, mass[0] = M.  c may be +inf. */
-int oracle_accel_rows(int64_t N, const double* mass, double G, double c, double eps, const double* pos,
-                      const double* vel, int64_t nrows, const int64_t* rows, double* acc_rows)
+int oracle_accel_rows_terms(int64_t N, const double* mass, double G, double c, double eps, const double* pos,
+                            const double* vel, int64_t nrows, const int64_t* rows, int terms, double* acc_rows)
 {
     int rc = check_args(N, mass, G, c, eps);
     if (rc) return rc;
+    if (terms & ~(ORACLE_CROSS_STAR | ORACLE_CROSS_BH)) return ORACLE_EINVAL;
     if (!pos || !vel || !acc_rows || nrows < 0) return ORACLE_EINVAL;
     if (rows)
         for (int64_t q = 0; q < nrows; ++q)
@@ -202,10 +312,16 @@ int oracle_accel_rows(int64_t N, const double* mass, double G, double c, double 
         return ORACLE_ENOMEM;
     }
     const real inv_c2 = 1 / ((real)c * (real)c);
-    accel_real(N, m, (real)G, inv_c2, (real)eps * (real)eps, x, v, nrows, rows, a);
+    accel_real(N, m, (real)G, inv_c2, (real)eps * (real)eps, x, v, nrows, rows, terms, a);
     for (int64_t q = 0; q < 3 * nrows; ++q) acc_rows[q] = (double)a[q];
     free(m), free(x), free(v), free(a);
     return ORACLE_OK;
+}
+
+int oracle_accel_rows(int64_t N, const double* mass, double G, double c, double eps, const double* pos,
+                      const double* vel, int64_t nrows, const int64_t* rows, double* acc_rows)
+{
+    return oracle_accel_rows_terms(N, mass, G, c, eps, pos, vel, nrows, rows, 0, acc_rows);
 }
 
 int oracle_accel(int64_t N, const double* mass, double G, double c, double eps, const double* pos,
@@ -222,11 +338,12 @@ int oracle_accel(int64_t N, const double* mass, double G, double c, double eps, 
  * The acceleration depends on v (1PN), so the velocity stages are formed explicitly.
  * pos, vel are updated in place, nsteps times.
  * ------------------------------------------------------------------------------------- */
-int oracle_step(int64_t N, const double* mass, double G, double c, double eps, double* pos, double* vel,
-                double dt, int64_t nsteps)
+int oracle_step_terms(int64_t N, const double* mass, double G, double c, double eps, double* pos, double* vel,
+                      double dt, int64_t nsteps, int terms)
 {
     int rc = check_args(N, mass, G, c, eps);
     if (rc) return rc;
+    if (terms & ~(ORACLE_CROSS_STAR | ORACLE_CROSS_BH)) return ORACLE_EINVAL;
     if (!pos || !vel || nsteps < 0 || !isfinite(dt)) return ORACLE_EINVAL;
     const int64_t n3 = 3 * N;
     real *m = to_real(mass, N), *x = to_real(pos, n3), *v = to_real(vel, n3);
@@ -247,7 +364,7 @@ int oracle_step(int64_t N, const double* mass, double G, double c, double eps, d
                 vs[q] = st ? v[q] + cstage[st] * h * kv[st - 1][q] : v[q];
             }
             for (int64_t q = 0; q < n3; ++q) kx[st][q] = vs[q];
-            accel_real(N, m, g, inv_c2, eps2, xs, vs, N, NULL, kv[st]);
+            accel_real(N, m, g, inv_c2, eps2, xs, vs, N, NULL, terms, kv[st]);
         }
         for (int64_t q = 0; q < n3; ++q) {
             x[q] += h / 6 * (kx[0][q] + 2 * kx[1][q] + 2 * kx[2][q] + kx[3][q]);
@@ -257,6 +374,12 @@ int oracle_step(int64_t N, const double* mass, double G, double c, double eps, d
     for (int64_t q = 0; q < n3; ++q) pos[q] = (double)x[q], vel[q] = (double)v[q];
     free(m), free(x), free(v), free(w);
     return ORACLE_OK;
+}
+
+int oracle_step(int64_t N, const double* mass, double G, double c, double eps, double* pos, double* vel,
+                double dt, int64_t nsteps)
+{
+    return oracle_step_terms(N, mass, G, c, eps, pos, vel, dt, nsteps, 0);
 }
 
 /* ---------------------------------------------------------------------------------------

@@ -25,6 +25,10 @@ _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "pn_oracle.c"
 _LIBS: dict[str, ctypes.CDLL] = {}
 
+# `terms` bit mask of the NEXT rows; 0 = the hot path
+CROSS_STAR = 1  # [a_i]_Cross, Eq. 2.6
+CROSS_BH = 2    # [a_1]_Cross, Eq. 2.3
+
 N_ENERGY_TERMS = 11
 ENERGY_TERM_NAMES = ("T1", "T2", "T3", "T4", "P1", "P2", "P3", "P4", "P5", "P6", "P7")
 
@@ -75,7 +79,10 @@ def _load(kind: str) -> ctypes.CDLL:
     lib.oracle_accel_rows.argtypes = [i64, dp, dbl, dbl, dbl, dp, dp, i64, ip, dp]
     lib.oracle_step.argtypes = [i64, dp, dbl, dbl, dbl, dp, dp, dbl, i64]
     lib.oracle_energy.argtypes = [i64, dp, dbl, dbl, dbl, dp, dp, dp, dp]
-    for f in (lib.oracle_accel, lib.oracle_accel_rows, lib.oracle_step, lib.oracle_energy):
+    lib.oracle_accel_rows_terms.argtypes = [i64, dp, dbl, dbl, dbl, dp, dp, i64, ip, ctypes.c_int, dp]
+    lib.oracle_step_terms.argtypes = [i64, dp, dbl, dbl, dbl, dp, dp, dbl, i64, ctypes.c_int]
+    for f in (lib.oracle_accel, lib.oracle_accel_rows, lib.oracle_step, lib.oracle_energy, lib.oracle_accel_rows_terms,
+              lib.oracle_step_terms):
         f.restype = ctypes.c_int
     lib.oracle_set_threads.argtypes = [ctypes.c_int]
     lib.oracle_set_threads.restype = None
@@ -105,8 +112,10 @@ def _check(rc: int, what: str):
 class Oracle:
     """The paper's hot path on the host.  Body 0 is the massive object (mass[0] = M)."""
 
-    def __init__(self, mass, G: float, c: float, softening: float, kind: str = "ref", threads: int | None = None):
+    def __init__(self, mass, G: float, c: float, softening: float, kind: str = "ref", threads: int | None = None,
+                 terms: int = 0):
         self.kind = kind
+        self.terms = int(terms)
         self.lib = _load(kind)
         self.mass = np.ascontiguousarray(mass, dtype=np.float64).copy()
         self.N = int(self.mass.shape[0])
@@ -123,10 +132,7 @@ class Oracle:
         return int(self.lib.oracle_mantissa_bits())
 
     def accel(self, pos, vel) -> np.ndarray:
-        n, m, pos, vel = _prep(self.mass, pos, vel)
-        acc = np.empty((n, 3), dtype=np.float64)
-        _check(self.lib.oracle_accel(n, _d(m), self.G, self.c, self.eps, _d(pos), _d(vel), _d(acc)), "oracle_accel")
-        return acc
+        return self.accel_rows(pos, vel, np.arange(self.N, dtype=np.int64))
 
     def accel_rows(self, pos, vel, rows) -> np.ndarray:
         n, m, pos, vel = _prep(self.mass, pos, vel)
@@ -134,8 +140,9 @@ class Oracle:
         acc = np.empty((rows.shape[0], 3), dtype=np.float64)
         rp = rows.ctypes.data_as(ctypes.POINTER(ctypes.c_int64))
         _check(
-            self.lib.oracle_accel_rows(n, _d(m), self.G, self.c, self.eps, _d(pos), _d(vel), rows.shape[0], rp, _d(acc)),
-            "oracle_accel_rows",
+            self.lib.oracle_accel_rows_terms(n, _d(m), self.G, self.c, self.eps, _d(pos), _d(vel), rows.shape[0], rp,
+                                             self.terms, _d(acc)),
+            "oracle_accel_rows_terms",
         )
         return acc
 
@@ -143,7 +150,8 @@ class Oracle:
         """Returns (pos, vel) after nsteps classical-RK4 steps; inputs are not modified."""
         n, m, pos, vel = _prep(self.mass, pos, vel)
         pos, vel = pos.copy(), vel.copy()
-        _check(self.lib.oracle_step(n, _d(m), self.G, self.c, self.eps, _d(pos), _d(vel), float(dt), int(nsteps)), "oracle_step")
+        _check(self.lib.oracle_step_terms(n, _d(m), self.G, self.c, self.eps, _d(pos), _d(vel), float(dt), int(nsteps),
+                                          self.terms), "oracle_step_terms")
         return pos, vel
 
     def energy(self, pos, vel, terms: bool = False):

@@ -345,3 +345,72 @@ def test_invalid_arguments_rejected():
         Oracle([1.0, 1.0], 1.0, 10.0, -1.0).accel(np.zeros((2, 3)), np.zeros((2, 3)))
     with pytest.raises(ValueError):
         Oracle([1.0, 1.0], 1.0, 10.0, 0.0).accel(np.zeros((3, 3)), np.zeros((3, 3)))
+
+
+# ------------------------------------------------------------------ NEXT rows: the Cross terms, Eqs. 2.3 and 2.6
+def _eih_residuals_terms(lam, c, kind, terms):
+    mass, pos, vel = _eih_system(lam)
+    o = Oracle(mass, 1.0, c, 0.0, kind=kind, terms=terms)
+    a = o.accel(pos, vel)
+    a_eih = np.array([[float(t) for t in row] for row in eih.eih_acc(list(mass), _to_list(pos), _to_list(vel), 1.0, c)])
+    d = np.abs(a - a_eih)
+    return d[0].max(), d[1:].max()
+
+
+@pytest.mark.parametrize("kind", KINDS)
+def test_cross_terms_vs_full_eih_residual_scaling(kind):
+    """With [a_i]_Cross (Eq. 2.6) the star equations agree with the full EIH theory to O(lam^2) and with [a_1]_Cross
+    (Eq. 2.3) the massive object's to O(lam^3): the truncation orders the paper states.  Every term of
+    Eq. 2.6 is O(lam) and every term of Eq. 2.3 O(lam^2), so a wrong coefficient, sign or index in any of them leaves a
+    residual one order lower and breaks the ratios below."""
+    from oracle.pn_oracle import CROSS_BH, CROSS_STAR
+
+    c = 10.0
+    lams = (1e-1, 1e-2, 1e-3)
+    both = {lam: _eih_residuals_terms(lam, c, kind, CROSS_STAR | CROSS_BH) for lam in lams}
+    star_only = {lam: _eih_residuals_terms(lam, c, kind, CROSS_STAR) for lam in lams}
+    for hi, lo in ((1e-1, 1e-2), (1e-2, 1e-3)):
+        assert both[hi][1] / both[lo][1] == pytest.approx(100.0, rel=0.15)       # a_i residual ~ lam^2
+        assert both[hi][0] / both[lo][0] == pytest.approx(1000.0, rel=0.15)      # a_1 residual ~ lam^3
+        assert star_only[hi][0] / star_only[lo][0] == pytest.approx(100.0, rel=0.15)  # without Eq. 2.3: still lam^2
+    # the star equations do not depend on which a_1 equation is used
+    assert star_only[1e-2][1] == pytest.approx(both[1e-2][1], rel=1e-9)
+    # sizes seen when the reading was fixed: 0.18 lam^2 and 4.2e-4 lam^3 at c = 10
+    assert both[1e-2][1] == pytest.approx(0.1767e-4, rel=0.02) and both[1e-2][0] == pytest.approx(4.232e-10, rel=0.02)
+    # and both are 1PN terms: residuals scale with 1/c^2
+    b100 = _eih_residuals_terms(1e-2, 100.0, kind, CROSS_STAR | CROSS_BH)
+    assert both[1e-2][1] / b100[1] == pytest.approx(100.0, rel=0.05)
+
+
+def test_cross_terms_vanish_in_the_newtonian_limit_and_for_massless_stars():
+    from oracle.pn_oracle import CROSS_BH, CROSS_STAR
+
+    p = inputs.random_small(12, seed=3, M=1.0, m_scale=1e-2, c=10.0, softening=1e-2, bh_moving=True)
+    hot = Oracle(p.mass, p.G, math.inf, p.softening).accel(p.pos, p.vel)
+    full = Oracle(p.mass, p.G, math.inf, p.softening, terms=CROSS_STAR | CROSS_BH).accel(p.pos, p.vel)
+    assert np.array_equal(hot, full)  # c = inf: every Cross term carries 1/c^2
+    m0 = p.mass.copy()
+    m0[1:] = 0.0  # massless tracers: every Cross term carries a star mass
+    hot = Oracle(m0, p.G, p.c, p.softening).accel(p.pos, p.vel)
+    full = Oracle(m0, p.G, p.c, p.softening, terms=CROSS_STAR | CROSS_BH).accel(p.pos, p.vel)
+    assert np.array_equal(hot, full)
+
+
+def test_cross_terms_two_body_finite_mass_periastron_advance():
+    """Two bodies, m/M = 0.01, zero-momentum frame, relative orbit a = 1, e = 0.5: the 1PN advance per orbit is
+    6 pi G (M + m) / (c^2 a (1 - e^2)) (total mass).  The hot path misses the O(m/M) part (ratio 0.971); with the
+    self terms of Eqs. 2.3 and 2.6 (first lines) the ratio is 0.999."""
+    from oracle.pn_oracle import CROSS_BH, CROSS_STAR
+
+    a, e, c, M, m = 1.0, 0.5, 100.0, 1.0, 1e-2
+    mu = M + m
+    rp, vp = a * (1 - e), math.sqrt(mu * (1 + e) / (a * (1 - e)))
+    mass = np.array([M, m])
+    pos = np.array([[-rp * m / mu, 0, 0], [rp * M / mu, 0, 0]])
+    vel = np.array([[0, -vp * m / mu, 0], [0, vp * M / mu, 0]])
+    period = 2 * math.pi * math.sqrt(a**3 / mu)
+    expected = 6 * math.pi * mu / (c * c * a * (1 - e * e))
+    got = {t: _periastron_angle_after_one_orbit(Oracle(mass, 1.0, c, 0.0, terms=t), pos, vel, period) / expected
+           for t in (0, CROSS_STAR | CROSS_BH)}
+    assert got[CROSS_STAR | CROSS_BH] == pytest.approx(1.0, abs=2.5e-3)
+    assert got[0] == pytest.approx(0.9714, abs=2e-3)
