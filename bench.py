@@ -33,8 +33,9 @@ if str(ROOT) not in sys.path:
 #   2 symmetric: 3 DADD + 12 DFMA + 5 DMUL = 20 per UNORDERED pair (+1 MUFU.RSQ64H) = 10 per ordered pair
 #   4 symmetric, equal-mass form (every star has the same mass, as in every BASELINE.json config): the two mass
 #     multiplications go: 3 DADD + 12 DFMA + 3 DMUL = 18 per unordered pair = 9 per ordered pair
+#   5 ordered pairs with the Cross terms of Eq. 2.6 (--cross): 36 DADD + 124 DFMA + 56 DMUL per 4 pairs = 54 per ordered pair
 PAIR_KERNELS = {0: ("pair_fp64_kernel", 15, 24.0), 2: ("pair_sym_fp64_kernel", 10, 16.0),
-                4: ("pair_sym_fp64_kernel<EQM>", 9, 15.0)}
+                4: ("pair_sym_fp64_kernel<EQM>", 9, 15.0), 5: ("pair_cross_fp64_kernel", 54, 85.0)}
 SMS, FP64_LANES_PER_SM = 148, 64
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu --set full
 # captures (profiles/), keyed by (variant, N_s); null when no capture exists for the workload
@@ -198,10 +199,10 @@ def oracle_rows(p, budget_pairs=3.0e9):
     return rows, f"4 force evaluations per step on a seeded subset of {r} of {p.n_stars} i-rows, each against all j"
 
 
-def cpu_baseline(p, target_s=12.0, max_steps=200) -> dict:
+def cpu_baseline(p, target_s=12.0, max_steps=200, terms=0) -> dict:
     from oracle.pn_oracle import Oracle
 
-    o = Oracle(p.mass, p.G, p.c, p.softening, kind="fast")
+    o = Oracle(p.mass, p.G, p.c, p.softening, kind="fast", terms=terms)
     rows, what = oracle_rows(p)
     pairs, t0, n = 0, time.perf_counter(), 0
     while n < max_steps and (time.perf_counter() - t0 < target_s or n == 0):
@@ -221,7 +222,7 @@ def run_reference(args) -> None:
     from oracle.pn_oracle import Oracle
 
     p = make_problem(args.workload)
-    o = Oracle(p.mass, p.G, p.c, p.softening, kind="fast")
+    o = Oracle(p.mass, p.G, p.c, p.softening, kind="fast", terms=1 if args.cross else 0)
     # bound the whole run to ~4e10 pair visits (about 1.5 min on 8 cores) whatever K is
     rows, what = oracle_rows(p, budget_pairs=max(2.0e8, 4.0e10 / max(1, args.steps)))
     for _ in range(args.warmup):
@@ -266,6 +267,7 @@ def workload_config(p, args) -> dict:
     return {"workload": p.name, "N": p.N, "n_stars": p.n_stars, "pairs_per_force_eval": p.pairs_per_eval,
             "force_evals_per_step": 4, "dt": p.dt, "c": p.c, "softening": p.softening, "M": float(p.mass[0]),
             "integrator": "classical RK4", "energy_evals_in_timed_region": 2,
+            "force": "hot path + [a_i]_Cross (Eq. 2.6)" if getattr(args, "cross", False) else "hot path (north_star)",
             "l2": "flushed (256 MiB write) between timed steps, outside the per-step event pairs",
             "parallelism": f"replicas x{args.gpus}" if args.gpus > 1 else "single GPU"}
 
@@ -297,6 +299,8 @@ def run_ours(args) -> None:
     K, W = args.steps, max(3, args.warmup)
     stream = torch.cuda.current_stream()
     pn = PN(p.mass, p.G, p.c, p.softening, stream=stream)
+    if args.cross:
+        pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, binding.PN_CROSS_STAR)
     cfg = pn.pn_get_pair_config()
     pos_d, vel_d = torch.from_numpy(p.pos).cuda(), torch.from_numpy(p.vel).cuda()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
@@ -399,7 +403,7 @@ def run_ours(args) -> None:
             "peak_measured_dfma": dfma_peak,
             "frac_of_measured_dfma": (achieved / dfma_peak) if achieved and dfma_peak else None,
         }
-        base = cpu_baseline(p) if not args.no_cpu_baseline else None
+        base = cpu_baseline(p, terms=1 if args.cross else 0) if not args.no_cpu_baseline else None
         line = {
             "metric": "fp64 pair-interactions/s", "value": value, "unit": "pair-interactions/s", "n_gpus": world,
             "steps": K, "warmup": W, "ms_per_step": ms_total_m / K, "higher_is_better": True, "scaling": "weak",
@@ -442,8 +446,11 @@ def run_sweep(args) -> None:
         pos, vel = torch.from_numpy(p.pos).cuda(), torch.from_numpy(p.vel).cuda()
         acc = torch.empty_like(pos)
         pn.pn_set_option(binding.PN_OPT_TIME_PAIR, 1)
-        for prec, pname, peak in ((binding.PN_FP64, "fp64", peak64), (binding.PN_FP32_PAIR, "fp32pair", peak32)):
+        # third leg: the first NEXT row of the scope table, [a_i]_Cross (Eq. 2.6) fused into an fp64 ordered-pair kernel
+        for prec, pname, peak, cross in ((binding.PN_FP64, "fp64", peak64, 0), (binding.PN_FP32_PAIR, "fp32pair", peak32, 0),
+                                         (binding.PN_FP64, "fp64+cross", peak64, binding.PN_CROSS_STAR)):
             pn.pn_set_option(binding.PN_OPT_PAIR_PRECISION, prec)
+            pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, cross)
             instr = pn.pn_get_pair_config()["fp64_instr_per_pair"]  # pipe instructions per ordered pair of the kernel in use
             reps = 5 if p.n_stars < 200000 else 2
             for _ in range(2):
@@ -479,6 +486,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cross", action="store_true", help="add [a_i]_Cross, Eq. 2.6 (NEXT-1 of the scope table) to the force")
     args = ap.parse_args()
     if args.sweep:
         run_sweep(args)

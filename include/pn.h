@@ -55,6 +55,14 @@ extern "C" {
                                    kernel accumulates rho^-3 d on both sides and applies the common G m once per partial sum
                                    (9 instead of 10 FP64 instructions per ordered pair); 0: always the general-mass form */
 
+#define PN_OPT_CROSS_TERMS 7    /* 0 (default): the hot path of north_star; PN_CROSS_STAR: add [a_i]_Cross, Eq. 2.6
+                                   (PAPER.md:70-86), to every star's acceleration -- the first NEXT row of the scope table:
+                                   its O(N^2) sums are fused into an fp64 ordered-pair kernel that also produces the
+                                   Newtonian star-star term (54 FP64 instructions per ordered pair), its O(N) parts go into
+                                   the epilogue.  Applies to pn_accel and pn_step; pn_energy is Eq. 2.7 either way.
+                                   [a_1]_Cross (Eq. 2.3) is not built: the massive object keeps Eqs. 2.1 + 2.2. */
+#define PN_CROSS_STAR 1
+
 /* PN_OPT_PAIR_PRECISION values */
 #define PN_FP64 0      /* fp64 pair arithmetic and accumulation (parity 1e-12) */
 #define PN_FP32_PAIR 1 /* fp32 pair arithmetic on two-float positions, fp64 accumulation (parity 1e-5) */
@@ -104,7 +112,8 @@ int pn_get_pair_config(pn_ctx* ctx, int32_t* cfg_host); /* 8 ints: threads/block
                                                            slots (j-splits / groups), grid blocks, padded N_s, pipe
                                                            instructions per ordered pair, variant (0 fp64 tiled,
                                                            1 fp32 tiled, 2 fp64 symmetric, 3 fp32 symmetric,
-                                                           4 fp64 symmetric, equal-mass form) */
+                                                           4 fp64 symmetric, equal-mass form,
+                                                           5 fp64 ordered pairs with the Cross terms of Eq. 2.6) */
 
 int pn_measure_fp64_peak(pn_ctx* ctx, double* tflops_host); /* sustained FP64 FMA rate of this device from a register-only
                                                               DFMA-chain kernel (2 flops per FMA), best of 3: the measured

@@ -20,6 +20,8 @@ constexpr int kNT = 128;        // threads per block of the pair / energy / epil
 constexpr int kTJ = 128;        // j records per shared-memory tile
 constexpr int kGraphBatch = 16; // RK4 steps captured in the batched graph
 constexpr int kSMs = 148;       // B200
+constexpr int kCrossI = 2;      // i-stars per thread of pair_cross_fp64_kernel
+constexpr int kCrossTJ = 64;    // its j tile (96 B records)
 
 thread_local std::string g_create_error;
 
@@ -35,6 +37,10 @@ struct pn_ctx {
 
     // options
     int precision = PN_FP64, use_graph = 1, time_pair = 0, j_split_opt = 0, kernel_opt = PN_PAIR_AUTO, eqm_opt = 1;
+    int cross = 0;            // PN_OPT_CROSS_TERMS mask
+    CRec* crec = nullptr;     // cross mode: per-star records, block partials and totals of the O(N) sums, 6-component partials
+    double *cblk = nullptr, *csum = nullptr, *part6 = nullptr;
+    int c_split = 1, c_tiles_per_split = 0;
     bool equal_mass = false;  // every star has the same mass > 0
     double gm_eq = 0;
 
@@ -143,7 +149,10 @@ bool use_sym(const pn_ctx* c)
 
 bool use_eqm(const pn_ctx* c) { return c->equal_mass && c->eqm_opt && c->precision == PN_FP64 && use_sym(c); }
 
-int active_split(const pn_ctx* c) { return use_sym(c) ? c->sym_G : c->n_split; }
+// kernels of the pair stage of one force evaluation (the epilogue is counted by the callers)
+int kernels_per_eval(const pn_ctx* c) { return c->cross ? 3 : (c->precision == PN_FP32_PAIR ? 2 : 1); }
+
+int active_split(const pn_ctx* c) { return c->cross ? c->c_split : (use_sym(c) ? c->sym_G : c->n_split); }
 
 void destroy_graphs(pn_ctx* c)
 {
@@ -215,7 +224,14 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
         PN_CUDA(c, cudaEventRecord(c->ev[c->ev_used], st));
     }
     const bool mask = (c->eps2 == 0.0);
-    if (c->precision == PN_FP32_PAIR) {
+    if (c->cross) {  // NEXT-1: star-star Newtonian + pair part of [a_i]_Cross in one ordered-pair pass (fp64)
+        const int nb = c->np / kNT;
+        cross_prep_kernel<kNT><<<nb, kNT, 0, st>>>(c->jrec[set], c->v[set], c->bh[set], c->crec, c->cblk, c->n_stars, c->np);
+        cross_sum_kernel<<<1, 256, 0, st>>>(c->cblk, nb, c->csum);
+        dim3 grid(c->np / (kCrossI * kNT), c->c_split);
+        pair_cross_fp64_kernel<kCrossI, 2, kNT, kCrossTJ><<<grid, kNT, 0, st>>>(c->crec, c->bh[set], c->part6, c->np,
+                                                                               c->c_tiles_per_split, c->eps2, c->GM);
+    } else if (c->precision == PN_FP32_PAIR) {
         split_kernel<<<(c->np + 255) / 256, 256, 0, st>>>(c->jrec[set], c->frec, c->n_stars, c->np);
         PN_CUDA(c, cudaGetLastError());
         dim3 grid(c->n_itiles, c->n_split);
@@ -257,7 +273,8 @@ EpiArgs epi_args(pn_ctx* c, int set, double* acc_out)
     EpiArgs a;
     a.jrec = c->jrec[set];
     a.v = c->v[set];
-    a.part = c->part;
+    a.part = c->cross ? c->part6 : c->part;
+    a.csum = c->csum;
     a.x0 = c->x0, a.v0 = c->v0, a.sx = c->sx, a.sv = c->sv;
     a.bh = c->bh[set];
     a.bh_part = c->bh_part;
@@ -277,7 +294,10 @@ int enqueue_rk4_step(pn_ctx* c, cudaStream_t st, bool timed)
     for (int stage = 0; stage < 4; ++stage) {
         int rc = launch_pair(c, 0, st, timed);
         if (rc) return rc;
-        epilogue_kernel<MODE_RK4, kNT><<<grid, kNT, 0, st>>>(a, stage);
+        if (c->cross)
+            epilogue_kernel<MODE_RK4, kNT, true><<<grid, kNT, 0, st>>>(a, stage);
+        else
+            epilogue_kernel<MODE_RK4, kNT, false><<<grid, kNT, 0, st>>>(a, stage);
         PN_CUDA(c, cudaGetLastError());
     }
     return PN_OK;
@@ -350,7 +370,7 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     // i per thread: larger i-tiles amortise the shared-memory broadcast; small N needs more blocks instead
     ctx->ipt = ctx->n_stars >= 3072 ? 2 : 1;
     choose_sym(ctx);
-    const int ti = std::max(ctx->ipt * kNT, ctx->sym_U);  // both are powers of two: np suits every pair kernel
+    const int ti = std::max(std::max(ctx->ipt * kNT, ctx->sym_U), kCrossI * kNT);  // powers of two: np suits every pair kernel
     ctx->np = (ctx->n_stars + ti - 1) / ti * ti;
     choose_sym_groups(ctx);
     ctx->n_itiles = ctx->np / (ctx->ipt * kNT);
@@ -435,6 +455,7 @@ int pn_destroy(pn_ctx* c)
     cudaFree(c->x0), cudaFree(c->v0), cudaFree(c->sx), cudaFree(c->sv);
     cudaFree(c->part), cudaFree(c->bh_part), cudaFree(c->ticket), cudaFree(c->prm);
     cudaFree(c->io_pos), cudaFree(c->io_vel), cudaFree(c->io_acc);
+    cudaFree(c->crec), cudaFree(c->cblk), cudaFree(c->csum), cudaFree(c->part6);
     cudaFree(c->frec), cudaFree(c->erec), cudaFree(c->blk_prep), cudaFree(c->blk_pair), cudaFree(c->d_energy);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     cudaGetLastError();
@@ -470,6 +491,24 @@ int pn_set_option(pn_ctx* c, int key, int value)
                 return fail(c, PN_EINVAL, "pn_set_option: unknown pair kernel %d", value);
             c->kernel_opt = value;
             return PN_OK;
+        case PN_OPT_CROSS_TERMS: {
+            if (value != 0 && value != PN_CROSS_STAR)
+                return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_CROSS_TERMS takes 0 or PN_CROSS_STAR ([a_1]_Cross, Eq. 2.3, is not built)");
+            if (value && !c->crec) {  // buffers of the cross path, on first use
+                const size_t np = c->np;
+                const int n_it = c->np / (kCrossI * kNT), n_t = c->np / kCrossTJ;
+                int s = std::max(1, std::min(std::min((kSMs * 16 + n_it - 1) / n_it, n_t), 64));
+                c->c_tiles_per_split = (n_t + s - 1) / s;
+                c->c_split = (n_t + c->c_tiles_per_split - 1) / c->c_tiles_per_split;
+                PN_CUDA(c, dalloc(&c->crec, np));
+                PN_CUDA(c, dalloc(&c->cblk, (np / kNT) * kCrossSums));
+                PN_CUDA(c, dalloc(&c->csum, kCrossSums));
+                PN_CUDA(c, dalloc(&c->part6, (size_t)c->c_split * 6 * np));
+            }
+            c->cross = value;
+            destroy_graphs(c);
+            return PN_OK;
+        }
         case PN_OPT_EQUAL_MASS:
             if (value != 0 && value != 1) return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_EQUAL_MASS takes 0 or 1");
             c->eqm_opt = value;
@@ -541,9 +580,12 @@ int pn_accel(pn_ctx* c, const double* pos, const double* vel, double* acc)
     PN_CUDA(c, cudaGetLastError());
     if (int rc = launch_pair(c, 1, c->stream, c->time_pair != 0)) return rc;
     const EpiArgs a = epi_args(c, 1, acc);
-    epilogue_kernel<MODE_ACCEL, kNT><<<c->np / kEpiStars, kNT, 0, c->stream>>>(a, 0);
+    if (c->cross)
+        epilogue_kernel<MODE_ACCEL, kNT, true><<<c->np / kEpiStars, kNT, 0, c->stream>>>(a, 0);
+    else
+        epilogue_kernel<MODE_ACCEL, kNT, false><<<c->np / kEpiStars, kNT, 0, c->stream>>>(a, 0);
     PN_CUDA(c, cudaGetLastError());
-    c->n_launch += (c->precision == PN_FP32_PAIR ? 4 : 3);
+    c->n_launch += 2 + kernels_per_eval(c);
     return PN_OK;
 }
 
@@ -578,7 +620,7 @@ int pn_step(pn_ctx* c, double dt, int64_t nsteps)
     if (eager) {
         for (int64_t s = 0; s < nsteps; ++s)
             if (int rc = enqueue_rk4_step(c, c->stream, c->time_pair != 0)) return rc;
-        c->n_launch += (c->precision == PN_FP32_PAIR ? 12 : 8) * nsteps;
+        c->n_launch += 4 * (1 + kernels_per_eval(c)) * nsteps;
         return PN_OK;
     }
     if (c->graph_split != c->n_split || c->graph_precision != c->precision || c->graph_sym != (int)use_sym(c) ||
@@ -597,7 +639,7 @@ int pn_step(pn_ctx* c, double dt, int64_t nsteps)
             if (int rc = build_graph(c, 1, &c->graph1)) return rc;
         for (; left > 0; --left) PN_CUDA(c, cudaGraphLaunch(c->graph1, c->stream));
     }
-    c->n_launch += (c->precision == PN_FP32_PAIR ? 12 : 8) * nsteps;
+    c->n_launch += 4 * (1 + kernels_per_eval(c)) * nsteps;
     return PN_OK;
 }
 
@@ -680,6 +722,11 @@ int pn_get_pair_config(pn_ctx* c, int32_t* cfg)
 {
     if (int rc = check_ctx(c)) return rc;
     if (!cfg) return fail(c, PN_EINVAL, "pn_get_pair_config: null pointer");
+    if (c->cross) {
+        cfg[0] = kNT, cfg[1] = kCrossI, cfg[2] = kCrossTJ, cfg[3] = c->c_split;
+        cfg[4] = (c->np / (kCrossI * kNT)) * c->c_split, cfg[5] = c->np, cfg[6] = 54, cfg[7] = 5;
+        return PN_OK;
+    }
     if (use_sym(c)) {
         cfg[0] = 32 * c->sym_W, cfg[1] = c->sym_I, cfg[2] = c->sym_U, cfg[3] = c->sym_G;
         cfg[4] = c->sym_G * (c->sym_G + 1) / 2, cfg[5] = c->np;

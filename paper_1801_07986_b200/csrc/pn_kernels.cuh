@@ -415,6 +415,176 @@ __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp64_kernel(const JRec*
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// NEXT-1 of the scope table: [a_i]_Cross, Eq. 2.6, fused into the star-star pair loop
+// (PN_OPT_CROSS_TERMS).  With x_ab = x_a - x_b, v_ij = v_i - v_j, every star-star r_ij -> rho_ij (reading R9):
+//   L0  5 G^2 m_i M x_i1 / r_i1^4 - (G m_i / r_i1^3) [ 4 v_i^2 x_i1 - 7 (v_i.x_i1) v_i ]
+//   L1  sum_j G^2 m_j M x_i1 / r_i1^3 ( 4/rho_ij + 5/(4 r_j1) + r_i1^2/(4 r_j1^3) - rho_ij^2/(4 r_j1^3) )
+//   L2  sum_j G^2 m_j M x_ij / rho_ij^3 ( 4/r_i1 + 5/(4 r_j1) - r_i1^2/(4 r_j1^3) + rho_ij^2/(4 r_j1^3) )
+//   L3  -(7/2) sum_j G^2 m_j M x_j1 / r_j1^3 ( 1/rho_ij - 1/r_i1 )
+//   L4  - sum_j (G m_j / r_i1^3) [ 4 (v_i.v_j) x_i1 - 3 (v_j.x_i1) v_i - 4 (v_i.x_i1) v_j ]
+//   L5  + sum_j (G m_j x_ij / rho_ij^3) [ v_i^2 - 2 |v_ij|^2 + (3/2)(v_j.x_ij)^2 / rho_ij^2 ]
+//   L6  + sum_j (G m_j / rho_ij^3) [ x_ij.(4 v_i - 3 v_j) ] v_ij
+// Regrouping (the oracle evaluates the lines as printed).  Everything in which the pair distance does not appear is a
+// sum over all j != i of a per-j quantity, i.e. a global sum minus star i's own term: with
+//   P = sum_j G m_j v_j,  Q1 = sum_j G m_j / r_j1,  Q3 = sum_j G m_j / r_j1^3,  W = sum_j G m_j x_j1 / r_j1^3
+// (cross_prep_kernel + cross_sum_kernel, O(N)) L4 and parts of L1 and L3 are O(N) work in the epilogue.  What is left for
+// the O(N^2) loop, per ordered pair with d = x_ij, y = 1/rho_ij, s = G m_j y^3:
+//   a^SS -= s d                                                           (the Newtonian term of Eq. 2.4, 3 DFMA extra)
+//   A    += s g d,  g = GM f2 + v_i^2 - 2 |v_ij|^2 + (3/2)(v_j.d)^2 y^2,   f2 = 4/r_i1 + 5/(4 r_j1) + (rho^2 - r_i1^2)/(4 r_j1^3)
+//   S    += G m_j (4 y - rho^2 / (4 r_j1^3))           (L1: coefficient of GM x_i1 / r_i1^3)
+//   Y    += y (G m_j x_j1 / r_j1^3)                    (L3: times -(7/2) GM)
+//   H    += h,  V += h v_j,   h = s (4 v_i.d - 3 v_j.d) (L6 = H v_i - V)
+// = 54 FP64-pipe instructions + 1 MUFU.RSQ64H per ordered pair.  Tiled form (ordered pairs, j tiles of 96 B records
+// through double-buffered shared memory, I i-stars per thread); output part[S][6][np]: a^SS and the pair part of the
+// Cross term per j-chunk, reduced in fixed order by the epilogue.
+// ---------------------------------------------------------------------------------------------------------
+struct __align__(16) CRec {
+    double x, y, z, gm;      // position, G m_j
+    double vx, vy, vz, a5;   // velocity, 5 / (4 r_j1)
+    double b, wx, wy, wz;    // 1 / (4 r_j1^3),  G m_j x_j1 / r_j1^3
+};
+static_assert(sizeof(CRec) == 96, "CRec must be 96 bytes");
+
+constexpr int kCrossSums = 8;  // P (3), Q1, Q3, W (3)
+
+template <int NT>
+__global__ void __launch_bounds__(NT) cross_prep_kernel(const JRec* __restrict__ jrec, const double* __restrict__ v,
+                                                        const BhState* __restrict__ bh, CRec* __restrict__ crec,
+                                                        double* __restrict__ blk /* [grid][8] */, int n_stars, int np)
+{
+    __shared__ double red[kCrossSums][NT / 32];
+    const int i = blockIdx.x * NT + threadIdx.x;
+    double sums[kCrossSums] = {0, 0, 0, 0, 0, 0, 0, 0};
+    if (i < np) {
+        const JRec r = jrec[i];
+        CRec o;
+        o.x = r.x, o.y = r.y, o.z = r.z, o.gm = r.gm;
+        o.vx = o.vy = o.vz = o.a5 = o.b = o.wx = o.wy = o.wz = 0.0;
+        if (i < n_stars) {
+            const double d[3] = {r.x - bh->xs[0], r.y - bh->xs[1], r.z - bh->xs[2]};  // x_j1
+            const double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+            const double inv_r = 1.0 / sqrt(r2);
+            const double inv_r3 = inv_r * inv_r * inv_r;
+            o.vx = v[i], o.vy = v[np + i], o.vz = v[2 * np + i];
+            o.a5 = 1.25 * inv_r, o.b = 0.25 * inv_r3;
+            o.wx = r.gm * d[0] * inv_r3, o.wy = r.gm * d[1] * inv_r3, o.wz = r.gm * d[2] * inv_r3;
+            sums[0] = r.gm * o.vx, sums[1] = r.gm * o.vy, sums[2] = r.gm * o.vz;
+            sums[3] = r.gm * inv_r, sums[4] = r.gm * inv_r3;
+            sums[5] = o.wx, sums[6] = o.wy, sums[7] = o.wz;
+        }
+        crec[i] = o;
+    }
+#pragma unroll
+    for (int q = 0; q < kCrossSums; ++q) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) sums[q] += __shfl_down_sync(0xffffffffu, sums[q], o);
+        if ((threadIdx.x & 31) == 0) red[q][threadIdx.x >> 5] = sums[q];
+    }
+    __syncthreads();
+    if (threadIdx.x < kCrossSums) {
+        double s = 0;
+        for (int w = 0; w < NT / 32; ++w) s += red[threadIdx.x][w];
+        blk[(size_t)blockIdx.x * kCrossSums + threadIdx.x] = s;
+    }
+}
+
+// fixed-order sum of the block partials: one warp per quantity
+__global__ void __launch_bounds__(256) cross_sum_kernel(const double* __restrict__ blk, int n_blk, double* __restrict__ out)
+{
+    const int q = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double s = 0;
+    for (int b = lane; b < n_blk; b += 32) s += blk[(size_t)b * kCrossSums + q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if (lane == 0) out[q] = s;
+}
+
+template <int I, int MINB, int NT, int TJ>
+__global__ void __launch_bounds__(NT, MINB) pair_cross_fp64_kernel(const CRec* __restrict__ crec, const BhState* __restrict__ bh,
+                                                                   double* __restrict__ part /* [S][6][np] */, int np,
+                                                                   int tiles_per_split, double eps2, double GM)
+{
+    __shared__ CRec sj[2][TJ];
+    const int tid = threadIdx.x;
+    double xi[I], yi[I], zi[I], vxi[I], vyi[I], vzi[I], ri2[I], ci[I], vi2[I];
+    double nx[I], ny[I], nz[I], ax[I], ay[I], az[I], S[I], Yx[I], Yy[I], Yz[I], H[I], Vx[I], Vy[I], Vz[I];
+    int ii[I];
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        ii[k] = blockIdx.x * (I * NT) + tid + k * NT;
+        const CRec c = crec[ii[k]];
+        xi[k] = c.x, yi[k] = c.y, zi[k] = c.z, vxi[k] = c.vx, vyi[k] = c.vy, vzi[k] = c.vz;
+        const double dx = c.x - bh->xs[0], dy = c.y - bh->xs[1], dz = c.z - bh->xs[2];
+        ri2[k] = dx * dx + dy * dy + dz * dz;
+        ci[k] = 4.0 / sqrt(ri2[k]);
+        vi2[k] = c.vx * c.vx + c.vy * c.vy + c.vz * c.vz;
+        nx[k] = ny[k] = nz[k] = ax[k] = ay[k] = az[k] = S[k] = Yx[k] = Yy[k] = Yz[k] = H[k] = Vx[k] = Vy[k] = Vz[k] = 0.0;
+    }
+    const int n_tiles = np / TJ;
+    const int t_begin = blockIdx.y * tiles_per_split;
+    const int t_end = min(n_tiles, t_begin + tiles_per_split);
+    constexpr int kVec = TJ * 6;  // double2 per tile
+    auto fill = [&](int buf, int t) {
+        const double2* src = reinterpret_cast<const double2*>(crec + (size_t)t * TJ);
+        double2* dst = reinterpret_cast<double2*>(sj[buf]);
+        for (int q = tid; q < kVec; q += NT) dst[q] = src[q];
+    };
+    if (t_begin < t_end) fill(0, t_begin);
+    __syncthreads();
+    for (int t = t_begin; t < t_end; ++t) {
+        const int buf = (t - t_begin) & 1;
+        if (t + 1 < t_end) fill(buf ^ 1, t + 1);
+        const CRec* tile = sj[buf];
+        const int j0 = t * TJ;
+#pragma unroll 2
+        for (int jj = 0; jj < TJ; ++jj) {
+            const CRec r = tile[jj];
+#pragma unroll
+            for (int k = 0; k < I; ++k) {
+                const bool self = (j0 + jj == ii[k]);  // j != i in every sum of Eq. 2.6 (eps > 0 does not cancel it here)
+                const double dx = xi[k] - r.x, dy = yi[k] - r.y, dz = zi[k] - r.z;  // x_ij
+                const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+                const double y0 = rsqrt_seed(r2);
+                const double e = fma(-r2, y0 * y0, 1.0);
+                double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1 / rho to full fp64 accuracy
+                y = self ? 0.0 : y;
+                const double gm = self ? 0.0 : r.gm;
+                const double y2 = y * y;
+                const double s = gm * (y2 * y);  // G m_j / rho^3
+                nx[k] = fma(-s, dx, nx[k]), ny[k] = fma(-s, dy, ny[k]), nz[k] = fma(-s, dz, nz[k]);
+                const double ux = vxi[k] - r.vx, uy = vyi[k] - r.vy, uz = vzi[k] - r.vz;  // v_ij
+                const double uu = fma(ux, ux, fma(uy, uy, uz * uz));
+                const double vjx = fma(r.vx, dx, fma(r.vy, dy, r.vz * dz));
+                const double vix = fma(vxi[k], dx, fma(vyi[k], dy, vzi[k] * dz));
+                const double f2 = fma(r2 - ri2[k], r.b, r.a5) + ci[k];
+                double g = fma(GM, f2, vi2[k]);
+                g = fma(-2.0, uu, g);
+                g = fma(1.5, (vjx * vjx) * y2, g);
+                const double sg = s * g;
+                ax[k] = fma(sg, dx, ax[k]), ay[k] = fma(sg, dy, ay[k]), az[k] = fma(sg, dz, az[k]);
+                S[k] = fma(gm, fma(-r2, r.b, 4.0 * y), S[k]);
+                Yx[k] = fma(y, r.wx, Yx[k]), Yy[k] = fma(y, r.wy, Yy[k]), Yz[k] = fma(y, r.wz, Yz[k]);
+                const double h = s * fma(4.0, vix, -3.0 * vjx);
+                H[k] += h;
+                Vx[k] = fma(h, r.vx, Vx[k]), Vy[k] = fma(h, r.vy, Vy[k]), Vz[k] = fma(h, r.vz, Vz[k]);
+            }
+        }
+        __syncthreads();
+    }
+    double* out = part + (size_t)blockIdx.y * 6 * np;
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        const double dx = xi[k] - bh->xs[0], dy = yi[k] - bh->xs[1], dz = zi[k] - bh->xs[2];  // x_i1
+        const double inv_r = 0.25 * ci[k];
+        const double c1 = GM * inv_r * inv_r * inv_r * S[k];  // L1 pair part: GM x_i1 / r_i1^3 * S
+        out[ii[k]] = nx[k], out[np + ii[k]] = ny[k], out[2 * np + ii[k]] = nz[k];
+        out[3 * np + ii[k]] = fma(c1, dx, ax[k]) - 3.5 * GM * Yx[k] + fma(H[k], vxi[k], -Vx[k]);
+        out[4 * np + ii[k]] = fma(c1, dy, ay[k]) - 3.5 * GM * Yy[k] + fma(H[k], vyi[k], -Vy[k]);
+        out[5 * np + ii[k]] = fma(c1, dz, az[k]) - 3.5 * GM * Yz[k] + fma(H[k], vzi[k], -Vz[k]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // S1 variant: fp32 pair arithmetic, fp64 accumulation (PN_FP32_PAIR, parity 1e-5).
 // Positions are split into two floats, hi = fl32(x), lo = fl32(x - hi), so that the pair separation
 //   d = (hi_j - hi_i) + (lo_j - lo_i)
@@ -712,19 +882,23 @@ struct EpiArgs {
     const StepParams* prm;
     int n_stars, np, n_split;
     double GM, inv_c2;
+    const double* csum;   // CROSS: P (3), Q1, Q3, W (3) of cross_sum_kernel
 };
 
 enum { MODE_ACCEL = 0, MODE_RK4 = 1 };
 
 constexpr int kEpiStars = 32;  // stars per epilogue block: lane = star, warp w sums the partial-sum slots w, w + NW, ...
 
-template <int MODE, int NT>
+// CROSS: the partial sums carry 6 components (a^SS and the pair part of [a_i]_Cross, Eq. 2.6); the O(N) parts of the
+// Cross term are added here (see pair_cross_fp64_kernel).
+template <int MODE, int NT, bool CROSS>
 __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
 {
     constexpr int NW = NT / 32;
+    constexpr int NC = CROSS ? 6 : 3;
     static_assert(NW == 4, "the fixed-order cross-warp sum below is written for 4 warps");
     __shared__ double red[3 * NW];
-    __shared__ double wsum[NW][3][kEpiStars];
+    __shared__ double wsum[NW][NC][kEpiStars];
     __shared__ bool is_last;
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int i = blockIdx.x * kEpiStars + lane;
@@ -732,32 +906,35 @@ __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
 
     // fixed-order reduction of the partial-sum slots.  Every load is a coalesced 256 B row of one (slot, component);
     // 4 slots x 3 components are in flight per thread, so the O(S N) read runs at L2/HBM bandwidth, not latency.
-    double ss[3] = {0, 0, 0};
+    double ss[NC];
+#pragma unroll
+    for (int k = 0; k < NC; ++k) ss[k] = 0.0;
     if (i < A.n_stars) {
-        const size_t stride = (size_t)NW * 3 * np;
-        const double* p = A.part + (size_t)w * 3 * np + i;
+        constexpr int UN = CROSS ? 2 : 4;  // slots in flight per thread (12 loads either way)
+        const size_t stride = (size_t)NW * NC * np;
+        const double* p = A.part + (size_t)w * NC * np + i;
         int s = w;
-        for (; s + 3 * NW < A.n_split; s += 4 * NW, p += 4 * stride) {
-            double q[4][3];
+        for (; s + (UN - 1) * NW < A.n_split; s += UN * NW, p += UN * stride) {
+            double q[UN][NC];
 #pragma unroll
-            for (int u = 0; u < 4; ++u)
+            for (int u = 0; u < UN; ++u)
 #pragma unroll
-                for (int k = 0; k < 3; ++k) q[u][k] = __ldcg(p + u * stride + (size_t)k * np);
+                for (int k = 0; k < NC; ++k) q[u][k] = __ldcg(p + u * stride + (size_t)k * np);
 #pragma unroll
-            for (int u = 0; u < 4; ++u)
+            for (int u = 0; u < UN; ++u)
 #pragma unroll
-                for (int k = 0; k < 3; ++k) ss[k] += q[u][k];
+                for (int k = 0; k < NC; ++k) ss[k] += q[u][k];
         }
         for (; s < A.n_split; s += NW, p += stride)
 #pragma unroll
-            for (int k = 0; k < 3; ++k) ss[k] += __ldcg(p + (size_t)k * np);
+            for (int k = 0; k < NC; ++k) ss[k] += __ldcg(p + (size_t)k * np);
     }
 #pragma unroll
-    for (int k = 0; k < 3; ++k) wsum[w][k][lane] = ss[k];
+    for (int k = 0; k < NC; ++k) wsum[w][k][lane] = ss[k];
     __syncthreads();
     if (w == 0) {
 #pragma unroll
-        for (int k = 0; k < 3; ++k) ss[k] = ((wsum[0][k][lane] + wsum[1][k][lane]) + wsum[2][k][lane]) + wsum[3][k][lane];
+        for (int k = 0; k < NC; ++k) ss[k] = ((wsum[0][k][lane] + wsum[1][k][lane]) + wsum[2][k][lane]) + wsum[3][k][lane];
     }
     const bool live = (w == 0) && (i < A.n_stars);
 
@@ -784,6 +961,23 @@ __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
         const double gv = -A.inv_c2 * 3.0 * vx;
 #pragma unroll
         for (int k = 0; k < 3; ++k) a[k] = ss[k] + cs * (fx * x[k] + fv * vel[k]);
+        if (CROSS) {
+            // [a_i]_Cross = L0 + the O(N) parts of L1, L3, L4 (global sums minus this star's own term) + pair part
+            const double P[3] = {A.csum[0] - rec.gm * vel[0], A.csum[1] - rec.gm * vel[1], A.csum[2] - rec.gm * vel[2]};
+            const double Q1 = A.csum[3] - rec.gm * inv_r, Q3 = A.csum[4] - rec.gm * inv_r3;
+            const double W[3] = {A.csum[5] - rec.gm * x[0] * inv_r3, A.csum[6] - rec.gm * x[1] * inv_r3,
+                                 A.csum[7] - rec.gm * x[2] * inv_r3};
+            const double vP = vel[0] * P[0] + vel[1] * P[1] + vel[2] * P[2];
+            const double xP = x[0] * P[0] + x[1] * P[1] + x[2] * P[2];
+            // coefficient of x_i1: L0 (5 G m_i GM / r^4 - 4 G m_i v^2 / r^3) + L1 (GM/r^3)(5/4 Q1 + r^2/4 Q3) - L4 4 (v.P)/r^3
+            const double kx = inv_r3 * (5.0 * rec.gm * GMr - 4.0 * rec.gm * v2 + A.GM * (1.25 * Q1 + 0.25 * r2 * Q3) - 4.0 * vP);
+            // coefficient of v_i: L0 7 G m_i (v.x)/r^3 + L4 3 (P.x)/r^3
+            const double kv = inv_r3 * (7.0 * rec.gm * vx + 3.0 * xP);
+            const double kp = 4.0 * vx * inv_r3;       // L4: + 4 (v_i.x_i1) P / r^3
+            const double kw = 3.5 * A.GM * inv_r;      // L3: + (7/2) GM W / r_i1
+#pragma unroll
+            for (int k = 0; k < 3; ++k) a[k] += A.inv_c2 * (ss[3 + k] + kx * x[k] + kv * vel[k] + kp * P[k] + kw * W[k]);
+        }
         b0 = cb * (gx * x[0] + gv * vel[0]);
         b1 = cb * (gx * x[1] + gv * vel[1]);
         b2 = cb * (gx * x[2] + gv * vel[2]);

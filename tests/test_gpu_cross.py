@@ -1,0 +1,96 @@
+"""GPU parity of the first NEXT row of the scope table: [a_i]_Cross, Eq. 2.6, switched on with
+PN_OPT_CROSS_TERMS = PN_CROSS_STAR, against the oracle's literal evaluation (terms = CROSS_STAR).  Same tolerance as the
+hot path: err_i = max_k |a_ik - ref_ik| / ||ref_i||_2 <= 1e-12."""
+import numpy as np
+import pytest
+
+from oracle.pn_oracle import CROSS_STAR, Oracle
+from paper_1801_07986_b200 import inputs
+from tests.conftest import rel_err_rows
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL_ACC = 1e-12
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _pn_cross(p):
+    from paper_1801_07986_b200 import PN, binding
+
+    pn = PN(p.mass, p.G, p.c, p.softening)
+    pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, binding.PN_CROSS_STAR)
+    return pn
+
+
+@pytest.mark.parametrize("n_stars", [1, 2, 3, 129, 1023, 4099, 13001])
+def test_cross_accel_parity_sizes(n_stars):
+    if n_stars <= 3:
+        p = inputs.random_small(n_stars, seed=700 + n_stars, M=1.0, m_scale=1e-2, c=10.0, softening=1e-3, bh_moving=True)
+    else:
+        p = inputs.plummer_bh(n_stars, seed=700 + n_stars, c=20.0)  # a small c makes the 1PN terms 25 x larger than at c = 100
+    ref = Oracle(p.mass, p.G, p.c, p.softening, terms=CROSS_STAR).accel(p.pos, p.vel)
+    hot = Oracle(p.mass, p.G, p.c, p.softening).accel(p.pos, p.vel)
+    with _pn_cross(p) as pn:
+        assert pn.pn_get_pair_config()["variant"] == 5
+        acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
+    assert rel_err_rows(acc, ref).max() <= TOL_ACC
+    if n_stars >= 2:  # the Cross term is really there (with one star only the O(m_i) self line is left)
+        assert rel_err_rows(hot[1:], ref[1:]).max() > 1e-9
+    assert np.array_equal(ref[0], hot[0])  # the massive object keeps Eqs. 2.1 + 2.2
+
+
+@pytest.mark.parametrize("gen", ["cusp", "unequal_eps0", "tracers"])
+def test_cross_accel_parity_other_inputs(gen):
+    if gen == "cusp":
+        p = inputs.cusp_bh(3000, seed=5)
+    elif gen == "unequal_eps0":
+        p = inputs.random_small(500, seed=8, M=1.0, m_scale=1e-3, c=10.0, softening=0.0, bh_moving=True)
+    else:
+        p = inputs.plummer_bh(700, seed=9, c=30.0)
+        p.mass[10:200] = 0.0
+    ref = Oracle(p.mass, p.G, p.c, p.softening, terms=CROSS_STAR).accel(p.pos, p.vel)
+    with _pn_cross(p) as pn:
+        acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
+    assert np.isfinite(acc).all()
+    assert rel_err_rows(acc, ref).max() <= TOL_ACC
+
+
+def test_cross_switch_off_restores_the_hot_path_bitwise_and_is_deterministic():
+    from paper_1801_07986_b200 import PN, binding
+
+    p = inputs.plummer_bh(4099, seed=11, c=20.0)
+    with PN(p.mass, p.G, p.c, p.softening) as pn:
+        pos, vel = _dev(p.pos), _dev(p.vel)
+        a0 = pn.pn_accel(pos, vel).cpu().numpy()
+        pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, binding.PN_CROSS_STAR)
+        c1 = pn.pn_accel(pos, vel).cpu().numpy()
+        c2 = pn.pn_accel(pos, vel).cpu().numpy()
+        pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, 0)
+        a1 = pn.pn_accel(pos, vel).cpu().numpy()
+        with pytest.raises(binding.PNError):
+            pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, 2)  # [a_1]_Cross is not built
+    assert np.array_equal(a0, a1) and np.array_equal(c1, c2) and not np.array_equal(a0, c1)
+
+
+def test_cross_rk4_trajectory_tracks_oracle():
+    """pn_step with the Cross terms (graph and plain launches) against the oracle's RK4 with the same terms."""
+    from paper_1801_07986_b200 import binding
+
+    p = inputs.plummer_bh(600, seed=13, c=20.0, dt=1e-3)
+    xr, vr = Oracle(p.mass, p.G, p.c, p.softening, terms=CROSS_STAR).step(p.pos, p.vel, p.dt, 20)
+    xh, vh = Oracle(p.mass, p.G, p.c, p.softening).step(p.pos, p.vel, p.dt, 20)
+    out = []
+    for use_graph in (1, 0):
+        with _pn_cross(p) as pn:
+            pn.pn_set_option(binding.PN_OPT_USE_GRAPH, use_graph)
+            pn.pn_set_state_host(p.pos, p.vel)
+            pn.pn_step(p.dt, 20)
+            out.append(pn.pn_get_state_host())
+    (x, v), (x2, v2) = out
+    assert np.array_equal(x, x2) and np.array_equal(v, v2)
+    assert max(rel_err_rows(x, xr).max(), rel_err_rows(v, vr).max()) <= 1e-11
+    assert rel_err_rows(v, vh).max() > 1e-9  # and it is not the hot-path trajectory
