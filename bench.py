@@ -34,8 +34,10 @@ if str(ROOT) not in sys.path:
 #   4 symmetric, equal-mass form (every star has the same mass, as in every BASELINE.json config): the two mass
 #     multiplications go: 3 DADD + 12 DFMA + 3 DMUL = 18 per unordered pair = 9 per ordered pair
 #   5 ordered pairs with the Cross terms of Eq. 2.6 (--cross): 36 DADD + 124 DFMA + 56 DMUL per 4 pairs = 54 per ordered pair
+#   6 the same plus the O(N^2) sum of Eq. 2.3 (--cross full): 59 per ordered pair
 PAIR_KERNELS = {0: ("pair_fp64_kernel", 15, 24.0), 2: ("pair_sym_fp64_kernel", 10, 16.0),
-                4: ("pair_sym_fp64_kernel<EQM>", 9, 15.0), 5: ("pair_cross_fp64_kernel", 54, 85.0)}
+                4: ("pair_sym_fp64_kernel<EQM>", 9, 15.0), 5: ("pair_cross_fp64_kernel", 54, 85.0),
+                6: ("pair_cross_fp64_kernel<BHX>", 59, 93.0)}
 SMS, FP64_LANES_PER_SM = 148, 64
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu --set full
 # captures (profiles/), keyed by (variant, N_s); null when no capture exists for the workload
@@ -222,7 +224,7 @@ def run_reference(args) -> None:
     from oracle.pn_oracle import Oracle
 
     p = make_problem(args.workload)
-    o = Oracle(p.mass, p.G, p.c, p.softening, kind="fast", terms=1 if args.cross else 0)
+    o = Oracle(p.mass, p.G, p.c, p.softening, kind="fast", terms=cross_mask(args))
     # bound the whole run to ~4e10 pair visits (about 1.5 min on 8 cores) whatever K is
     rows, what = oracle_rows(p, budget_pairs=max(2.0e8, 4.0e10 / max(1, args.steps)))
     for _ in range(args.warmup):
@@ -263,11 +265,18 @@ def whole_job_rate(world: int, steps: int, pairs_per_step: int, seconds: float) 
     return world * steps * pairs_per_step / seconds
 
 
+def cross_mask(args) -> int:
+    """PN_OPT_CROSS_TERMS value (== the oracle's terms mask): 0, 1 = Eq. 2.6, 3 = Eqs. 2.6 + 2.3."""
+    return {None: 0, "star": 1, "full": 3}[getattr(args, "cross", None)]
+
+
 def workload_config(p, args) -> dict:
     return {"workload": p.name, "N": p.N, "n_stars": p.n_stars, "pairs_per_force_eval": p.pairs_per_eval,
             "force_evals_per_step": 4, "dt": p.dt, "c": p.c, "softening": p.softening, "M": float(p.mass[0]),
             "integrator": "classical RK4", "energy_evals_in_timed_region": 2,
-            "force": "hot path + [a_i]_Cross (Eq. 2.6)" if getattr(args, "cross", False) else "hot path (north_star)",
+            "force": {None: "hot path (north_star)", "star": "hot path + [a_i]_Cross (Eq. 2.6)",
+                      "full": "hot path + [a_i]_Cross (Eq. 2.6) + [a_1]_Cross (Eq. 2.3): the paper's full limited-1PN force"}[
+                          getattr(args, "cross", None)],
             "l2": "flushed (256 MiB write) between timed steps, outside the per-step event pairs",
             "parallelism": f"replicas x{args.gpus}" if args.gpus > 1 else "single GPU"}
 
@@ -300,7 +309,7 @@ def run_ours(args) -> None:
     stream = torch.cuda.current_stream()
     pn = PN(p.mass, p.G, p.c, p.softening, stream=stream)
     if args.cross:
-        pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, binding.PN_CROSS_STAR)
+        pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, cross_mask(args))
     cfg = pn.pn_get_pair_config()
     pos_d, vel_d = torch.from_numpy(p.pos).cuda(), torch.from_numpy(p.vel).cuda()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
@@ -403,7 +412,7 @@ def run_ours(args) -> None:
             "peak_measured_dfma": dfma_peak,
             "frac_of_measured_dfma": (achieved / dfma_peak) if achieved and dfma_peak else None,
         }
-        base = cpu_baseline(p, terms=1 if args.cross else 0) if not args.no_cpu_baseline else None
+        base = cpu_baseline(p, terms=cross_mask(args)) if not args.no_cpu_baseline else None
         line = {
             "metric": "fp64 pair-interactions/s", "value": value, "unit": "pair-interactions/s", "n_gpus": world,
             "steps": K, "warmup": W, "ms_per_step": ms_total_m / K, "higher_is_better": True, "scaling": "weak",
@@ -448,7 +457,8 @@ def run_sweep(args) -> None:
         pn.pn_set_option(binding.PN_OPT_TIME_PAIR, 1)
         # third leg: the first NEXT row of the scope table, [a_i]_Cross (Eq. 2.6) fused into an fp64 ordered-pair kernel
         for prec, pname, peak, cross in ((binding.PN_FP64, "fp64", peak64, 0), (binding.PN_FP32_PAIR, "fp32pair", peak32, 0),
-                                         (binding.PN_FP64, "fp64+cross", peak64, binding.PN_CROSS_STAR)):
+                                         (binding.PN_FP64, "fp64+cross", peak64, binding.PN_CROSS_STAR),
+                                         (binding.PN_FP64, "fp64+cross_full", peak64, binding.PN_CROSS_STAR | binding.PN_CROSS_BH)):
             pn.pn_set_option(binding.PN_OPT_PAIR_PRECISION, prec)
             pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, cross)
             instr = pn.pn_get_pair_config()["fp64_instr_per_pair"]  # pipe instructions per ordered pair of the kernel in use
@@ -474,6 +484,49 @@ def run_sweep(args) -> None:
         pn.pn_destroy()
 
 
+# PAPER.md:137-142, Table 3.2: elapsed seconds of 32 RK4 steps + energy at both ends, mean of 10 samples,
+# N: (CPU+GPU [Tesla K20c via Goose], CPU only [one core of an i7-3770K])
+PAPER_TABLE_3_2 = {100: (1.5392, 0.3479), 300: (1.9651, 3.0501), 1000: (1.941, 33.652), 3000: (5.0517, 302.31),
+                   10000: (38.934, 3358.6), 30000: (339.956, 30188.0)}
+
+
+def run_paper_timing(args) -> None:
+    """The paper's timing experiment with its full limited-1PN force (Eqs. 2.1-2.6) through the C-ABI: per N, 10 samples of
+    [pn_energy, pn_step(dt, 32), pn_energy], device-resident state, wall clock around the three calls (pn_energy
+    synchronises).  Context against another machine's numbers, not a target."""
+    import torch
+
+    from paper_1801_07986_b200 import PN, binding, inputs
+
+    torch.cuda.set_device(0)
+    for n_total, (t_gpu_paper, t_cpu_paper) in PAPER_TABLE_3_2.items():
+        p = inputs.cold_shell_bh(n_total, seed=n_total)
+        pn = PN(p.mass, p.G, p.c, p.softening, stream=torch.cuda.current_stream())
+        pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, binding.PN_CROSS_STAR | binding.PN_CROSS_BH)
+        pos, vel = torch.from_numpy(p.pos).cuda(), torch.from_numpy(p.vel).cuda()
+        samples, drift = [], None
+        for rep in range(12):  # 2 warm-up + 10 samples
+            pn.pn_set_state(pos, vel)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            e0 = pn.pn_energy()
+            pn.pn_step(p.dt, 32)
+            e1 = pn.pn_energy()
+            dt = time.perf_counter() - t0
+            if rep >= 2:
+                samples.append(dt)
+            drift = (e1 - e0) / abs(e0)
+        mean, sd = float(np.mean(samples)), float(np.std(samples, ddof=1))
+        print(json.dumps({
+            "workload": "paper_timing (PAPER.md:130-144, Table 3.2)", "N": n_total, "rk4_steps": 32, "energy_evals": 2,
+            "force": "full limited 1PN (Eqs. 2.1-2.6)", "elapsed_s_mean": mean, "elapsed_s_sd": sd, "samples": len(samples),
+            "energy_drift_32_steps": drift, "paper_elapsed_s_k20c": t_gpu_paper, "paper_elapsed_s_cpu_1core": t_cpu_paper,
+            "paper_hardware": "Tesla K20c + Core i7-3770K (Goose 1.3.3)", "ratio_vs_paper_gpu": t_gpu_paper / mean,
+            "ratio_vs_paper_cpu": t_cpu_paper / mean, "pair_config": pn.pn_get_pair_config(),
+            "note": "initial conditions of the paper's timing runs are not given; cold shell of PAPER.md:152-160"}), flush=True)
+        pn.pn_destroy()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--sweep", action="store_true", help="config-5 single-evaluation sweep (one JSON line per case)")
@@ -486,9 +539,16 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cross", action="store_true", help="add [a_i]_Cross, Eq. 2.6 (NEXT-1 of the scope table) to the force")
+    ap.add_argument("--cross", nargs="?", const="star", default=None, choices=["star", "full"],
+                    help="add the Cross terms (NEXT rows of the scope table): star = [a_i]_Cross, Eq. 2.6; "
+                         "full = also [a_1]_Cross, Eq. 2.3 (the paper's full limited-1PN force)")
+    ap.add_argument("--paper-timing", action="store_true",
+                    help="the paper's timing experiment (PAPER.md:130-144, Table 3.2): 32 RK4 steps + 2 energy evaluations of "
+                         "the full limited-1PN force at N = 100 ... 30000, one JSON line per N")
     args = ap.parse_args()
-    if args.sweep:
+    if args.paper_timing:
+        run_paper_timing(args)
+    elif args.sweep:
         run_sweep(args)
     elif args.impl == "reference":
         run_reference(args)

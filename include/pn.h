@@ -59,9 +59,12 @@ extern "C" {
                                    (PAPER.md:70-86), to every star's acceleration -- the first NEXT row of the scope table:
                                    its O(N^2) sums are fused into an fp64 ordered-pair kernel that also produces the
                                    Newtonian star-star term (54 FP64 instructions per ordered pair), its O(N) parts go into
-                                   the epilogue.  Applies to pn_accel and pn_step; pn_energy is Eq. 2.7 either way.
-                                   [a_1]_Cross (Eq. 2.3) is not built: the massive object keeps Eqs. 2.1 + 2.2. */
+                                   the epilogue.  PN_CROSS_STAR | PN_CROSS_BH: also [a_1]_Cross, Eq. 2.3, the
+                                   second NEXT row -- the paper's full limited-1PN force (one more O(N^2) sum per star in the
+                                   same kernel, 59 instructions per pair; the rest is O(N)).  Applies to pn_accel and
+                                   pn_step; pn_energy is Eq. 2.7 either way. */
 #define PN_CROSS_STAR 1
+#define PN_CROSS_BH 2
 
 /* PN_OPT_PAIR_PRECISION values */
 #define PN_FP64 0      /* fp64 pair arithmetic and accumulation (parity 1e-12) */
@@ -113,7 +116,8 @@ int pn_get_pair_config(pn_ctx* ctx, int32_t* cfg_host); /* 8 ints: threads/block
                                                            instructions per ordered pair, variant (0 fp64 tiled,
                                                            1 fp32 tiled, 2 fp64 symmetric, 3 fp32 symmetric,
                                                            4 fp64 symmetric, equal-mass form,
-                                                           5 fp64 ordered pairs with the Cross terms of Eq. 2.6) */
+                                                           5 fp64 ordered pairs with the Cross terms of Eq. 2.6,
+                                                           6 the same with the O(N^2) sum of Eq. 2.3) */
 
 int pn_measure_fp64_peak(pn_ctx* ctx, double* tflops_host); /* sustained FP64 FMA rate of this device from a register-only
                                                               DFMA-chain kernel (2 flops per FMA), best of 3: the measured

@@ -17,7 +17,7 @@ LIB_PATH = PKG / "libpn.so"
 
 PN_OK, PN_EINVAL, PN_ECUDA, PN_ESTATE, PN_ENOMEM = 0, -1, -2, -3, -4
 PN_OPT_PAIR_PRECISION, PN_OPT_USE_GRAPH, PN_OPT_TIME_PAIR, PN_OPT_J_SPLIT, PN_OPT_PAIR_KERNEL, PN_OPT_EQUAL_MASS, PN_OPT_CROSS_TERMS = 1, 2, 3, 4, 5, 6, 7
-PN_CROSS_STAR = 1
+PN_CROSS_STAR, PN_CROSS_BH = 1, 2
 PN_FP64, PN_FP32_PAIR = 0, 1
 PN_PAIR_AUTO, PN_PAIR_TILED, PN_PAIR_SYMMETRIC = 0, 1, 2
 

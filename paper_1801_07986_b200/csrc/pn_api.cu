@@ -229,8 +229,12 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
         cross_prep_kernel<kNT><<<nb, kNT, 0, st>>>(c->jrec[set], c->v[set], c->bh[set], c->crec, c->cblk, c->n_stars, c->np);
         cross_sum_kernel<<<1, 256, 0, st>>>(c->cblk, nb, c->csum);
         dim3 grid(c->np / (kCrossI * kNT), c->c_split);
-        pair_cross_fp64_kernel<kCrossI, 2, kNT, kCrossTJ><<<grid, kNT, 0, st>>>(c->crec, c->bh[set], c->part6, c->np,
-                                                                               c->c_tiles_per_split, c->eps2, c->GM);
+        if (c->cross & PN_CROSS_BH)
+            pair_cross_fp64_kernel<kCrossI, 2, kNT, kCrossTJ, true><<<grid, kNT, 0, st>>>(c->crec, c->bh[set], c->part6, c->np,
+                                                                                         c->c_tiles_per_split, c->eps2, c->GM);
+        else
+            pair_cross_fp64_kernel<kCrossI, 2, kNT, kCrossTJ, false><<<grid, kNT, 0, st>>>(c->crec, c->bh[set], c->part6, c->np,
+                                                                                          c->c_tiles_per_split, c->eps2, c->GM);
     } else if (c->precision == PN_FP32_PAIR) {
         split_kernel<<<(c->np + 255) / 256, 256, 0, st>>>(c->jrec[set], c->frec, c->n_stars, c->np);
         PN_CUDA(c, cudaGetLastError());
@@ -294,10 +298,12 @@ int enqueue_rk4_step(pn_ctx* c, cudaStream_t st, bool timed)
     for (int stage = 0; stage < 4; ++stage) {
         int rc = launch_pair(c, 0, st, timed);
         if (rc) return rc;
-        if (c->cross)
-            epilogue_kernel<MODE_RK4, kNT, true><<<grid, kNT, 0, st>>>(a, stage);
+        if (c->cross & PN_CROSS_BH)
+            epilogue_kernel<MODE_RK4, kNT, 2><<<grid, kNT, 0, st>>>(a, stage);
+        else if (c->cross)
+            epilogue_kernel<MODE_RK4, kNT, 1><<<grid, kNT, 0, st>>>(a, stage);
         else
-            epilogue_kernel<MODE_RK4, kNT, false><<<grid, kNT, 0, st>>>(a, stage);
+            epilogue_kernel<MODE_RK4, kNT, 0><<<grid, kNT, 0, st>>>(a, stage);
         PN_CUDA(c, cudaGetLastError());
     }
     return PN_OK;
@@ -492,8 +498,8 @@ int pn_set_option(pn_ctx* c, int key, int value)
             c->kernel_opt = value;
             return PN_OK;
         case PN_OPT_CROSS_TERMS: {
-            if (value != 0 && value != PN_CROSS_STAR)
-                return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_CROSS_TERMS takes 0 or PN_CROSS_STAR ([a_1]_Cross, Eq. 2.3, is not built)");
+            if (value != 0 && value != PN_CROSS_STAR && value != (PN_CROSS_STAR | PN_CROSS_BH))
+                return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_CROSS_TERMS takes 0, PN_CROSS_STAR or PN_CROSS_STAR | PN_CROSS_BH");
             if (value && !c->crec) {  // buffers of the cross path, on first use
                 const size_t np = c->np;
                 const int n_it = c->np / (kCrossI * kNT), n_t = c->np / kCrossTJ;
@@ -503,7 +509,7 @@ int pn_set_option(pn_ctx* c, int key, int value)
                 PN_CUDA(c, dalloc(&c->crec, np));
                 PN_CUDA(c, dalloc(&c->cblk, (np / kNT) * kCrossSums));
                 PN_CUDA(c, dalloc(&c->csum, kCrossSums));
-                PN_CUDA(c, dalloc(&c->part6, (size_t)c->c_split * 6 * np));
+                PN_CUDA(c, dalloc(&c->part6, (size_t)c->c_split * 7 * np));
             }
             c->cross = value;
             destroy_graphs(c);
@@ -580,10 +586,12 @@ int pn_accel(pn_ctx* c, const double* pos, const double* vel, double* acc)
     PN_CUDA(c, cudaGetLastError());
     if (int rc = launch_pair(c, 1, c->stream, c->time_pair != 0)) return rc;
     const EpiArgs a = epi_args(c, 1, acc);
-    if (c->cross)
-        epilogue_kernel<MODE_ACCEL, kNT, true><<<c->np / kEpiStars, kNT, 0, c->stream>>>(a, 0);
+    if (c->cross & PN_CROSS_BH)
+        epilogue_kernel<MODE_ACCEL, kNT, 2><<<c->np / kEpiStars, kNT, 0, c->stream>>>(a, 0);
+    else if (c->cross)
+        epilogue_kernel<MODE_ACCEL, kNT, 1><<<c->np / kEpiStars, kNT, 0, c->stream>>>(a, 0);
     else
-        epilogue_kernel<MODE_ACCEL, kNT, false><<<c->np / kEpiStars, kNT, 0, c->stream>>>(a, 0);
+        epilogue_kernel<MODE_ACCEL, kNT, 0><<<c->np / kEpiStars, kNT, 0, c->stream>>>(a, 0);
     PN_CUDA(c, cudaGetLastError());
     c->n_launch += 2 + kernels_per_eval(c);
     return PN_OK;
@@ -724,7 +732,8 @@ int pn_get_pair_config(pn_ctx* c, int32_t* cfg)
     if (!cfg) return fail(c, PN_EINVAL, "pn_get_pair_config: null pointer");
     if (c->cross) {
         cfg[0] = kNT, cfg[1] = kCrossI, cfg[2] = kCrossTJ, cfg[3] = c->c_split;
-        cfg[4] = (c->np / (kCrossI * kNT)) * c->c_split, cfg[5] = c->np, cfg[6] = 54, cfg[7] = 5;
+        cfg[4] = (c->np / (kCrossI * kNT)) * c->c_split, cfg[5] = c->np;
+        cfg[6] = (c->cross & PN_CROSS_BH) ? 59 : 54, cfg[7] = (c->cross & PN_CROSS_BH) ? 6 : 5;
         return PN_OK;
     }
     if (use_sym(c)) {

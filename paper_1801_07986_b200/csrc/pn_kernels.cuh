@@ -442,8 +442,9 @@ struct __align__(16) CRec {
     double x, y, z, gm;      // position, G m_j
     double vx, vy, vz, a5;   // velocity, 5 / (4 r_j1)
     double b, wx, wy, wz;    // 1 / (4 r_j1^3),  G m_j x_j1 / r_j1^3
+    double rj2, pad;         // r_j1^2 (used by the [a_1]_Cross sum only)
 };
-static_assert(sizeof(CRec) == 96, "CRec must be 96 bytes");
+static_assert(sizeof(CRec) == 112, "CRec must be 112 bytes");
 
 constexpr int kCrossSums = 8;  // P (3), Q1, Q3, W (3)
 
@@ -459,14 +460,14 @@ __global__ void __launch_bounds__(NT) cross_prep_kernel(const JRec* __restrict__
         const JRec r = jrec[i];
         CRec o;
         o.x = r.x, o.y = r.y, o.z = r.z, o.gm = r.gm;
-        o.vx = o.vy = o.vz = o.a5 = o.b = o.wx = o.wy = o.wz = 0.0;
+        o.vx = o.vy = o.vz = o.a5 = o.b = o.wx = o.wy = o.wz = o.rj2 = o.pad = 0.0;
         if (i < n_stars) {
             const double d[3] = {r.x - bh->xs[0], r.y - bh->xs[1], r.z - bh->xs[2]};  // x_j1
             const double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
             const double inv_r = 1.0 / sqrt(r2);
             const double inv_r3 = inv_r * inv_r * inv_r;
             o.vx = v[i], o.vy = v[np + i], o.vz = v[2 * np + i];
-            o.a5 = 1.25 * inv_r, o.b = 0.25 * inv_r3;
+            o.a5 = 1.25 * inv_r, o.b = 0.25 * inv_r3, o.rj2 = r2;
             o.wx = r.gm * d[0] * inv_r3, o.wy = r.gm * d[1] * inv_r3, o.wz = r.gm * d[2] * inv_r3;
             sums[0] = r.gm * o.vx, sums[1] = r.gm * o.vy, sums[2] = r.gm * o.vz;
             sums[3] = r.gm * inv_r, sums[4] = r.gm * inv_r3;
@@ -499,15 +500,24 @@ __global__ void __launch_bounds__(256) cross_sum_kernel(const double* __restrict
     if (lane == 0) out[q] = s;
 }
 
-template <int I, int MINB, int NT, int TJ>
+// BHX (NEXT-2, [a_1]_Cross, Eq. 2.3): with x_1j = x_1 - x_j and i, j both running over the stars,
+//   4 sum_j G^2 m_j^2 x_1j / r_1j^4
+//   + sum_{j != k} G^2 m_j m_k x_1j / r_1j^3 ( 4/r_1k + 5/(4 rho_jk) + (r_1j^2 - r_1k^2)/(4 rho_jk^3) )
+//   - (7/2) sum_{j != k} G^2 m_j m_k x_jk / (rho_jk^3 r_1j)                  [= + (7/2) sum_j (G m_j / r_1j) a_j^SS]
+//   - sum_{j, k} (G m_j m_k / (M r_1j^3)) [ 4 (v_j.v_k) x_1j - 3 (v_j.x_1j) v_k - 4 (v_k.x_1j) v_j ]   [O(N) with P]
+// needs one more O(N^2) sum per star, U_i = sum_{j != i} G m_j ( 5/(4 rho) + (r_i1^2 - r_j1^2)/(4 rho^3) ) (5 more FP64
+// instructions per pair, 7th output component); everything else is O(N) work in the epilogue, summed over the stars by
+// the reduction that already builds a_1.
+template <int I, int MINB, int NT, int TJ, bool BHX>
 __global__ void __launch_bounds__(NT, MINB) pair_cross_fp64_kernel(const CRec* __restrict__ crec, const BhState* __restrict__ bh,
-                                                                   double* __restrict__ part /* [S][6][np] */, int np,
+                                                                   double* __restrict__ part /* [S][6 + BHX][np] */, int np,
                                                                    int tiles_per_split, double eps2, double GM)
 {
+    constexpr int NC = BHX ? 7 : 6;
     __shared__ CRec sj[2][TJ];
     const int tid = threadIdx.x;
     double xi[I], yi[I], zi[I], vxi[I], vyi[I], vzi[I], ri2[I], ci[I], vi2[I];
-    double nx[I], ny[I], nz[I], ax[I], ay[I], az[I], S[I], Yx[I], Yy[I], Yz[I], H[I], Vx[I], Vy[I], Vz[I];
+    double nx[I], ny[I], nz[I], ax[I], ay[I], az[I], S[I], Yx[I], Yy[I], Yz[I], H[I], Vx[I], Vy[I], Vz[I], U[I];
     int ii[I];
 #pragma unroll
     for (int k = 0; k < I; ++k) {
@@ -518,12 +528,12 @@ __global__ void __launch_bounds__(NT, MINB) pair_cross_fp64_kernel(const CRec* _
         ri2[k] = dx * dx + dy * dy + dz * dz;
         ci[k] = 4.0 / sqrt(ri2[k]);
         vi2[k] = c.vx * c.vx + c.vy * c.vy + c.vz * c.vz;
-        nx[k] = ny[k] = nz[k] = ax[k] = ay[k] = az[k] = S[k] = Yx[k] = Yy[k] = Yz[k] = H[k] = Vx[k] = Vy[k] = Vz[k] = 0.0;
+        nx[k] = ny[k] = nz[k] = ax[k] = ay[k] = az[k] = S[k] = Yx[k] = Yy[k] = Yz[k] = H[k] = Vx[k] = Vy[k] = Vz[k] = U[k] = 0.0;
     }
     const int n_tiles = np / TJ;
     const int t_begin = blockIdx.y * tiles_per_split;
     const int t_end = min(n_tiles, t_begin + tiles_per_split);
-    constexpr int kVec = TJ * 6;  // double2 per tile
+    constexpr int kVec = TJ * 7;  // double2 per tile
     auto fill = [&](int buf, int t) {
         const double2* src = reinterpret_cast<const double2*>(crec + (size_t)t * TJ);
         double2* dst = reinterpret_cast<double2*>(sj[buf]);
@@ -567,13 +577,15 @@ __global__ void __launch_bounds__(NT, MINB) pair_cross_fp64_kernel(const CRec* _
                 const double h = s * fma(4.0, vix, -3.0 * vjx);
                 H[k] += h;
                 Vx[k] = fma(h, r.vx, Vx[k]), Vy[k] = fma(h, r.vy, Vy[k]), Vz[k] = fma(h, r.vz, Vz[k]);
+                if (BHX) U[k] = fma(gm * y, fma((ri2[k] - r.rj2) * y2, 0.25, 1.25), U[k]);
             }
         }
         __syncthreads();
     }
-    double* out = part + (size_t)blockIdx.y * 6 * np;
+    double* out = part + (size_t)blockIdx.y * NC * np;
 #pragma unroll
     for (int k = 0; k < I; ++k) {
+        if (BHX) out[6 * np + ii[k]] = U[k];
         const double dx = xi[k] - bh->xs[0], dy = yi[k] - bh->xs[1], dz = zi[k] - bh->xs[2];  // x_i1
         const double inv_r = 0.25 * ci[k];
         const double c1 = GM * inv_r * inv_r * inv_r * S[k];  // L1 pair part: GM x_i1 / r_i1^3 * S
@@ -891,11 +903,12 @@ constexpr int kEpiStars = 32;  // stars per epilogue block: lane = star, warp w 
 
 // CROSS: the partial sums carry 6 components (a^SS and the pair part of [a_i]_Cross, Eq. 2.6); the O(N) parts of the
 // Cross term are added here (see pair_cross_fp64_kernel).
-template <int MODE, int NT, bool CROSS>
+// CROSS = 2: additionally the star's share of [a_1]_Cross (Eq. 2.3), 7th component U (see pair_cross_fp64_kernel<BHX>).
+template <int MODE, int NT, int CROSS>
 __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
 {
     constexpr int NW = NT / 32;
-    constexpr int NC = CROSS ? 6 : 3;
+    constexpr int NC = CROSS == 2 ? 7 : (CROSS ? 6 : 3);
     static_assert(NW == 4, "the fixed-order cross-warp sum below is written for 4 warps");
     __shared__ double red[3 * NW];
     __shared__ double wsum[NW][NC][kEpiStars];
@@ -961,6 +974,9 @@ __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
         const double gv = -A.inv_c2 * 3.0 * vx;
 #pragma unroll
         for (int k = 0; k < 3; ++k) a[k] = ss[k] + cs * (fx * x[k] + fv * vel[k]);
+        b0 = cb * (gx * x[0] + gv * vel[0]);
+        b1 = cb * (gx * x[1] + gv * vel[1]);
+        b2 = cb * (gx * x[2] + gv * vel[2]);
         if (CROSS) {
             // [a_i]_Cross = L0 + the O(N) parts of L1, L3, L4 (global sums minus this star's own term) + pair part
             const double P[3] = {A.csum[0] - rec.gm * vel[0], A.csum[1] - rec.gm * vel[1], A.csum[2] - rec.gm * vel[2]};
@@ -977,10 +993,21 @@ __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
             const double kw = 3.5 * A.GM * inv_r;      // L3: + (7/2) GM W / r_i1
 #pragma unroll
             for (int k = 0; k < 3; ++k) a[k] += A.inv_c2 * (ss[3 + k] + kx * x[k] + kv * vel[k] + kp * P[k] + kw * W[k]);
+            if (CROSS == 2) {
+                // this star's share of [a_1]_Cross (x_1j = -x): T0 + T1 along x, T2 along a_j^SS, T3 with the FULL sum P
+                const double Pf[3] = {A.csum[0], A.csum[1], A.csum[2]};
+                const double vPf = vel[0] * Pf[0] + vel[1] * Pf[1] + vel[2] * Pf[2];
+                const double xPf = x[0] * Pf[0] + x[1] * Pf[1] + x[2] * Pf[2];
+                const double gr3 = rec.gm * inv_r3, g_M = gr3 / A.GM;
+                const double tx = -(4.0 * rec.gm * gr3 * inv_r + gr3 * (4.0 * Q1 + ss[6])) + 4.0 * g_M * vPf;  // times x
+                const double tP = -3.0 * g_M * vx;                                                             // times P
+                const double tv = -4.0 * g_M * xPf;                                                            // times v_j
+                const double ta = 3.5 * rec.gm * inv_r;                                                        // times a_j^SS
+                b0 += A.inv_c2 * (tx * x[0] + tP * Pf[0] + tv * vel[0] + ta * ss[0]);
+                b1 += A.inv_c2 * (tx * x[1] + tP * Pf[1] + tv * vel[1] + ta * ss[1]);
+                b2 += A.inv_c2 * (tx * x[2] + tP * Pf[2] + tv * vel[2] + ta * ss[2]);
+            }
         }
-        b0 = cb * (gx * x[0] + gv * vel[0]);
-        b1 = cb * (gx * x[1] + gv * vel[1]);
-        b2 = cb * (gx * x[2] + gv * vel[2]);
     }
 
     double hh = 0, dt = 0;

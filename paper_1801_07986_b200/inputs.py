@@ -142,6 +142,23 @@ def uniform_ball_bh(k: int, M: float = 0.1, c: float = 100.0, softening: float =
                    {"model": "uniform ball+bh", "seed": k})
 
 
+def cold_shell_bh(n_total: int = 10000, seed: int = 0, name: str | None = None) -> Problem:
+    """The paper's own model as a stand-in for its timing runs, whose initial conditions are not
+    given: N - 1 equal-mass stars, m = 1e-4, at rest, uniform in the shell 1 < r < 10; a massive object
+    of mass M = 100 m = 0.01 at the origin; c = G = 1, softening 1e-3, dt = 2^-15.  (The paper draws the positions
+    with an LCG whose constants it does not give; here numpy's PCG64 with the given seed.)"""
+    n_stars = n_total - 1
+    rng = np.random.default_rng(seed)
+    r = (1.0 + rng.uniform(0.0, 1.0, n_stars) * (10.0 ** 3 - 1.0)) ** (1.0 / 3.0)
+    x = r[:, None] * _isotropic(rng, n_stars)
+    m = 1e-4
+    mass = np.concatenate([[100.0 * m], np.full(n_stars, m)])
+    pos = np.vstack([np.zeros(3), x])
+    vel = np.zeros_like(pos)
+    return Problem(name or f"cold_shell_N{n_total}_seed{seed}", mass, pos, vel, 1.0, 1.0, 1e-3, 2.0 ** -15, 32,
+                   {"model": "cold shell+bh (paper)", "seed": seed})
+
+
 def config(idx: int, **kw) -> Problem:
     """BASELINE.json configs by number (1-based, as SURVEY.md section 8(d) lists them)."""
     if idx == 1:

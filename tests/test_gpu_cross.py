@@ -1,10 +1,10 @@
-"""GPU parity of the first NEXT row of the scope table: [a_i]_Cross, Eq. 2.6, switched on with
-PN_OPT_CROSS_TERMS = PN_CROSS_STAR, against the oracle's literal evaluation (terms = CROSS_STAR).  Same tolerance as the
-hot path: err_i = max_k |a_ik - ref_ik| / ||ref_i||_2 <= 1e-12."""
+"""GPU parity of the NEXT rows of the scope table: [a_i]_Cross, Eq. 2.6, and [a_1]_Cross, Eq. 2.3
+(PAPER.md:51-57), switched on with PN_OPT_CROSS_TERMS = PN_CROSS_STAR [| PN_CROSS_BH], against the oracle's literal
+evaluation with the same terms.  Same tolerance as the hot path: err_i = max_k |a_ik - ref_ik| / ||ref_i||_2 <= 1e-12."""
 import numpy as np
 import pytest
 
-from oracle.pn_oracle import CROSS_STAR, Oracle
+from oracle.pn_oracle import CROSS_BH, CROSS_STAR, Oracle
 from paper_1801_07986_b200 import inputs
 from tests.conftest import rel_err_rows
 
@@ -18,33 +18,42 @@ def _dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-def _pn_cross(p):
+TERMS = [CROSS_STAR, CROSS_STAR | CROSS_BH]  # the oracle's mask values equal the library's PN_CROSS_* values
+
+
+def _pn_cross(p, terms=CROSS_STAR):
     from paper_1801_07986_b200 import PN, binding
 
+    assert (binding.PN_CROSS_STAR, binding.PN_CROSS_BH) == (CROSS_STAR, CROSS_BH)
     pn = PN(p.mass, p.G, p.c, p.softening)
-    pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, binding.PN_CROSS_STAR)
+    pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, terms)
     return pn
 
 
+@pytest.mark.parametrize("terms", TERMS)
 @pytest.mark.parametrize("n_stars", [1, 2, 3, 129, 1023, 4099, 13001])
-def test_cross_accel_parity_sizes(n_stars):
+def test_cross_accel_parity_sizes(n_stars, terms):
     if n_stars <= 3:
         p = inputs.random_small(n_stars, seed=700 + n_stars, M=1.0, m_scale=1e-2, c=10.0, softening=1e-3, bh_moving=True)
     else:
         p = inputs.plummer_bh(n_stars, seed=700 + n_stars, c=20.0)  # a small c makes the 1PN terms 25 x larger than at c = 100
-    ref = Oracle(p.mass, p.G, p.c, p.softening, terms=CROSS_STAR).accel(p.pos, p.vel)
+    ref = Oracle(p.mass, p.G, p.c, p.softening, terms=terms).accel(p.pos, p.vel)
     hot = Oracle(p.mass, p.G, p.c, p.softening).accel(p.pos, p.vel)
-    with _pn_cross(p) as pn:
-        assert pn.pn_get_pair_config()["variant"] == 5
+    with _pn_cross(p, terms) as pn:
+        assert pn.pn_get_pair_config()["variant"] == (6 if terms & CROSS_BH else 5)
         acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
     assert rel_err_rows(acc, ref).max() <= TOL_ACC
     if n_stars >= 2:  # the Cross term is really there (with one star only the O(m_i) self line is left)
         assert rel_err_rows(hot[1:], ref[1:]).max() > 1e-9
-    assert np.array_equal(ref[0], hot[0])  # the massive object keeps Eqs. 2.1 + 2.2
+    if terms & CROSS_BH:
+        assert rel_err_rows(hot[:1], ref[:1]).max() > 1e-9  # [a_1]_Cross is really there
+    else:
+        assert np.array_equal(ref[0], hot[0])  # the massive object keeps Eqs. 2.1 + 2.2
 
 
+@pytest.mark.parametrize("terms", TERMS)
 @pytest.mark.parametrize("gen", ["cusp", "unequal_eps0", "tracers"])
-def test_cross_accel_parity_other_inputs(gen):
+def test_cross_accel_parity_other_inputs(gen, terms):
     if gen == "cusp":
         p = inputs.cusp_bh(3000, seed=5)
     elif gen == "unequal_eps0":
@@ -52,8 +61,8 @@ def test_cross_accel_parity_other_inputs(gen):
     else:
         p = inputs.plummer_bh(700, seed=9, c=30.0)
         p.mass[10:200] = 0.0
-    ref = Oracle(p.mass, p.G, p.c, p.softening, terms=CROSS_STAR).accel(p.pos, p.vel)
-    with _pn_cross(p) as pn:
+    ref = Oracle(p.mass, p.G, p.c, p.softening, terms=terms).accel(p.pos, p.vel)
+    with _pn_cross(p, terms) as pn:
         acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
     assert np.isfinite(acc).all()
     assert rel_err_rows(acc, ref).max() <= TOL_ACC
@@ -72,20 +81,21 @@ def test_cross_switch_off_restores_the_hot_path_bitwise_and_is_deterministic():
         pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, 0)
         a1 = pn.pn_accel(pos, vel).cpu().numpy()
         with pytest.raises(binding.PNError):
-            pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, 2)  # [a_1]_Cross is not built
+            pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, binding.PN_CROSS_BH)  # Eq. 2.3 needs the sums of Eq. 2.6: not alone
     assert np.array_equal(a0, a1) and np.array_equal(c1, c2) and not np.array_equal(a0, c1)
 
 
-def test_cross_rk4_trajectory_tracks_oracle():
+@pytest.mark.parametrize("terms", TERMS)
+def test_cross_rk4_trajectory_tracks_oracle(terms):
     """pn_step with the Cross terms (graph and plain launches) against the oracle's RK4 with the same terms."""
     from paper_1801_07986_b200 import binding
 
     p = inputs.plummer_bh(600, seed=13, c=20.0, dt=1e-3)
-    xr, vr = Oracle(p.mass, p.G, p.c, p.softening, terms=CROSS_STAR).step(p.pos, p.vel, p.dt, 20)
+    xr, vr = Oracle(p.mass, p.G, p.c, p.softening, terms=terms).step(p.pos, p.vel, p.dt, 20)
     xh, vh = Oracle(p.mass, p.G, p.c, p.softening).step(p.pos, p.vel, p.dt, 20)
     out = []
     for use_graph in (1, 0):
-        with _pn_cross(p) as pn:
+        with _pn_cross(p, terms) as pn:
             pn.pn_set_option(binding.PN_OPT_USE_GRAPH, use_graph)
             pn.pn_set_state_host(p.pos, p.vel)
             pn.pn_step(p.dt, 20)
