@@ -527,6 +527,39 @@ def run_paper_timing(args) -> None:
         pn.pn_destroy()
 
 
+def run_cold_collapse(args) -> None:
+    """The paper's test model (Fig. 2): N = 10^4 bodies, cold shell 1 < r < 10, M = 100 m = 0.01,
+    c = G = 1, softening 1e-3, classical RK4 with dt = 2^k, full limited-1PN force; relative energy error against t.
+    The paper reports about 1e-2 at t = 10, nearly independent of dt in {2^-17, 2^-16, 2^-15} (its
+    figures are missing from the extraction).  One JSON line per output time."""
+    import torch
+
+    from paper_1801_07986_b200 import PN, binding, inputs
+
+    torch.cuda.set_device(0)
+    p = inputs.cold_shell_bh(args.collapse_n, seed=0)
+    dt = 2.0 ** args.dt_log2
+    pn = PN(p.mass, p.G, p.c, p.softening, stream=torch.cuda.current_stream())
+    if not args.collapse_hot_path:
+        pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, binding.PN_CROSS_STAR | binding.PN_CROSS_BH)
+    pn.pn_set_state(torch.from_numpy(p.pos).cuda(), torch.from_numpy(p.vel).cuda())
+    e0 = pn.pn_energy()
+    chunk = max(1, int(round(args.collapse_every / dt)))
+    n_chunks = int(round(args.t_end / (chunk * dt)))
+    t_wall = time.perf_counter()
+    for k in range(1, n_chunks + 1):
+        pn.pn_step(dt, chunk)
+        e = pn.pn_energy()
+        x, v = pn.pn_get_state()
+        r = torch.linalg.norm(x[1:] - x[0], dim=1)
+        print(json.dumps({"workload": "cold_collapse (PAPER.md:152-176)", "N": p.N, "dt_log2": args.dt_log2,
+                          "force": "hot path" if args.collapse_hot_path else "full limited 1PN (Eqs. 2.1-2.6)",
+                          "t": k * chunk * dt, "steps": k * chunk, "energy": e, "rel_energy_error": (e - e0) / abs(e0),
+                          "r_min_to_bh": float(r.min()), "r_median": float(r.median()),
+                          "wall_s": time.perf_counter() - t_wall}), flush=True)
+    pn.pn_destroy()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--sweep", action="store_true", help="config-5 single-evaluation sweep (one JSON line per case)")
@@ -542,11 +575,19 @@ def main():
     ap.add_argument("--cross", nargs="?", const="star", default=None, choices=["star", "full"],
                     help="add the Cross terms (NEXT rows of the scope table): star = [a_i]_Cross, Eq. 2.6; "
                          "full = also [a_1]_Cross, Eq. 2.3 (the paper's full limited-1PN force)")
+    ap.add_argument("--cold-collapse", action="store_true", help="the paper's test model: energy error against t (JSON lines)")
+    ap.add_argument("--collapse-n", type=int, default=10000)
+    ap.add_argument("--dt-log2", type=int, default=-15)
+    ap.add_argument("--t-end", type=float, default=10.0)
+    ap.add_argument("--collapse-every", type=float, default=0.25, help="output interval in time units")
+    ap.add_argument("--collapse-hot-path", action="store_true", help="without the Cross terms")
     ap.add_argument("--paper-timing", action="store_true",
                     help="the paper's timing experiment (PAPER.md:130-144, Table 3.2): 32 RK4 steps + 2 energy evaluations of "
                          "the full limited-1PN force at N = 100 ... 30000, one JSON line per N")
     args = ap.parse_args()
-    if args.paper_timing:
+    if args.cold_collapse:
+        run_cold_collapse(args)
+    elif args.paper_timing:
         run_paper_timing(args)
     elif args.sweep:
         run_sweep(args)

@@ -107,6 +107,11 @@ int pn_step(pn_ctx* ctx, double dt, int64_t nsteps);
  * O(N^2) pair sum in compensated fp64.  Synchronises the stream; *E_host is a host double. */
 int pn_energy(pn_ctx* ctx, double* E_host);
 
+/* Total 1PN momentum of the internal state, Eq. 2.8 (the third NEXT row of the scope table) in the
+ * reading R16 of DESIGN.md: the EIH momentum with every term kept that the paper's error order needs.  P_host: 3 host
+ * doubles.  O(N^2) pair sum over the unordered star pairs in compensated fp64.  Synchronises the stream. */
+int pn_momentum(pn_ctx* ctx, double* P_host);
+
 /* Bookkeeping for benchmarks. */
 int pn_get_launch_count(pn_ctx* ctx, int64_t* n_kernels_host);          /* kernels launched (graph nodes count) */
 int pn_get_pair_time(pn_ctx* ctx, double* ms_total_host, int64_t* n_launches_host, int reset); /* PN_OPT_TIME_PAIR;

@@ -467,3 +467,67 @@ int oracle_energy(int64_t N, const double* mass, double G_, double c, double eps
     free(m), free(x), free(v), free(row);
     return ORACLE_OK;
 }
+
+/* ---------------------------------------------------------------------------------------
+ * NEXT-3 of the scope table: total 1PN momentum, Eq. 2.8.  The extraction garbles the indices of the
+ * second sum in the braces ("sum_i (G m_i m_j / r_1j)[v_i + (v_i.n_ij) n_ij]").  Reading R16: the 1PN
+ * momentum of the parent (EIH) theory, sum_a m_a v_a (1 + v_a^2 / 2c^2) - (1/2c^2) sum_{a != b} (G m_a m_b / r_ab)
+ * [v_a + (v_a.n_ab) n_ab], with every term kept that is needed for the error order the paper states,
+ * O(G m_i^3 v_i / (c^2 M r)):
+ *   P = M v_1 + sum_i m_i v_i (1 + v_i^2 / 2c^2)
+ *       - (1/2c^2) { sum_i (G M m_i / r_1i) [ v_i + (v_i.n_1i) n_1i ]            (a = star i, b = #1; printed)
+ *                  + sum_i (G M m_i / r_1i) [ v_1 + (v_1.n_1i) n_1i ]            (a = #1, b = star i; O(m^2) as v_1 = O(m))
+ *                  + sum_{i != j} (G m_i m_j / rho_ij) [ v_i + (v_i.n_ij) n_ij ] }   (stars; softened, n_ij = x_ij / rho_ij)
+ * Dropped: (1/2c^2) M v_1^2 v_1 = O(m^3).  Pinned by the O(lam^3) residual against the EIH momentum.
+ * ------------------------------------------------------------------------------------- */
+int oracle_momentum(int64_t N, const double* mass, double G_, double c, double eps, const double* pos,
+                    const double* vel, double* P_out)
+{
+    int rc = check_args(N, mass, G_, c, eps);
+    if (rc) return rc;
+    if (!pos || !vel || !P_out) return ORACLE_EINVAL;
+    real *m = to_real(mass, N), *x = to_real(pos, 3 * N), *v = to_real(vel, 3 * N);
+    real* row = (real*)calloc((size_t)N * 3, sizeof(real));
+    if (!m || !x || !v || !row) {
+        free(m), free(x), free(v), free(row);
+        return ORACLE_ENOMEM;
+    }
+    const real G = (real)G_, M = m[0], inv_c2 = 1 / ((real)c * (real)c), eps2 = (real)eps * (real)eps;
+    const real* v1 = v;
+    real P[3], B[3] = {0, 0, 0}, S[3] = {0, 0, 0};
+    for (int k = 0; k < 3; ++k) P[k] = M * v1[k];
+    for (int64_t i = 1; i < N; ++i) {
+        real x1i[3], n1i[3];
+        for (int k = 0; k < 3; ++k) x1i[k] = x[k] - x[3 * i + k];
+        const real r1i = R_SQRT(dot3(x1i, x1i));
+        for (int k = 0; k < 3; ++k) n1i[k] = x1i[k] / r1i;
+        const real* vi = v + 3 * i;
+        const real vi2 = dot3(vi, vi);
+        for (int k = 0; k < 3; ++k) {
+            P[k] += m[i] * vi[k] * (1 + (real)0.5 * inv_c2 * vi2);
+            B[k] += G * M * m[i] / r1i * (vi[k] + dot3(vi, n1i) * n1i[k]);
+            B[k] += G * M * m[i] / r1i * (v1[k] + dot3(v1, n1i) * n1i[k]);
+        }
+    }
+#ifdef _OPENMP
+#pragma omp parallel for schedule(dynamic, 16)
+#endif
+    for (int64_t i = 1; i < N; ++i) {
+        const real* vi = v + 3 * i;
+        real acc[3] = {0, 0, 0};
+        for (int64_t j = 1; j < N; ++j) {
+            if (j == i) continue;
+            real xij[3], nij[3];
+            for (int k = 0; k < 3; ++k) xij[k] = x[3 * i + k] - x[3 * j + k];
+            const real rho = R_SQRT(dot3(xij, xij) + eps2);
+            for (int k = 0; k < 3; ++k) nij[k] = xij[k] / rho;
+            for (int k = 0; k < 3; ++k) acc[k] += G * m[i] * m[j] / rho * (vi[k] + dot3(vi, nij) * nij[k]);
+        }
+        for (int k = 0; k < 3; ++k) row[3 * i + k] = acc[k];
+    }
+    for (int64_t i = 1; i < N; ++i)
+        for (int k = 0; k < 3; ++k) S[k] += row[3 * i + k];
+    for (int k = 0; k < 3; ++k) P_out[k] = (double)(P[k] - (real)0.5 * inv_c2 * (B[k] + S[k]));
+    free(m), free(x), free(v), free(row);
+    return ORACLE_OK;
+}

@@ -79,6 +79,8 @@ def _load(kind: str) -> ctypes.CDLL:
     lib.oracle_accel_rows.argtypes = [i64, dp, dbl, dbl, dbl, dp, dp, i64, ip, dp]
     lib.oracle_step.argtypes = [i64, dp, dbl, dbl, dbl, dp, dp, dbl, i64]
     lib.oracle_energy.argtypes = [i64, dp, dbl, dbl, dbl, dp, dp, dp, dp]
+    lib.oracle_momentum.argtypes = [i64, dp, dbl, dbl, dbl, dp, dp, dp]
+    lib.oracle_momentum.restype = ctypes.c_int
     lib.oracle_accel_rows_terms.argtypes = [i64, dp, dbl, dbl, dbl, dp, dp, i64, ip, ctypes.c_int, dp]
     lib.oracle_step_terms.argtypes = [i64, dp, dbl, dbl, dbl, dp, dp, dbl, i64, ctypes.c_int]
     for f in (lib.oracle_accel, lib.oracle_accel_rows, lib.oracle_step, lib.oracle_energy, lib.oracle_accel_rows_terms,
@@ -153,6 +155,13 @@ class Oracle:
         _check(self.lib.oracle_step_terms(n, _d(m), self.G, self.c, self.eps, _d(pos), _d(vel), float(dt), int(nsteps),
                                           self.terms), "oracle_step_terms")
         return pos, vel
+
+    def momentum(self, pos, vel) -> np.ndarray:
+        """Total 1PN momentum, Eq. 2.8 in the reading R16 of DESIGN.md."""
+        n, m, pos, vel = _prep(self.mass, pos, vel)
+        out = np.zeros(3, dtype=np.float64)
+        _check(self.lib.oracle_momentum(n, _d(m), self.G, self.c, self.eps, _d(pos), _d(vel), _d(out)), "oracle_momentum")
+        return out
 
     def energy(self, pos, vel, terms: bool = False):
         n, m, pos, vel = _prep(self.mass, pos, vel)

@@ -24,7 +24,7 @@ PN_PAIR_AUTO, PN_PAIR_TILED, PN_PAIR_SYMMETRIC = 0, 1, 2
 # every symbol include/pn.h declares (tests check that the library exports all of them)
 EXPORTS = (
     "pn_create", "pn_destroy", "pn_set_stream", "pn_set_option", "pn_set_state", "pn_get_state",
-    "pn_set_state_host", "pn_get_state_host", "pn_accel", "pn_accel_host", "pn_step", "pn_energy",
+    "pn_set_state_host", "pn_get_state_host", "pn_accel", "pn_accel_host", "pn_step", "pn_energy", "pn_momentum",
     "pn_get_launch_count", "pn_get_pair_time", "pn_get_pair_config", "pn_measure_fp64_peak", "pn_last_error",
     "pn_version",
 )
@@ -60,6 +60,7 @@ def load_library() -> ctypes.CDLL:
     lib.pn_accel_host.argtypes = [vp, vp, vp, vp]
     lib.pn_step.argtypes = [vp, dbl, i64]
     lib.pn_energy.argtypes = [vp, ctypes.POINTER(dbl)]
+    lib.pn_momentum.argtypes = [vp, ctypes.POINTER(dbl)]
     lib.pn_get_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
     lib.pn_get_pair_time.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(i64), ci]
     lib.pn_get_pair_config.argtypes = [vp, ctypes.POINTER(ctypes.c_int32)]
@@ -183,6 +184,11 @@ class PN:
         e = ctypes.c_double(0.0)
         _check(self._lib, self._ctx, self._lib.pn_energy(self._ctx, ctypes.byref(e)))
         return e.value
+
+    def pn_momentum(self) -> np.ndarray:
+        out = (ctypes.c_double * 3)()
+        _check(self._lib, self._ctx, self._lib.pn_momentum(self._ctx, out))
+        return np.array(list(out), dtype=np.float64)
 
     def pn_get_launch_count(self) -> int:
         n = ctypes.c_int64(0)

@@ -41,6 +41,7 @@ struct pn_ctx {
     CRec* crec = nullptr;     // cross mode: per-star records, block partials and totals of the O(N) sums, 6-component partials
     double *cblk = nullptr, *csum = nullptr, *part6 = nullptr;
     int c_split = 1, c_tiles_per_split = 0;
+    double* blk_mom = nullptr;  // pn_momentum scratch
     bool equal_mass = false;  // every star has the same mass > 0
     double gm_eq = 0;
 
@@ -461,7 +462,7 @@ int pn_destroy(pn_ctx* c)
     cudaFree(c->x0), cudaFree(c->v0), cudaFree(c->sx), cudaFree(c->sv);
     cudaFree(c->part), cudaFree(c->bh_part), cudaFree(c->ticket), cudaFree(c->prm);
     cudaFree(c->io_pos), cudaFree(c->io_vel), cudaFree(c->io_acc);
-    cudaFree(c->crec), cudaFree(c->cblk), cudaFree(c->csum), cudaFree(c->part6);
+    cudaFree(c->crec), cudaFree(c->cblk), cudaFree(c->csum), cudaFree(c->part6), cudaFree(c->blk_mom);
     cudaFree(c->frec), cudaFree(c->erec), cudaFree(c->blk_prep), cudaFree(c->blk_pair), cudaFree(c->d_energy);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     cudaGetLastError();
@@ -669,6 +670,32 @@ int pn_energy(pn_ctx* c, double* E)
     PN_CUDA(c, cudaGetLastError());
     c->n_launch += 3;
     PN_CUDA(c, cudaMemcpyAsync(E, c->d_energy, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    PN_CUDA(c, cudaStreamSynchronize(c->stream));
+    return PN_OK;
+}
+
+int pn_momentum(pn_ctx* c, double* P)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!P) return fail(c, PN_EINVAL, "pn_momentum: null pointer");
+    if (!c->have_state) return fail(c, PN_ESTATE, "pn_momentum: no state set");
+    const int n_it = c->np / kNT;
+    if (!c->blk_mom) {  // [n_it][6] + [n_it * e_split][6] + 3 results, on first use
+        PN_CUDA(c, dalloc(&c->blk_mom, 6 * (size_t)n_it * (1 + c->e_split) + 3));
+    }
+    double* blk_prep = c->blk_mom;
+    double* blk_pair = c->blk_mom + 6 * (size_t)n_it;
+    double* d_out = blk_pair + 6 * (size_t)n_it * c->e_split;
+    energy_prep_kernel<kNT><<<n_it, kNT, 0, c->stream>>>(c->jrec[0], c->v[0], c->bh[0], c->erec, c->blk_prep, c->n_stars, c->np,
+                                                        c->GM, c->G, c->inv_c2);  // builds the ERec stream
+    momentum_prep_kernel<kNT><<<n_it, kNT, 0, c->stream>>>(c->jrec[0], c->v[0], c->bh[0], blk_prep, c->n_stars, c->np, c->GM, c->G,
+                                                          c->inv_c2);
+    dim3 grid(n_it, c->e_split);
+    momentum_pair_kernel<kNT, kTJ><<<grid, kNT, 0, c->stream>>>(c->erec, blk_pair, c->n_stars, c->np, c->eps2, c->G);
+    momentum_final_kernel<256><<<1, 256, 0, c->stream>>>(blk_prep, n_it, blk_pair, n_it * c->e_split, c->bh[0], c->M, c->inv_c2, d_out);
+    PN_CUDA(c, cudaGetLastError());
+    c->n_launch += 4;
+    PN_CUDA(c, cudaMemcpyAsync(P, d_out, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     PN_CUDA(c, cudaStreamSynchronize(c->stream));
     return PN_OK;
 }

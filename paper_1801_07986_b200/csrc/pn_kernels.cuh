@@ -1338,4 +1338,136 @@ __global__ void __launch_bounds__(NT) energy_final_kernel(const double* __restri
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// NEXT-3 of the scope table: total 1PN momentum, Eq. 2.8 in the reading R16 of DESIGN.md:
+//   P = M v_1 + sum_i m_i v_i (1 + v_i^2/2c^2)
+//       - (1/2c^2) { sum_i (GM m_i / r_1i)[v_i + (v_i.n_1i) n_1i + v_1 + (v_1.n_1i) n_1i]
+//                  + sum_{i != j} (G m_i m_j / rho_ij)[v_i + (v_i.x_ij) x_ij / rho_ij^2] }.
+// The pair sum is symmetrised, sum_{i<j} (G m_i m_j / rho)[u + (u.d) d / rho^2] with u = v_i + v_j, d = x_ij, and walks
+// the unordered pairs exactly like energy_pair_kernel (same ERec stream, same grouped compensated summation).
+// ---------------------------------------------------------------------------------------------------------
+template <int NT>
+__global__ void __launch_bounds__(NT) momentum_prep_kernel(const JRec* __restrict__ jrec, const double* __restrict__ v,
+                                                           const BhState* __restrict__ bh, double* __restrict__ blk /* [grid][6] */,
+                                                           int n_stars, int np, double GM, double G, double inv_c2)
+{
+    __shared__ double red[2 * (NT / 32)];
+    const int i = blockIdx.x * NT + threadIdx.x;
+    double t[3] = {0, 0, 0};
+    if (i < n_stars) {
+        const JRec r = jrec[i];
+        const double vv[3] = {v[i], v[np + i], v[2 * np + i]};
+        const double v1[3] = {bh->vs[0], bh->vs[1], bh->vs[2]};
+        const double d[3] = {bh->xs[0] - r.x, bh->xs[1] - r.y, bh->xs[2] - r.z};  // x_1i
+        const double inv_r = 1.0 / sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        const double m = r.gm / G;
+        const double v2 = vv[0] * vv[0] + vv[1] * vv[1] + vv[2] * vv[2];
+        const double w[3] = {vv[0] + v1[0], vv[1] + v1[1], vv[2] + v1[2]};
+        const double wn = (w[0] * d[0] + w[1] * d[1] + w[2] * d[2]) * inv_r * inv_r;  // (w.n) / r
+        const double U = GM * m * inv_r;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) t[k] = m * vv[k] * (1.0 + 0.5 * inv_c2 * v2) - 0.5 * inv_c2 * U * (w[k] + wn * d[k]);
+    }
+    double* b = blk + 6 * (size_t)blockIdx.x;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        double hi = t[k], lo = 0;
+        block_sum_dd<NT>(hi, lo, red);
+        if (threadIdx.x == 0) b[2 * k] = hi, b[2 * k + 1] = lo;
+    }
+}
+
+template <int NT, int TJ>
+__global__ void __launch_bounds__(NT) momentum_pair_kernel(const ERec* __restrict__ erec, double* __restrict__ blk /* [grid][6] */,
+                                                           int n_stars, int np, double eps2, double G)
+{
+    static_assert(NT == TJ, "i-tiles and j-tiles share one index space");
+    constexpr int kGroup = 8;
+    __shared__ ERec sj[TJ];
+    __shared__ double red[2 * (NT / 32)];
+    const int tid = threadIdx.x;
+    const int i = blockIdx.x * NT + tid;
+    const ERec me = erec[i];
+    double hi[3] = {0, 0, 0}, lo[3] = {0, 0, 0};
+    const int n_tiles = np / TJ;
+    const int per = (n_tiles - (int)blockIdx.x + (int)gridDim.y - 1) / (int)gridDim.y;
+    const int t_begin = blockIdx.x + blockIdx.y * per;
+    const int t_end = min(n_tiles, t_begin + per);
+    for (int t = t_begin; t < t_end; ++t) {
+        __syncthreads();
+        {
+            const double2* src = reinterpret_cast<const double2*>(erec + (size_t)t * TJ);
+            double2* dst = reinterpret_cast<double2*>(sj);
+            for (int q = tid; q < TJ * 4; q += NT) dst[q] = src[q];
+        }
+        __syncthreads();
+        const int j0 = t * TJ;
+#pragma unroll 1
+        for (int jb = 0; jb < TJ; jb += kGroup) {
+            double g[3] = {0, 0, 0};
+#pragma unroll
+            for (int u = 0; u < kGroup; ++u) {
+                const int jj = jb + u;
+                const ERec r = sj[jj];
+                const double dx = me.x - r.x, dy = me.y - r.y, dz = me.z - r.z;  // x_ij
+                const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+                const double y0 = rsqrt_seed(r2);
+                const double e = fma(-r2, y0 * y0, 1.0);
+                double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1 / rho
+                y = (j0 + jj <= i) ? 0.0 : y;  // i < j only (also keeps the self pair's 1/0 out when eps = 0)
+                const double ux = me.vx + r.vx, uy = me.vy + r.vy, uz = me.vz + r.vz;
+                const double ud = fma(ux, dx, fma(uy, dy, uz * dz)) * (y * y);
+                const double c = r.gm * y;
+                g[0] = fma(c, fma(ud, dx, ux), g[0]);
+                g[1] = fma(c, fma(ud, dy, uy), g[1]);
+                g[2] = fma(c, fma(ud, dz, uz), g[2]);
+            }
+#pragma unroll
+            for (int k = 0; k < 3; ++k) two_sum_acc(hi[k], lo[k], g[k]);
+        }
+    }
+    const bool real_star = i < n_stars;  // pad stars (coincident, massless) may hold NaN with eps = 0
+    const double mi = me.gm / G;
+    double* b = blk + 6 * ((size_t)blockIdx.y * gridDim.x + blockIdx.x);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        double h = real_star ? hi[k] * mi : 0.0, l = real_star ? lo[k] * mi : 0.0;
+        block_sum_dd<NT>(h, l, red);
+        if (tid == 0) b[2 * k] = h, b[2 * k + 1] = l;
+    }
+}
+
+// out[0..2] = P.  One block; fixed order.
+template <int NT>
+__global__ void __launch_bounds__(NT) momentum_final_kernel(const double* __restrict__ blk_prep, int n_prep,
+                                                            const double* __restrict__ blk_pair, int n_pair,
+                                                            const BhState* __restrict__ bh, double M, double inv_c2,
+                                                            double* __restrict__ out)
+{
+    __shared__ double red[2 * (NT / 32)];
+    for (int k = 0; k < 3; ++k) {
+        double a_hi = 0, a_lo = 0, p_hi = 0, p_lo = 0;
+        for (int q = threadIdx.x; q < n_prep; q += NT) {
+            two_sum_acc(a_hi, a_lo, blk_prep[6 * q + 2 * k]);
+            a_lo += blk_prep[6 * q + 2 * k + 1];
+        }
+        for (int q = threadIdx.x; q < n_pair; q += NT) {
+            two_sum_acc(p_hi, p_lo, blk_pair[6 * q + 2 * k]);
+            p_lo += blk_pair[6 * q + 2 * k + 1];
+        }
+        block_sum_dd<NT>(a_hi, a_lo, red);
+        block_sum_dd<NT>(p_hi, p_lo, red);
+        if (threadIdx.x == 0) {
+            double hi = 0, lo = 0;
+            two_sum_acc(hi, lo, M * bh->vs[k]);
+            two_sum_acc(hi, lo, a_hi);
+            lo += a_lo;
+            two_sum_acc(hi, lo, -0.5 * inv_c2 * p_hi);
+            lo += -0.5 * inv_c2 * p_lo;
+            out[k] = hi + lo;
+        }
+        __syncthreads();
+    }
+}
+
 }  // namespace pn

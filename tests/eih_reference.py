@@ -110,3 +110,24 @@ def eih_energy(m, x, v, G, c):
                     continue
                 E1 += G * G * m[a] * m[b] * m[cc] / (r * r_(a, cc)) / 2
     return E0 + E1 / c2
+
+
+def eih_momentum(m, x, v, G, c):
+    """1PN total momentum of the EIH theory: sum m v (1 + v^2/2c^2) - (1/2c^2) sum_{a!=b} (G m_a m_b / r)[v_a + (v_a.n) n]."""
+    m = _v(m)
+    x = [_v(p) for p in x]
+    v = [_v(p) for p in v]
+    G, c2 = mpf(G), mpf(c) ** 2
+    n = len(m)
+    P = [mpf(0)] * 3
+    for a in range(n):
+        v2 = _dot(v[a], v[a])
+        P = [P[k] + m[a] * v[a][k] * (1 + v2 / (2 * c2)) for k in range(3)]
+        for b in range(n):
+            if b == a:
+                continue
+            d = _sub(x[a], x[b])
+            r = sqrt(_dot(d, d))
+            nab = [t / r for t in d]
+            P = [P[k] - G * m[a] * m[b] / r * (v[a][k] + _dot(v[a], nab) * nab[k]) / (2 * c2) for k in range(3)]
+    return P

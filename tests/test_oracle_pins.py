@@ -414,3 +414,53 @@ def test_cross_terms_two_body_finite_mass_periastron_advance():
            for t in (0, CROSS_STAR | CROSS_BH)}
     assert got[CROSS_STAR | CROSS_BH] == pytest.approx(1.0, abs=2.5e-3)
     assert got[0] == pytest.approx(0.9714, abs=2e-3)
+
+
+# ------------------------------------------------------------------ NEXT-3: total 1PN momentum, Eq. 2.8 (reading R16)
+@pytest.mark.parametrize("kind", KINDS)
+def test_momentum_vs_full_eih_residual_scaling(kind):
+    """Eq. 2.8 in the reading R16 keeps every EIH momentum term up to second order in the star masses: the residual is
+    the dropped (1/2c^2) M v_1^2 v_1 = O(lam^3) (the error order the paper states).  Without the a = #1
+    term or without the star-star sum the residual would be O(lam^2)."""
+    res = {}
+    for lam in (1e-1, 1e-2, 1e-3):
+        mass, pos, vel = _eih_system(lam, seed=2)
+        P_eih = np.array([float(t) for t in eih.eih_momentum(list(mass), _to_list(pos), _to_list(vel), 1.0, 10.0)])
+        P = Oracle(mass, 1.0, 10.0, 0.0, kind=kind).momentum(pos, vel)
+        res[lam] = np.abs(P - P_eih).max()
+    assert res[1e-1] / res[1e-2] == pytest.approx(1000.0, rel=0.05)
+    assert res[1e-2] / res[1e-3] == pytest.approx(1000.0, rel=0.05)
+    assert res[1e-2] == pytest.approx(1.5756e-10, rel=0.01)  # 1.58e-4 lam^3 at c = 10, seen when the reading was fixed
+
+
+def test_eih_reference_conserves_its_own_momentum():
+    """Pin of the pin: d/dt P_EIH along the EIH flow is O(c^-4)."""
+    m, x, v = _eih_system(0.3, seed=4)
+    out = {}
+    for c in (10.0, 100.0):
+        a = np.array([[float(t) for t in r] for r in eih.eih_acc(list(m), _to_list(x), _to_list(v), 1.0, c)])
+        h = 1e-6
+        Pp = np.array([float(t) for t in eih.eih_momentum(list(m), _to_list(x + h * v), _to_list(v + h * a), 1.0, c)])
+        Pm = np.array([float(t) for t in eih.eih_momentum(list(m), _to_list(x - h * v), _to_list(v - h * a), 1.0, c)])
+        out[c] = np.abs((Pp - Pm) / (2 * h)).max()
+    assert out[10.0] / out[100.0] == pytest.approx(1e4, rel=0.05)
+
+
+@pytest.mark.parametrize("kind", KINDS)
+def test_momentum_newtonian_limit_and_softening(kind):
+    p = inputs.random_small(40, seed=21, M=1.0, m_scale=1e-2, c=10.0, softening=0.05, bh_moving=True)
+    P_newton = (p.mass[:, None] * p.vel).sum(0)
+    assert Oracle(p.mass, p.G, math.inf, p.softening, kind=kind).momentum(p.pos, p.vel) == pytest.approx(P_newton, rel=1e-14, abs=1e-18)
+    # the 1PN part written independently in numpy (softened star-star distances, unsoftened distances to body 0)
+    n = p.N
+    d = p.pos[:, None, :] - p.pos[None, :, :]
+    soft = np.full((n, n), p.softening**2)
+    soft[0, :] = soft[:, 0] = 0.0
+    r = np.sqrt((d**2).sum(-1) + soft)
+    np.fill_diagonal(r, np.inf)
+    nv = (d * p.vel[:, None, :]).sum(-1) / r  # (v_a . n_ab)
+    pair = (p.G * p.mass[:, None] * p.mass[None, :] / r)[:, :, None] * (p.vel[:, None, :] + (nv / r)[:, :, None] * d)
+    v2 = (p.vel**2).sum(1)
+    v2[0] = 0.0  # the (1/2c^2) M v_1^2 v_1 term is dropped (O(m^3))
+    P = P_newton + (p.mass * v2 / (2 * p.c**2))[:, None].__mul__(p.vel).sum(0) - pair.sum((0, 1)) / (2 * p.c**2)
+    assert Oracle(p.mass, p.G, p.c, p.softening, kind=kind).momentum(p.pos, p.vel) == pytest.approx(P, rel=1e-12, abs=1e-16)
