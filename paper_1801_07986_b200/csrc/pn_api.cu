@@ -425,7 +425,7 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA(dalloc(&ctx->frec, np));
     {
         const int n_it = (int)(np / kNT);
-        int s = (kSMs * 8 + n_it - 1) / n_it;
+        int s = (kSMs * 8 + n_it / 2 - 1) / (n_it / 2);  // the energy pair kernel runs n_it / 2 mirrored i-tile pairs per j-split
         s = std::max(1, std::min(s, std::min(ctx->n_tiles, 64)));
         ctx->e_tiles_per_split = (ctx->n_tiles + s - 1) / s;
         ctx->e_split = (ctx->n_tiles + ctx->e_tiles_per_split - 1) / ctx->e_tiles_per_split;
@@ -661,11 +661,11 @@ int pn_energy(pn_ctx* c, double* E)
     energy_prep_kernel<kNT><<<n_it, kNT, 0, c->stream>>>(c->jrec[0], c->v[0], c->bh[0], c->erec, c->blk_prep, c->n_stars, c->np,
                                                         c->GM, c->G, c->inv_c2);
     PN_CUDA(c, cudaGetLastError());
-    dim3 grid(n_it, c->e_split);
+    dim3 grid(n_it / 2, c->e_split);
     energy_pair_kernel<kNT, kTJ><<<grid, kNT, 0, c->stream>>>(c->erec, c->blk_pair, c->n_stars, c->np, c->eps2, c->G,
                                                               c->inv_c2);
     PN_CUDA(c, cudaGetLastError());
-    energy_final_kernel<256><<<1, 256, 0, c->stream>>>(c->blk_prep, n_it, c->blk_pair, n_it * c->e_split, c->bh[0], c->M, c->GM,
+    energy_final_kernel<256><<<1, 256, 0, c->stream>>>(c->blk_prep, n_it, c->blk_pair, (n_it / 2) * c->e_split, c->bh[0], c->M, c->GM,
                                                        c->G, c->inv_c2, c->d_energy);
     PN_CUDA(c, cudaGetLastError());
     c->n_launch += 3;

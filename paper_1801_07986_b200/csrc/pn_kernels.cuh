@@ -1242,59 +1242,68 @@ __global__ void __launch_bounds__(NT) energy_pair_kernel(const ERec* __restrict_
     __shared__ ERec sj[TJ];
     __shared__ double red[2 * (NT / 32)];
     const int tid = threadIdx.x;
-    const int i = blockIdx.x * NT + tid;
     constexpr int kEGroup = 8;
     static_assert(TJ % kEGroup == 0, "tile must be a multiple of the summation group");
-    const ERec me = erec[i];
-    const double mi = me.gm / G;
-    const double wi1 = me.w - 1.0, c35 = 3.5 * inv_c2, c05 = 0.5 * inv_c2;
+    static_assert(NT == TJ, "i-tiles and j-tiles share one index space");
+    const double c35 = 3.5 * inv_c2, c05 = 0.5 * inv_c2;
+    const int n_tiles = np / TJ;  // even (np is a multiple of 2 NT)
     double hi = 0, lo = 0;
 
-    static_assert(NT == TJ, "i-tiles and j-tiles share one index space");
-    const int n_tiles = np / TJ;
-    const int per = (n_tiles - (int)blockIdx.x + (int)gridDim.y - 1) / (int)gridDim.y;
-    const int t_begin = blockIdx.x + blockIdx.y * per;
-    const int t_end = min(n_tiles, t_begin + per);
-    for (int t = t_begin; t < t_end; ++t) {
-        __syncthreads();
-        {
-            const double2* src = reinterpret_cast<const double2*>(erec + (size_t)t * TJ);
-            double2* dst = reinterpret_cast<double2*>(sj);
-            for (int q = tid; q < TJ * 4; q += NT) dst[q] = src[q];
-        }
-        __syncthreads();
-        const int j0 = t * TJ;
-#pragma unroll 1
-        for (int jb = 0; jb < TJ; jb += kEGroup) {
-            // kEGroup terms are added plainly (their sum is tiny next to the running total), then the group sum goes
-            // into the compensated accumulator: one TwoSum per kEGroup pairs instead of one per pair
-            double g = 0.0;
-#pragma unroll
-            for (int u = 0; u < kEGroup; ++u) {
-                const int jj = jb + u;
-                const ERec r = sj[jj];
-                const double dx = me.x - r.x, dy = me.y - r.y, dz = me.z - r.z;  // x_ij
-                const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
-                const double y0 = rsqrt_seed(r2);
-                const double t2 = y0 * y0;
-                const double e = fma(-r2, t2, 1.0);
-                const double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1/rho to full fp64 accuracy
-                const double vv = fma(me.vx, r.vx, fma(me.vy, r.vy, me.vz * r.vz));
-                const double xvi = fma(dx, me.vx, fma(dy, me.vy, dz * me.vz));
-                const double xvj = fma(dx, r.vx, fma(dy, r.vy, dz * r.vz));
-                // q = -1 + (1/c^2)[w_i + w_j - 7/2 v_i.v_j - 1/2 (x_ij.v_i)(x_ij.v_j)/rho^2]; me.w, r.w carry the 1/c^2
-                double q = wi1 + r.w;
-                q = fma(-c35, vv, q);
-                q = fma(-c05, (xvi * xvj) * (y * y), q);
-                double term = (r.gm * y) * q;
-                term = (j0 + jj <= i) ? 0.0 : term;  // i < j only (false only inside the diagonal tile)
-                g += term;
+    // i-tile `it` has n_tiles - it j-tiles to walk: a block takes tile blockIdx.x and its mirror n_tiles - 1 - blockIdx.x,
+    // so every block of the grid (n_tiles / 2, j-splits) has the same amount of work
+    for (int half = 0; half < 2; ++half) {
+        const int it = half ? n_tiles - 1 - (int)blockIdx.x : (int)blockIdx.x;
+        const int i = it * NT + tid;
+        const ERec me = erec[i];
+        const double wi1 = me.w - 1.0;
+        double h_hi = 0, h_lo = 0;
+        const int per = (n_tiles - it + (int)gridDim.y - 1) / (int)gridDim.y;
+        const int t_begin = it + blockIdx.y * per;
+        const int t_end = min(n_tiles, t_begin + per);
+        for (int t = t_begin; t < t_end; ++t) {
+            __syncthreads();
+            {
+                const double2* src = reinterpret_cast<const double2*>(erec + (size_t)t * TJ);
+                double2* dst = reinterpret_cast<double2*>(sj);
+                for (int q = tid; q < TJ * 4; q += NT) dst[q] = src[q];
             }
-            two_sum_acc(hi, lo, g);
+            __syncthreads();
+            const int j0 = t * TJ;
+#pragma unroll 1
+            for (int jb = 0; jb < TJ; jb += kEGroup) {
+                // kEGroup terms are added plainly (their sum is tiny next to the running total), then the group sum
+                // goes into the compensated accumulator: one TwoSum per kEGroup pairs instead of one per pair
+                double g = 0.0;
+#pragma unroll
+                for (int u = 0; u < kEGroup; ++u) {
+                    const int jj = jb + u;
+                    const ERec r = sj[jj];
+                    const double dx = me.x - r.x, dy = me.y - r.y, dz = me.z - r.z;  // x_ij
+                    const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+                    const double y0 = rsqrt_seed(r2);
+                    const double t2 = y0 * y0;
+                    const double e = fma(-r2, t2, 1.0);
+                    const double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1/rho to full fp64 accuracy
+                    const double vv = fma(me.vx, r.vx, fma(me.vy, r.vy, me.vz * r.vz));
+                    const double xvi = fma(dx, me.vx, fma(dy, me.vy, dz * me.vz));
+                    const double xvj = fma(dx, r.vx, fma(dy, r.vy, dz * r.vz));
+                    // q = -1 + (1/c^2)[w_i + w_j - 7/2 v_i.v_j - 1/2 (x_ij.v_i)(x_ij.v_j)/rho^2]; me.w, r.w carry the 1/c^2
+                    double q = wi1 + r.w;
+                    q = fma(-c35, vv, q);
+                    q = fma(-c05, (xvi * xvj) * (y * y), q);
+                    double term = (r.gm * y) * q;
+                    term = (j0 + jj <= i) ? 0.0 : term;  // i < j only (false only inside the diagonal tile)
+                    g += term;
+                }
+                two_sum_acc(h_hi, h_lo, g);
+            }
+        }
+        if (i < n_stars) {  // the factor m_i is common to all of star i's pairs
+            const double mi = me.gm / G;
+            two_sum_acc(hi, lo, h_hi * mi);
+            lo += h_lo * mi;
         }
     }
-    hi *= mi, lo *= mi;  // the factor m_i is common to all of thread i's pairs
-    if (i >= n_stars) hi = 0, lo = 0;
     block_sum_dd<NT>(hi, lo, red);
     if (tid == 0) {
         double* b = blk + 2 * ((size_t)blockIdx.y * gridDim.x + blockIdx.x);

@@ -236,6 +236,32 @@ def test_config1_trajectory_accel_and_energy_drift():
         assert worst_drift <= TOL_DRIFT
 
 
+def test_config3_like_cusp_trajectory_and_energy_drift():
+    """Config 3's recipe (Bahcall-Wolf cusp, mass ratio 1e4, c = 316, eps = 1e-4, dt = 1e-5, 20 steps) at a size the
+    oracle integrates in seconds: trajectory and drift parity where the dynamics is stiff (inner orbital period 2e-4, so
+    the energy drifts by percents within 20 steps: the drift must be the oracle's, not merely small)."""
+    p = inputs.cusp_bh(4095, seed=2)
+    o = Oracle(p.mass, p.G, p.c, p.softening)
+    with _pn(p) as pn:
+        pn.pn_set_state(_dev(p.pos), _dev(p.vel))
+        e0_gpu, e0_ref = pn.pn_energy(), o.energy(p.pos, p.vel)
+        assert e0_gpu == pytest.approx(e0_ref, rel=1e-13)
+        xr, vr = p.pos, p.vel
+        worst_traj = worst_drift = 0.0
+        drift_ref = 0.0
+        for _ in range(4):
+            pn.pn_step(p.dt, 5)
+            xr, vr = o.step(xr, vr, p.dt, 5)
+            xg, vg = pn.pn_get_state()
+            worst_traj = max(worst_traj, rel_err_rows(xg.cpu().numpy(), xr).max(), rel_err_rows(vg.cpu().numpy(), vr).max())
+            d_gpu = (pn.pn_energy() - e0_gpu) / abs(e0_gpu)
+            drift_ref = (o.energy(xr, vr) - e0_ref) / abs(e0_ref)
+            worst_drift = max(worst_drift, abs(d_gpu - drift_ref))
+    assert worst_traj <= 1e-10
+    assert worst_drift <= TOL_DRIFT
+    print(f"cusp 4095: oracle drift after 20 steps {drift_ref:.3e}, worst trajectory error {worst_traj:.2e}")
+
+
 def test_step_graph_and_plain_launches_agree_bitwise():
     from paper_1801_07986_b200 import binding
 
