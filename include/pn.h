@@ -46,8 +46,10 @@ extern "C" {
 /* pn_set_option keys */
 #define PN_OPT_PAIR_PRECISION 1 /* PN_FP64 (default) | PN_FP32_PAIR: arithmetic of the O(N^2) star-star pair loop */
 #define PN_OPT_USE_GRAPH 2      /* 1 (default): pn_step replays a captured CUDA graph; 0: plain launches */
-#define PN_OPT_TIME_PAIR 3      /* 1: bracket every star-star pair-kernel launch with CUDA events (forces plain
-                                   launches); read with pn_get_pair_time.  0 (default) */
+#define PN_OPT_TIME_PAIR 3      /* 1: bracket the pair stage of every force evaluation with CUDA events (pn_step: event-record
+                                   nodes inside a one-step CUDA graph; plain launches when PN_OPT_USE_GRAPH is 0); read with
+                                   pn_get_pair_time.  2: as 1, but in pn_step only the first of the four force evaluations
+                                   of a step is bracketed (a quarter of the instrumentation).  0 (default) */
 #define PN_OPT_J_SPLIT 4        /* 0 (default): automatic; > 0: force the number of j-chunks per i-tile (tiled kernel) */
 #define PN_OPT_PAIR_KERNEL 5    /* which fp64 star-star kernel: PN_PAIR_AUTO (default) | PN_PAIR_TILED | PN_PAIR_SYMMETRIC */
 

@@ -69,6 +69,13 @@ struct pn_ctx {
     double dt_dev = NAN;
 
     cudaGraphExec_t graph1 = nullptr, graphB = nullptr;
+    // timed one-step graph (PN_OPT_TIME_PAIR with graphs): event-record nodes around the pair stage of each RK4 stage;
+    // the events are swapped for fresh ones before every launch
+    cudaGraph_t graphT_src = nullptr;
+    cudaGraphExec_t graphT = nullptr;
+    cudaEvent_t tev[8] = {};
+    cudaGraphNode_t tnode[8] = {};
+    int cap_ev = -1;  // >= 0 while the timed graph is captured: next template event
     int graph_split = -1, graph_precision = -1, graph_sym = -1, graph_eqm = -1;
 
     int64_t n_launch = 0;
@@ -159,6 +166,8 @@ void destroy_graphs(pn_ctx* c)
 {
     if (c->graph1) cudaGraphExecDestroy(c->graph1), c->graph1 = nullptr;
     if (c->graphB) cudaGraphExecDestroy(c->graphB), c->graphB = nullptr;
+    if (c->graphT) cudaGraphExecDestroy(c->graphT), c->graphT = nullptr;
+    if (c->graphT_src) cudaGraphDestroy(c->graphT_src), c->graphT_src = nullptr;
 }
 
 // ---- launches ---------------------------------------------------------------------------------------------
@@ -212,16 +221,22 @@ void launch_pair_sym(pn_ctx* c, int set, cudaStream_t st)
         eqm ? launch_pair_sym_v<I, W, MINB, false, true>(c, set, st) : launch_pair_sym_v<I, W, MINB, false, false>(c, set, st);
 }
 
+int reserve_events(pn_ctx* c, size_t n)
+{
+    while (c->ev_used + n > c->ev.size()) {
+        cudaEvent_t e;
+        PN_CUDA(c, cudaEventCreate(&e));
+        c->ev.push_back(e);
+    }
+    return PN_OK;
+}
+
 int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
 {
-    if (timed) {
-        if (c->ev_used + 2 > c->ev.size()) {
-            for (int q = 0; q < 2; ++q) {
-                cudaEvent_t e;
-                PN_CUDA(c, cudaEventCreate(&e));
-                c->ev.push_back(e);
-            }
-        }
+    if (timed && c->cap_ev >= 0) {
+        PN_CUDA(c, cudaEventRecordWithFlags(c->tev[c->cap_ev], st, cudaEventRecordExternal));  // a real event-record node
+    } else if (timed) {
+        if (int rc = reserve_events(c, 2)) return rc;
         PN_CUDA(c, cudaEventRecord(c->ev[c->ev_used], st));
     }
     const bool mask = (c->eps2 == 0.0);
@@ -266,7 +281,10 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
     else
         mask ? launch_pair_fp64<1, 8, 4, true>(c, set, st) : launch_pair_fp64<1, 8, 4, false>(c, set, st);
     PN_CUDA(c, cudaGetLastError());
-    if (timed) {
+    if (timed && c->cap_ev >= 0) {
+        PN_CUDA(c, cudaEventRecordWithFlags(c->tev[c->cap_ev + 1], st, cudaEventRecordExternal));
+        c->cap_ev += 2;
+    } else if (timed) {
         PN_CUDA(c, cudaEventRecord(c->ev[c->ev_used + 1], st));
         c->ev_used += 2;
     }
@@ -297,7 +315,7 @@ int enqueue_rk4_step(pn_ctx* c, cudaStream_t st, bool timed)
     const EpiArgs a = epi_args(c, 0, nullptr);
     const int grid = c->np / kEpiStars;
     for (int stage = 0; stage < 4; ++stage) {
-        int rc = launch_pair(c, 0, st, timed);
+        int rc = launch_pair(c, 0, st, timed && (c->time_pair != 2 || stage == 0));
         if (rc) return rc;
         if (c->cross & PN_CROSS_BH)
             epilogue_kernel<MODE_RK4, kNT, 2><<<grid, kNT, 0, st>>>(a, stage);
@@ -325,6 +343,39 @@ int build_graph(pn_ctx* c, int nrep, cudaGraphExec_t* out)
     e = cudaGraphInstantiate(out, g, 0);
     cudaGraphDestroy(g);
     if (e != cudaSuccess) return fail(c, PN_ECUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e));
+    return PN_OK;
+}
+
+// One RK4 step with event-record nodes around the pair stage of each of the 4 force evaluations.
+int build_timed_graph(pn_ctx* c)
+{
+    for (int q = 0; q < 8; ++q)
+        if (!c->tev[q]) PN_CUDA(c, cudaEventCreate(&c->tev[q]));
+    PN_CUDA(c, cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+    c->cap_ev = 0;
+    int rc = enqueue_rk4_step(c, c->cap_stream, true);
+    c->cap_ev = -1;
+    cudaError_t e = cudaStreamEndCapture(c->cap_stream, &c->graphT_src);
+    if (rc != PN_OK) return rc;
+    if (e != cudaSuccess) return fail(c, PN_ECUDA, "cudaStreamEndCapture (timed graph) failed: %s", cudaGetErrorString(e));
+    size_t n = 0;
+    PN_CUDA(c, cudaGraphGetNodes(c->graphT_src, nullptr, &n));
+    std::vector<cudaGraphNode_t> nodes(n);
+    PN_CUDA(c, cudaGraphGetNodes(c->graphT_src, nodes.data(), &n));
+    int found = 0;
+    for (cudaGraphNode_t nd : nodes) {
+        cudaGraphNodeType t;
+        PN_CUDA(c, cudaGraphNodeGetType(nd, &t));
+        if (t != cudaGraphNodeTypeEventRecord) continue;
+        cudaEvent_t ev;
+        PN_CUDA(c, cudaGraphEventRecordNodeGetEvent(nd, &ev));
+        for (int q = 0; q < 8; ++q)
+            if (ev == c->tev[q]) c->tnode[q] = nd, ++found;
+    }
+    const int want = (c->time_pair == 2) ? 2 : 8;
+    if (found != want) return fail(c, PN_ECUDA, "timed graph: %d of %d event-record nodes found", found, want);
+    e = cudaGraphInstantiate(&c->graphT, c->graphT_src, 0);
+    if (e != cudaSuccess) return fail(c, PN_ECUDA, "cudaGraphInstantiate (timed graph) failed: %s", cudaGetErrorString(e));
     return PN_OK;
 }
 
@@ -490,7 +541,8 @@ int pn_set_option(pn_ctx* c, int key, int value)
             c->use_graph = value;
             return PN_OK;
         case PN_OPT_TIME_PAIR:
-            if (value != 0 && value != 1) return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_TIME_PAIR takes 0 or 1");
+            if (value < 0 || value > 2) return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_TIME_PAIR takes 0, 1 or 2");
+            if ((value == 2) != (c->time_pair == 2)) destroy_graphs(c);  // the timed graph has 8 or 2 event nodes
             c->time_pair = value;
             return PN_OK;
         case PN_OPT_PAIR_KERNEL:
@@ -625,7 +677,7 @@ int pn_step(pn_ctx* c, double dt, int64_t nsteps)
         PN_CUDA(c, cudaStreamSynchronize(c->stream));  // p lives on this stack frame
         c->dt_dev = dt;
     }
-    const bool eager = !c->use_graph || c->time_pair;
+    const bool eager = !c->use_graph;
     if (eager) {
         for (int64_t s = 0; s < nsteps; ++s)
             if (int rc = enqueue_rk4_step(c, c->stream, c->time_pair != 0)) return rc;
@@ -636,6 +688,20 @@ int pn_step(pn_ctx* c, double dt, int64_t nsteps)
         c->graph_eqm != (int)use_eqm(c)) {
         destroy_graphs(c);
         c->graph_split = c->n_split, c->graph_precision = c->precision, c->graph_sym = (int)use_sym(c), c->graph_eqm = (int)use_eqm(c);
+    }
+    if (c->time_pair) {  // one-step graph whose event-record nodes get fresh events from the pool before every launch
+        if (!c->graphT)
+            if (int rc = build_timed_graph(c)) return rc;
+        for (int64_t s = 0; s < nsteps; ++s) {
+            const int ne = (c->time_pair == 2) ? 2 : 8;
+            if (int rc = reserve_events(c, ne)) return rc;
+            for (int q = 0; q < ne; ++q)
+                PN_CUDA(c, cudaGraphExecEventRecordNodeSetEvent(c->graphT, c->tnode[q], c->ev[c->ev_used + q]));
+            PN_CUDA(c, cudaGraphLaunch(c->graphT, c->stream));
+            c->ev_used += ne;
+        }
+        c->n_launch += 4 * (1 + kernels_per_eval(c)) * nsteps;
+        return PN_OK;
     }
     int64_t left = nsteps;
     if (left >= kGraphBatch) {

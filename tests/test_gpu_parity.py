@@ -279,6 +279,30 @@ def test_step_graph_and_plain_launches_agree_bitwise():
     assert rel_err_rows(out[0][0], xr).max() <= 1e-11 and rel_err_rows(out[0][1], vr).max() <= 1e-11
 
 
+def test_timed_graph_path_matches_and_counts_pair_launches():
+    """PN_OPT_TIME_PAIR keeps pn_step on a CUDA graph (event-record nodes around each pair stage): same state bitwise,
+    4 timed launches per step, with graphs and with plain launches."""
+    from paper_1801_07986_b200 import binding
+
+    p = inputs.plummer_bh(4099, seed=23)
+    ref = None
+    for time_pair, use_graph in ((0, 1), (1, 1), (1, 0), (2, 1), (2, 0)):
+        with _pn(p) as pn:
+            pn.pn_set_option(binding.PN_OPT_USE_GRAPH, use_graph)
+            pn.pn_set_option(binding.PN_OPT_TIME_PAIR, time_pair)
+            pn.pn_set_state_host(p.pos, p.vel)
+            pn.pn_step(p.dt, 3)
+            pn.pn_step(p.dt, 2)
+            x, v = pn.pn_get_state_host()
+            ms, n = pn.pn_get_pair_time()
+        if ref is None:
+            ref = (x, v)
+            assert n == 0
+        else:
+            assert np.array_equal(x, ref[0]) and np.array_equal(v, ref[1])
+            assert n == (20 if time_pair == 1 else 5) and 0.0 < ms < 50.0
+
+
 def test_step_changes_of_dt_are_honoured():
     p = inputs.plummer_bh(300, seed=13)
     o = Oracle(p.mass, p.G, p.c, p.softening)
