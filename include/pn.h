@@ -53,9 +53,10 @@ extern "C" {
 #define PN_OPT_J_SPLIT 4        /* 0 (default): automatic; > 0: force the number of j-chunks per i-tile (tiled kernel) */
 #define PN_OPT_PAIR_KERNEL 5    /* which fp64 star-star kernel: PN_PAIR_AUTO (default) | PN_PAIR_TILED | PN_PAIR_SYMMETRIC */
 
-#define PN_OPT_EQUAL_MASS 6     /* 1 (default): when every star has the same mass (checked in pn_create) the symmetric fp64
-                                   kernel accumulates rho^-3 d on both sides and applies the common G m once per partial sum
-                                   (9 instead of 10 FP64 instructions per ordered pair); 0: always the general-mass form */
+#define PN_OPT_EQUAL_MASS 6     /* 1 (default): when every star has the same mass (checked in pn_create) the symmetric
+                                   kernels accumulate rho^-3 d on both sides and apply the common G m once per partial sum
+                                   (9 instead of 10 FP64, 10 instead of 11 FP32 instructions per ordered pair); 0: always
+                                   the general-mass form */
 
 #define PN_OPT_CROSS_TERMS 7    /* 0 (default): the hot path of north_star; PN_CROSS_STAR: add [a_i]_Cross, Eq. 2.6
                                    (PAPER.md:70-86), to every star's acceleration -- the first NEXT row of the scope table:

@@ -155,7 +155,7 @@ bool use_sym(const pn_ctx* c)
     return c->n_stars >= 3072;
 }
 
-bool use_eqm(const pn_ctx* c) { return c->equal_mass && c->eqm_opt && c->precision == PN_FP64 && use_sym(c); }
+bool use_eqm(const pn_ctx* c) { return c->equal_mass && c->eqm_opt && use_sym(c); }
 
 // kernels of the pair stage of one force evaluation (the epilogue is counted by the callers)
 int kernels_per_eval(const pn_ctx* c) { return c->cross ? 3 : (c->precision == PN_FP32_PAIR ? 2 : 1); }
@@ -187,20 +187,29 @@ cudaError_t prepare_sym()
     if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     return e;
+}
+
+template <int I, int W, int MINB, bool MASK, bool EQM>
+void launch_pair_sym32_v(pn_ctx* c, cudaStream_t st)
+{
+    const int items = c->sym_G * (c->sym_G + 1) / 2;
+    pair_sym_fp32_kernel<I, W, MINB, MASK, EQM><<<items, 32 * W, kSymSmemBytes<I, W>, st>>>(c->frec, c->part, c->np, c->sym_T, c->sym_m,
+                                                                                           (float)c->eps2, c->gm_eq);
 }
 
 template <int I, int W, int MINB>
 void launch_pair_sym32(pn_ctx* c, cudaStream_t st)
 {
-    const int items = c->sym_G * (c->sym_G + 1) / 2;
-    const float e2 = (float)c->eps2;
-    if (c->eps2 == 0.0)
-        pair_sym_fp32_kernel<I, W, MINB, true><<<items, 32 * W, kSymSmemBytes<I, W>, st>>>(c->frec, c->part, c->np, c->sym_T, c->sym_m, e2);
+    const bool mask = (c->eps2 == 0.0), eqm = use_eqm(c);
+    if (mask)
+        eqm ? launch_pair_sym32_v<I, W, MINB, true, true>(c, st) : launch_pair_sym32_v<I, W, MINB, true, false>(c, st);
     else
-        pair_sym_fp32_kernel<I, W, MINB, false><<<items, 32 * W, kSymSmemBytes<I, W>, st>>>(c->frec, c->part, c->np, c->sym_T, c->sym_m, e2);
+        eqm ? launch_pair_sym32_v<I, W, MINB, false, true>(c, st) : launch_pair_sym32_v<I, W, MINB, false, false>(c, st);
 }
 
 template <int I, int W, int MINB, bool MASK, bool EQM>
@@ -832,7 +841,7 @@ int pn_get_pair_config(pn_ctx* c, int32_t* cfg)
     if (use_sym(c)) {
         cfg[0] = 32 * c->sym_W, cfg[1] = c->sym_I, cfg[2] = c->sym_U, cfg[3] = c->sym_G;
         cfg[4] = c->sym_G * (c->sym_G + 1) / 2, cfg[5] = c->np;
-        cfg[6] = (c->precision == PN_FP32_PAIR) ? 11 : (use_eqm(c) ? 9 : 10);
+        cfg[6] = (c->precision == PN_FP32_PAIR) ? (use_eqm(c) ? 10 : 11) : (use_eqm(c) ? 9 : 10);
         cfg[7] = (c->precision == PN_FP32_PAIR) ? 3 : (use_eqm(c) ? 4 : 2);
         return PN_OK;
     }

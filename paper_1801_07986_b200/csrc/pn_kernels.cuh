@@ -710,10 +710,10 @@ __global__ void __launch_bounds__(NT) pair_fp32_kernel(const FRec* __restrict__ 
 // ---------------------------------------------------------------------------------------------------------
 // S1 variant, symmetric form: fp32 pair arithmetic on two-float positions, every unordered pair once (same
 // decomposition, rotation and slot scheme as pair_sym_fp64_kernel).  Per unordered pair: 9 FADD + 9 FFMA + 4 FMUL =
-// 22 FP32-pipe instructions + 1 MUFU.RSQ (11 per ordered pair; the tiled form needs 18).  The i-side fp32 sums run
+// 22 FP32-pipe instructions + 1 MUFU.RSQ (11 per ordered pair; the tiled form needs 18; EQM, equal masses: 20 = 10).  The i-side fp32 sums run
 // over the 32 steps of one rotation, the j-side sums over its 32 I terms; both are then added in fp64.
 // ---------------------------------------------------------------------------------------------------------
-template <int I, int W, bool SYM, bool MASK>
+template <int I, int W, bool SYM, bool MASK, bool EQM>
 __device__ __forceinline__ void sym32_unit_tile(const float4* __restrict__ shi, const float4* __restrict__ slo,
                                                 double* __restrict__ cw, const float (&xh)[I], const float (&yh)[I],
                                                 const float (&zh)[I], const float (&xl)[I], const float (&yl)[I],
@@ -741,12 +741,12 @@ __device__ __forceinline__ void sym32_unit_tile(const float4* __restrict__ shi, 
                 const float y = rsqrt_seed_f32(r2);
                 float K = (y * y) * y;
                 if (MASK) K = (jj == i_local0 + 32 * k) ? 0.f : K;
-                const float sj = K * h.w;
+                const float sj = EQM ? K : K * h.w;  // EQM: the common G m is applied at the flush
                 fx[k] = fmaf(sj, dx, fx[k]);
                 fy[k] = fmaf(sj, dy, fy[k]);
                 fz[k] = fmaf(sj, dz, fz[k]);
                 if (SYM) {
-                    const float si = K * ngi[k];
+                    const float si = EQM ? -K : K * ngi[k];
                     bx = fmaf(si, dx, bx);
                     by = fmaf(si, dy, by);
                     bz = fmaf(si, dz, bz);
@@ -769,10 +769,10 @@ __device__ __forceinline__ void sym32_unit_tile(const float4* __restrict__ shi, 
     }
 }
 
-template <int I, int W, int MINB, bool MASK>
+template <int I, int W, int MINB, bool MASK, bool EQM>
 __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp32_kernel(const FRec* __restrict__ frec,
                                                                      double* __restrict__ part, int np, int n_tiles,
-                                                                     int m, float eps2)
+                                                                     int m, float eps2, double gm_eq)
 {
     constexpr int U = W * 32 * I;
     constexpr int NT = W * 32;
@@ -788,7 +788,7 @@ __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp32_kernel(const FRec*
     const int tb0 = B * m, tb1 = min(tb0 + m, n_tiles);
     const int i_local0 = w * 32 * I + lane;
     auto flush = [&](int slot, int tile, bool first, int n_src) {
-        sym_flush<U, NT>(&cacc[0][0][0], part + (size_t)slot * 3 * np + (size_t)tile * U, np, first, n_src, tid);
+        sym_flush<U, NT>(&cacc[0][0][0], part + (size_t)slot * 3 * np + (size_t)tile * U, np, first, n_src, tid, EQM ? gm_eq : 1.0);
     };
 
     for (int ta = ta0; ta < ta1; ++ta) {
@@ -809,9 +809,9 @@ __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp32_kernel(const FRec*
             }
             sym_sync<W>();
             if (ta == tb) {
-                sym32_unit_tile<I, W, false, MASK>(shi, slo, &cacc[w][0][0], xh, yh, zh, xl, yl, zl, ngi, ax, ay, az, eps2, lane, i_local0);
+                sym32_unit_tile<I, W, false, MASK, EQM>(shi, slo, &cacc[w][0][0], xh, yh, zh, xl, yl, zl, ngi, ax, ay, az, eps2, lane, i_local0);
             } else {
-                sym32_unit_tile<I, W, true, false>(shi, slo, &cacc[w][0][0], xh, yh, zh, xl, yl, zl, ngi, ax, ay, az, eps2, lane, i_local0);
+                sym32_unit_tile<I, W, true, false, EQM>(shi, slo, &cacc[w][0][0], xh, yh, zh, xl, yl, zl, ngi, ax, ay, az, eps2, lane, i_local0);
                 sym_sync<W>();
                 flush(A, tb, ta == ta0, W);
             }

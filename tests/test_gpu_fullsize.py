@@ -28,7 +28,7 @@ def _sample_rows(p, n, seed=4242):
     return np.unique(np.concatenate([rows, [e for e in extra if e < p.N]])).astype(np.int64)
 
 
-def _check_sampled(p, n_rows, precision=None, tol=TOL_ACC, kernel=None):
+def _check_sampled(p, n_rows, precision=None, tol=TOL_ACC, kernel=None, equal_mass_form=None):
     from paper_1801_07986_b200 import PN, binding
 
     rows = _sample_rows(p, n_rows)
@@ -38,6 +38,8 @@ def _check_sampled(p, n_rows, precision=None, tol=TOL_ACC, kernel=None):
             pn.pn_set_option(binding.PN_OPT_PAIR_PRECISION, precision)
         if kernel is not None:
             pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, kernel)
+        if equal_mass_form is not None:
+            pn.pn_set_option(binding.PN_OPT_EQUAL_MASS, equal_mass_form)
         acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
         cfg = pn.pn_get_pair_config()
     assert np.isfinite(acc).all()
@@ -130,18 +132,19 @@ def test_config3_energy_full_size():
 
 
 # ------------------------------------------------------------------ fp32-pair / fp64-accumulate variant
-@pytest.mark.parametrize("kernel", ["tiled", "symmetric"])
+@pytest.mark.parametrize("kernel", ["tiled", "symmetric", "symmetric_general"])
 @pytest.mark.parametrize("n_stars", [2, 129, 1023, 4099, 13001])
 def test_fp32_pair_variant_parity(n_stars, kernel):
     from paper_1801_07986_b200 import binding
 
+    eqm = 0 if kernel == "symmetric_general" else None  # equal-mass stars otherwise take the equal-mass form
     kernel = binding.PN_PAIR_TILED if kernel == "tiled" else binding.PN_PAIR_SYMMETRIC
 
     if n_stars == 2:  # two equal-mass recentred stars make a_1 pure rounding noise: use unequal masses instead
         p = inputs.random_small(2, seed=302, M=1.0, m_scale=1e-2, c=10.0, softening=1e-3)
     else:
         p = inputs.plummer_bh(n_stars, seed=300 + n_stars)
-    _check_sampled(p, 4096, precision=binding.PN_FP32_PAIR, tol=TOL_FP32, kernel=kernel)
+    _check_sampled(p, 4096, precision=binding.PN_FP32_PAIR, tol=TOL_FP32, kernel=kernel, equal_mass_form=eqm)
 
 
 def test_fp32_pair_variant_cusp_and_zero_softening():

@@ -464,3 +464,31 @@ def test_momentum_newtonian_limit_and_softening(kind):
     v2[0] = 0.0  # the (1/2c^2) M v_1^2 v_1 term is dropped (O(m^3))
     P = P_newton + (p.mass * v2 / (2 * p.c**2))[:, None].__mul__(p.vel).sum(0) - pair.sum((0, 1)) / (2 * p.c**2)
     assert Oracle(p.mass, p.G, p.c, p.softening, kind=kind).momentum(p.pos, p.vel) == pytest.approx(P, rel=1e-12, abs=1e-16)
+
+
+def test_cross_terms_two_body_finite_mass_energy_conservation():
+    """Two bodies, m/M = 0.01 and 0.03, e = 0.5, c = 100: along the flow with both Cross rows the energy of Eq. 2.7 only
+    shows the c^-4 excursion of the test-particle case (2.0e-6, independent of the mass ratio); along the hot path alone
+    it moves by O(m/M) of that scale (2.9e-5, 9.1e-5).  Pins the self lines of Eqs. 2.3 and 2.6 against Eq. 2.7."""
+    from oracle.pn_oracle import CROSS_BH, CROSS_STAR
+
+    a, e, c, M = 1.0, 0.5, 100.0, 1.0
+    out = {}
+    for m in (1e-2, 3e-2):
+        mu = M + m
+        rp, vp = a * (1 - e), math.sqrt(mu * (1 + e) / (a * (1 - e)))
+        mass = np.array([M, m])
+        pos = np.array([[-rp * m / mu, 0, 0], [rp * M / mu, 0, 0]])
+        vel = np.array([[0, -vp * m / mu, 0], [0, vp * M / mu, 0]])
+        dt = 2 * math.pi / math.sqrt(mu) / 2000
+        for terms in (0, CROSS_STAR | CROSS_BH):
+            o = Oracle(mass, 1.0, c, 0.0, terms=terms)
+            e0, x, v, worst = o.energy(pos, vel), pos, vel, 0.0
+            for _ in range(40):
+                x, v = o.step(x, v, dt, 50)
+                worst = max(worst, abs(o.energy(x, v) - e0) / abs(e0))
+            out[(m, terms)] = worst
+    for m in (1e-2, 3e-2):
+        assert out[(m, 3)] == pytest.approx(2.0e-6, rel=0.25)
+        assert out[(m, 0)] > 10 * out[(m, 3)]
+    assert out[(3e-2, 0)] / out[(1e-2, 0)] == pytest.approx(3.0, rel=0.15)
