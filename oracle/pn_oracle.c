@@ -34,8 +34,11 @@
  * limit c=inf against an independent numpy evaluation, Newton's third law, full N-body EIH
  * (Einstein-Infeld-Hoffmann) residual scaling in mpmath, test-particle periastron advance
  * 6 pi G M / (c^2 a (1-e^2)), RK4 4th-order convergence, 1PN two-body energy conservation.
- * Parity unpinned: the softening convention inside the 1PN star-star energy bracket
- * (n_ij -> x_ij / rho_ij, reading R9) -- exact at eps = 0, a convention otherwise.
+ * NEXT rows (Cross terms, Eqs. 2.3 and 2.6; momentum, Eq. 2.8): residual orders lam^3 / lam^2 / lam^3 against the full
+ * EIH acceleration and momentum, hand values for two bodies, bit-identity with the hot path at c = inf and for massless
+ * stars, two-body finite-mass periastron advance 6 pi G (M + m) / (c^2 a (1 - e^2)) and energy conservation.
+ * Parity unpinned: the softening convention inside the 1PN star-star energy bracket, the Cross terms and the
+ * momentum (every star-star r_ij -> rho_ij, n_ij -> x_ij / rho_ij, reading R9) -- exact at eps = 0, a convention otherwise.
  */
 #include <math.h>
 #include <stdint.h>

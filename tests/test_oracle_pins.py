@@ -492,3 +492,27 @@ def test_cross_terms_two_body_finite_mass_energy_conservation():
         assert out[(m, 3)] == pytest.approx(2.0e-6, rel=0.25)
         assert out[(m, 0)] > 10 * out[(m, 3)]
     assert out[(3e-2, 0)] / out[(1e-2, 0)] == pytest.approx(3.0, rel=0.15)
+
+
+def test_cross_terms_hand_values_two_bodies():
+    """By hand, G = 1, c = 10, M = 1 at the origin at rest, one star m = 1e-3 at x = (1, 0, 0) with v = (0, 1, 0)
+    (the first golden case, whose hot-path values are a_star = (-0.97, 0, 0), a_1 = (9.7e-4, 0, 0)).
+    Eq. 2.6 with one star is its first line only: 5 G^2 m M x_i1 / r^4 - (G m / r^3)[4 v^2 x_i1 - 7 (v.x_i1) v]
+      = 5e-3 (1,0,0) - 1e-3 [4 (1,0,0) - 0] = (1e-3, 0, 0);  a_star += 1e-3 / c^2 = 1e-5.
+    Eq. 2.3 with one star: 4 G^2 m^2 x_1j / r^4 = 4e-6 (-1,0,0); the (j,k) sums with r_jk are empty; the velocity sum has
+    the single term k = j: -(G m^2 / (M r^3)) [4 v^2 x_1j - 3 (v.x_1j) v - 4 (v.x_1j) v] = -1e-6 [4 (-1,0,0)] = (4e-6,0,0):
+    the two cancel, a_1 is unchanged."""
+    from oracle.pn_oracle import CROSS_BH, CROSS_STAR
+
+    mass = np.array([1.0, 1e-3])
+    pos = np.array([[0.0, 0, 0], [1.0, 0, 0]])
+    vel = np.array([[0.0, 0, 0], [0.0, 1.0, 0]])
+    a = Oracle(mass, 1.0, 10.0, 0.0, terms=CROSS_STAR | CROSS_BH).accel(pos, vel)
+    np.testing.assert_allclose(a[1], [-0.97 + 1e-5, 0.0, 0.0], rtol=1e-15, atol=1e-18)
+    np.testing.assert_allclose(a[0], [9.7e-4, 0.0, 0.0], rtol=1e-13, atol=1e-18)
+    # second star velocity along x: v = (0.5, 0, 0): L0 = 5e-3 (1,0,0) - 1e-3 [4 * 0.25 (1,0,0) - 7 * 0.5 * (0.5,0,0)]
+    #   = (5e-3 - 1e-3 + 1.75e-3, 0, 0) = (5.75e-3, 0, 0)
+    vel[1] = [0.5, 0.0, 0.0]
+    hot = Oracle(mass, 1.0, 10.0, 0.0).accel(pos, vel)
+    a = Oracle(mass, 1.0, 10.0, 0.0, terms=CROSS_STAR).accel(pos, vel)
+    np.testing.assert_allclose(a[1] - hot[1], [5.75e-5, 0.0, 0.0], rtol=1e-12, atol=1e-18)
