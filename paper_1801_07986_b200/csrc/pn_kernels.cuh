@@ -1,12 +1,24 @@
 // pn_kernels.cuh -- sm_100a kernels of the limited-1PN hot path (arXiv:1801.07986).
 // Product code: shares nothing with oracle/.  Citations: /root/reference/PAPER.md:<line>.
 //
+// Kernels, in the order of this file (DESIGN.md section 6 has the roofline of each):
+//   S1  pair_fp64_kernel          star-star Newtonian, every ordered pair, tiled (N_s < 3072, PN_PAIR_TILED)
+//       pair_sym_fp64_kernel      the same, every unordered pair once (Newton's third law), general / equal-mass form
+//       pair_cross_fp64_kernel    NEXT-1/2: S1 + the O(N^2) sums of the Cross terms, Eqs. 2.6 and 2.3 (cross_prep/sum: O(N))
+//       pair_fp32_kernel, pair_sym_fp32_kernel   fp32-pair / fp64-accumulate variant (split_kernel: two-float records)
+//   S2-S4  epilogue_kernel        partial-sum reduction, BH <-> star Newtonian + 1PN, a_1 reduction, fused RK4 stage update
+//   S5  energy_prep / energy_pair / energy_final   Eq. 2.7, compensated
+//   NEXT-3  momentum_prep / momentum_pair / momentum_final   Eq. 2.8, compensated
+//   pack / unpack (AoS <-> internal layout), fp64_peak_kernel (DFMA-chain probe)
+//
 // Internal data layout (all fp64, star index s = body index - 1, padded to NP):
 //   JRec  jrec[NP]      : stage position + mass constants of star s, 48 B, 16 B aligned.  This is the record the
-//                         O(N^2) pair kernel streams through shared memory; pad records have gm = 0, x = 1e100.
+//                         O(N^2) pair kernels read; pad records have gm = 0, x = 1e100.
 //   double v[3][NP]     : stage velocity, SoA
 //   double x0/v0[3][NP] : state at the beginning of the RK4 step;  double sx/sv[3][NP] : weighted sum of k's
-//   double part[S][3][NP]: per-j-chunk partial star-star accelerations (deterministic fixed-order reduction)
+//   double part[S][3][NP]: partial star-star accelerations, one slot per j-chunk (tiled) or j-group (symmetric), each entry
+//                         written by exactly one block; summed in fixed order by the epilogue (6 or 7 components per slot
+//                         in Cross mode)
 //   BhState             : the massive object's stage state, step state, k-sums (a handful of doubles)
 #pragma once
 #include <cuda_runtime.h>
