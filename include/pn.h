@@ -65,7 +65,8 @@ extern "C" {
                                    the epilogue.  PN_CROSS_STAR | PN_CROSS_BH: also [a_1]_Cross, Eq. 2.3, the
                                    second NEXT row -- the paper's full limited-1PN force (one more O(N^2) sum per star in the
                                    same kernel, 59 instructions per pair; the rest is O(N)).  Applies to pn_accel and
-                                   pn_step; pn_energy is Eq. 2.7 either way. */
+                                   pn_step; pn_energy is Eq. 2.7 either way.  The Cross path is fp64 only: while it is on,
+                                   PN_OPT_PAIR_PRECISION, PN_OPT_PAIR_KERNEL and PN_OPT_EQUAL_MASS have no effect. */
 #define PN_CROSS_STAR 1
 #define PN_CROSS_BH 2
 

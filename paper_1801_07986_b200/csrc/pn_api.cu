@@ -562,7 +562,9 @@ int pn_set_option(pn_ctx* c, int key, int value)
         case PN_OPT_CROSS_TERMS: {
             if (value != 0 && value != PN_CROSS_STAR && value != (PN_CROSS_STAR | PN_CROSS_BH))
                 return fail(c, PN_EINVAL, "pn_set_option: PN_OPT_CROSS_TERMS takes 0, PN_CROSS_STAR or PN_CROSS_STAR | PN_CROSS_BH");
-            if (value && !c->crec) {  // buffers of the cross path, on first use
+            if (value && !c->part6) {  // buffers of the cross path, on first use (part6 is allocated last)
+                cudaFree(c->crec), cudaFree(c->cblk), cudaFree(c->csum);  // left over from a failed earlier attempt
+                c->crec = nullptr, c->cblk = nullptr, c->csum = nullptr;
                 const size_t np = c->np;
                 const int n_it = c->np / (kCrossI * kNT), n_t = c->np / kCrossTJ;
                 int s = std::max(1, std::min(std::min((kSMs * 16 + n_it - 1) / n_it, n_t), 64));
