@@ -41,7 +41,8 @@ PAIR_KERNELS = {0: ("pair_fp64_kernel", 15, 24.0), 2: ("pair_sym_fp64_kernel", 1
 SMS, FP64_LANES_PER_SM = 148, 64
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu --set full
 # captures (profiles/), keyed by (variant, N_s); null when no capture exists for the workload
-NCU_DRAM_BYTES_PER_PAIR_LAUNCH = {(0, 16383): 793344, (2, 16383): 800000 + 943872, (4, 16383): 805120 + 237312}
+NCU_DRAM_BYTES_PER_PAIR_LAUNCH = {(0, 16383): 793344, (2, 16383): 800000 + 943872, (4, 16383): 805120 + 237312,
+                                  (4, 65535): 3248640 + 142522368}
 
 
 def load_peaks() -> dict:
