@@ -485,7 +485,9 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA(dalloc(&ctx->frec, np));
     {
         const int n_it = (int)(np / kNT);
-        int s = (kSMs * 8 + n_it / 2 - 1) / (n_it / 2);  // the energy pair kernel runs n_it / 2 mirrored i-tile pairs per j-split
+        // the energy pair kernel runs n_it / 2 mirrored i-tile pairs per j-split, all of equal work: aim at one full wave
+        // (7 blocks of 72 registers x 128 threads per SM) rather than a full wave plus a short one
+        int s = (kSMs * 7) / (n_it / 2);
         s = std::max(1, std::min(s, std::min(ctx->n_tiles, 64)));
         ctx->e_tiles_per_split = (ctx->n_tiles + s - 1) / s;
         ctx->e_split = (ctx->n_tiles + ctx->e_tiles_per_split - 1) / ctx->e_tiles_per_split;
