@@ -300,7 +300,7 @@ __device__ __forceinline__ void sym_unit_tile(const double2* __restrict__ sxy, c
 #pragma unroll 1
     for (int jb = 0; jb < U; jb += 32) {
         double bx = 0.0, by = 0.0, bz = 0.0;
-        constexpr int kUnr = 16 / I;  // 16 independent pairs in flight per warp (8: -3 %, measured)
+        constexpr int kUnr = 32 / I;  // rotation steps unrolled: 32 independent pairs per trip (16: -1 %, 8: -4 %, 128: -9 %, measured)
 #pragma unroll kUnr
         for (int r = 0; r < 32; ++r) {
             const int jj = jb + ((lane + r) & 31);
