@@ -212,9 +212,23 @@ def cpu_baseline(p, target_s=12.0, max_steps=200, terms=0) -> dict:
         pairs += oracle_step_sample(p, o, rows)
         n += 1
     dt = time.perf_counter() - t0
-    return {"value": pairs / dt, "unit": "pair-interactions/s", "cores": o.max_threads, "kind": "oracle",
-            "build": "oracle/pn_oracle.c -DORACLE_FAST (double, -O3 -march=native, OpenMP over i)",
-            "sample": f"{n} x {what}; {dt:.1f} s", "steps_per_s": (n / dt) if rows is None else None}
+    out = {"value": pairs / dt, "unit": "pair-interactions/s", "cores": o.max_threads, "kind": "oracle",
+           "build": "oracle/pn_oracle.c -DORACLE_FAST (double, -O3 -march=native, OpenMP over i)",
+           "sample": f"{n} x {what}; {dt:.1f} s", "steps_per_s": (n / dt) if rows is None else None}
+    # the like-for-like counterpart of the paper's single-core CPU column (Table 3.2): the same oracle on
+    # ONE thread, on a seeded subset of i-rows (rows are independent), about 5 s
+    n_all = o.max_threads
+    o1 = Oracle(p.mass, p.G, p.c, p.softening, kind="fast", terms=terms, threads=1)
+    rows1, _ = oracle_rows(p, budget_pairs=6.0e8 / (8.0 if terms else 1.0))
+    if rows1 is None:
+        rows1 = np.arange(1, p.N)
+    t0 = time.perf_counter()
+    pairs1 = oracle_step_sample(p, o1, rows1)
+    dt1 = time.perf_counter() - t0
+    o1.lib.oracle_set_threads(n_all)
+    out["one_core"] = {"value": pairs1 / dt1, "unit": "pair-interactions/s", "cores": 1,
+                       "sample": f"4 force evaluations on a seeded subset of {len(rows1)} of {p.n_stars} i-rows; {dt1:.1f} s"}
+    return out
 
 
 def run_reference(args) -> None:

@@ -739,7 +739,7 @@ __device__ __forceinline__ void sym32_unit_tile(const float4* __restrict__ shi, 
 #pragma unroll
         for (int k = 0; k < I; ++k) fx[k] = fy[k] = fz[k] = 0.f;
         float bx = 0.f, by = 0.f, bz = 0.f;
-        constexpr int kUnr = (I >= 4) ? 4 : 16 / I;
+        constexpr int kUnr = 16 / I;  // (32: no consistent gain in fp32, measured)
 #pragma unroll kUnr
         for (int r = 0; r < 32; ++r) {
             const int jj = jb + ((lane + r) & 31);

@@ -516,3 +516,34 @@ def test_cross_terms_hand_values_two_bodies():
     hot = Oracle(mass, 1.0, 10.0, 0.0).accel(pos, vel)
     a = Oracle(mass, 1.0, 10.0, 0.0, terms=CROSS_STAR).accel(pos, vel)
     np.testing.assert_allclose(a[1] - hot[1], [5.75e-5, 0.0, 0.0], rtol=1e-12, atol=1e-18)
+
+
+# ------------------------------------------------------------------ symmetries every term must respect
+def _rotation(seed):
+    rng = np.random.default_rng(seed)
+    q, r = np.linalg.qr(rng.standard_normal((3, 3)))
+    q *= np.sign(np.diag(r))
+    if np.linalg.det(q) < 0:
+        q[:, 0] = -q[:, 0]
+    return q
+
+
+@pytest.mark.parametrize("terms", [0, 1, 3])
+def test_rotation_covariance_translation_invariance_and_velocity_parity(terms):
+    """a(R x + t, R v) = R a(x, v) for a proper rotation R and a shift t; E is invariant, P rotates; every velocity term of
+    the limited equations is even in the velocities, so a(x, -v) = a(x, v), E(x, -v) = E(x, v), P(x, -v) = -P(x, v).
+    A transposed component, a stray index or an odd velocity power in any line breaks one of these."""
+    p = inputs.random_small(9, seed=77, M=1.0, m_scale=2e-2, c=5.0, softening=0.03, bh_moving=True)
+    R, t = _rotation(5), np.array([0.3, -1.1, 0.7])
+    o = Oracle(p.mass, p.G, p.c, p.softening, terms=terms)
+    a = o.accel(p.pos, p.vel)
+    xr, vr = p.pos @ R.T + t, p.vel @ R.T
+    np.testing.assert_allclose(o.accel(xr, vr), a @ R.T, rtol=0, atol=2e-13 * np.abs(a).max())
+    assert o.energy(xr, vr) == pytest.approx(o.energy(p.pos, p.vel), rel=1e-13)
+    np.testing.assert_allclose(o.momentum(xr, vr), R @ o.momentum(p.pos, p.vel), rtol=0, atol=1e-15)
+    np.testing.assert_allclose(o.accel(p.pos, -p.vel), a, rtol=0, atol=1e-15 * np.abs(a).max())
+    assert o.energy(p.pos, -p.vel) == pytest.approx(o.energy(p.pos, p.vel), rel=1e-15)
+    np.testing.assert_allclose(o.momentum(p.pos, -p.vel), -o.momentum(p.pos, p.vel), rtol=0, atol=1e-18)
+    # the 1PN terms are really exercised: they change the accelerations at the percent level here
+    aN = Oracle(p.mass, p.G, math.inf, p.softening).accel(p.pos, p.vel)
+    assert np.abs(a - aN).max() > 1e-3 * np.abs(a).max()
