@@ -63,7 +63,7 @@ struct pn_ctx {
     ERec* erec = nullptr;
     FRec* frec = nullptr;  // two-float records of the fp32-pair variant, rebuilt before every pair launch
     double *blk_prep = nullptr, *blk_pair = nullptr, *d_energy = nullptr;
-    int e_split = 1, e_tiles_per_split = 0;
+    int e_split = 1;
 
     bool have_state = false;
     double dt_dev = NAN;
@@ -489,8 +489,7 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
         // (7 blocks of 72 registers x 128 threads per SM) rather than a full wave plus a short one
         int s = (kSMs * 7) / (n_it / 2);
         s = std::max(1, std::min(s, std::min(ctx->n_tiles, 64)));
-        ctx->e_tiles_per_split = (ctx->n_tiles + s - 1) / s;
-        ctx->e_split = (ctx->n_tiles + ctx->e_tiles_per_split - 1) / ctx->e_tiles_per_split;
+        ctx->e_split = s;  // each i-tile splits its own range of j-tiles into e_split chunks inside the kernel
         CREATE_CUDA(dalloc(&ctx->blk_prep, 4 * (size_t)n_it));
         CREATE_CUDA(dalloc(&ctx->blk_pair, 2 * (size_t)n_it * ctx->e_split));
         CREATE_CUDA(dalloc(&ctx->d_energy, 1));
