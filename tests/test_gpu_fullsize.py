@@ -134,19 +134,6 @@ def test_config2_energy_and_short_run_drift():
     assert abs((e1 - e0) / abs(e0) - (e1_ref - e0_ref) / abs(e0_ref)) <= 1e-10
 
 
-def test_config3_energy_full_size():
-    """Config 3 (4.3e9 ordered pairs): energy against the oracle's double build (same source, -DORACLE_FAST;
-    the long-double build would take minutes)."""
-    from paper_1801_07986_b200 import PN
-
-    p = inputs.config(3)
-    ref = Oracle(p.mass, p.G, p.c, p.softening, kind="fast").energy(p.pos, p.vel)
-    with PN(p.mass, p.G, p.c, p.softening) as pn:
-        pn.pn_set_state_host(p.pos, p.vel)
-        e = pn.pn_energy()
-    assert e == pytest.approx(ref, rel=1e-12)
-
-
 # ------------------------------------------------------------------ fp32-pair / fp64-accumulate variant
 @pytest.mark.parametrize("kernel", ["tiled", "symmetric", "symmetric_general"])
 @pytest.mark.parametrize("n_stars", [2, 129, 1023, 4099, 13001])
