@@ -48,7 +48,7 @@ struct pn_ctx {
     // pair-kernel launch configuration
     int ipt = 1, n_itiles = 0, n_tiles = 0, n_split = 1, tiles_per_split = 0, max_split = 1;
     // symmetric pair kernel: unit tile U = 32 W I stars, T unit tiles in G groups of m
-    int sym_I = 0, sym_W = 0, sym_U = 0, sym_T = 0, sym_m = 0, sym_G = 0;
+    int sym_kind = 0, sym_I = 0, sym_W = 0, sym_U = 0, sym_T = 0, sym_m = 0, sym_G = 0;
 
     // device buffers.  Two stage sets: [0] integrator state, [1] scratch for pn_accel.
     JRec* jrec[2] = {nullptr, nullptr};
@@ -128,17 +128,25 @@ void choose_split(pn_ctx* c)
 
 constexpr int kSymMaxGroups = 128;  // partial-sum slots of the symmetric kernel (tail granularity vs epilogue traffic)
 
-// Symmetric (Newton's third law) kernel variants, by problem size: smaller unit tiles give enough blocks and a
-// fine-grained tail at small N, larger ones amortise the tile prologue at large N (pair kernel).
+// Symmetric (Newton's third law) kernel variants, by problem size (measured on a B200, profiles/r2_ncu_summary.md): the
+// j-split form (4 warps share one 128 x 128 unit-tile pair: work items a quarter as long) where the grid is small,
+// one-warp blocks around N_s = 16384, 512-star unit tiles (4 warps, 128 i-stars each) from 40000 stars on, where the
+// tile prologue and flush weigh least.
+enum { SYM_W1_U128 = 0, SYM_JS_U128 = 1, SYM_W4_U512 = 2 };
+
 void choose_sym(pn_ctx* c)
 {
     if (c->n_stars < 12288)
-        c->sym_I = 2, c->sym_W = 1;
-    else if (c->n_stars < 49152)
-        c->sym_I = 4, c->sym_W = 1;
+        c->sym_kind = SYM_JS_U128;
+    else if (c->n_stars < 20000)
+        c->sym_kind = SYM_W1_U128;
+    else if (c->n_stars < 40000)
+        c->sym_kind = SYM_JS_U128;
     else
-        c->sym_I = 4, c->sym_W = 4;
-    c->sym_U = 32 * c->sym_W * c->sym_I;
+        c->sym_kind = SYM_W4_U512;
+    c->sym_I = 4;
+    c->sym_W = (c->sym_kind == SYM_W1_U128) ? 1 : 4;
+    c->sym_U = (c->sym_kind == SYM_W4_U512) ? 512 : 128;
 }
 
 void choose_sym_groups(pn_ctx* c)
@@ -179,15 +187,22 @@ void launch_pair_fp64(pn_ctx* c, int set, cudaStream_t st)
 }
 
 // symmetric kernels <I, W, MINB>: one block per work item (group pair), W warps
-template <int I, int W, int MINB>
+template <int I, int W, int MINB, bool JS>
 cudaError_t prepare_sym()
 {
+    const int bytes = kSymSmemBytes<I, W, JS>;
+    cudaError_t e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, false, false, JS>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, true, false, JS>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, false, true, JS>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, true, true, JS>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    return e;
+}
+
+template <int I, int W, int MINB>
+cudaError_t prepare_sym32()
+{
     const int bytes = kSymSmemBytes<I, W>;
-    cudaError_t e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp64_kernel<I, W, MINB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    cudaError_t e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
@@ -212,22 +227,22 @@ void launch_pair_sym32(pn_ctx* c, cudaStream_t st)
         eqm ? launch_pair_sym32_v<I, W, MINB, false, true>(c, st) : launch_pair_sym32_v<I, W, MINB, false, false>(c, st);
 }
 
-template <int I, int W, int MINB, bool MASK, bool EQM>
+template <int I, int W, int MINB, bool JS, bool MASK, bool EQM>
 void launch_pair_sym_v(pn_ctx* c, int set, cudaStream_t st)
 {
     const int items = c->sym_G * (c->sym_G + 1) / 2;
-    pair_sym_fp64_kernel<I, W, MINB, MASK, EQM><<<items, 32 * W, kSymSmemBytes<I, W>, st>>>(c->jrec[set], c->part, c->np, c->sym_T,
-                                                                                           c->sym_m, c->eps2, c->gm_eq);
+    pair_sym_fp64_kernel<I, W, MINB, MASK, EQM, JS><<<items, 32 * W, kSymSmemBytes<I, W, JS>, st>>>(c->jrec[set], c->part, c->np, c->sym_T,
+                                                                                                   c->sym_m, c->eps2, c->gm_eq);
 }
 
-template <int I, int W, int MINB>
+template <int I, int W, int MINB, bool JS>
 void launch_pair_sym(pn_ctx* c, int set, cudaStream_t st)
 {
     const bool mask = (c->eps2 == 0.0), eqm = use_eqm(c);
     if (mask)
-        eqm ? launch_pair_sym_v<I, W, MINB, true, true>(c, set, st) : launch_pair_sym_v<I, W, MINB, true, false>(c, set, st);
+        eqm ? launch_pair_sym_v<I, W, MINB, JS, true, true>(c, set, st) : launch_pair_sym_v<I, W, MINB, JS, true, false>(c, set, st);
     else
-        eqm ? launch_pair_sym_v<I, W, MINB, false, true>(c, set, st) : launch_pair_sym_v<I, W, MINB, false, false>(c, set, st);
+        eqm ? launch_pair_sym_v<I, W, MINB, JS, false, true>(c, set, st) : launch_pair_sym_v<I, W, MINB, JS, false, false>(c, set, st);
 }
 
 int reserve_events(pn_ctx* c, size_t n)
@@ -266,9 +281,7 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
         dim3 grid(c->n_itiles, c->n_split);
         const float e2 = (float)c->eps2;
         if (use_sym(c)) {
-            if (c->sym_I == 2)
-                launch_pair_sym32<2, 1, 16>(c, st);
-            else if (c->sym_W == 1)
+            if (c->sym_U == 128)
                 launch_pair_sym32<4, 1, 8>(c, st);
             else
                 launch_pair_sym32<4, 4, 3>(c, st);
@@ -279,12 +292,12 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
             mask ? pair_fp32_kernel<1, kNT, kTJ, 32, true><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2)
                  : pair_fp32_kernel<1, kNT, kTJ, 32, false><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2);
     } else if (use_sym(c)) {
-        if (c->sym_I == 2)
-            launch_pair_sym<2, 1, 16>(c, set, st);
-        else if (c->sym_W == 1)
-            launch_pair_sym<4, 1, 8>(c, set, st);
+        if (c->sym_kind == SYM_JS_U128)
+            launch_pair_sym<4, 4, 3, true>(c, set, st);
+        else if (c->sym_kind == SYM_W1_U128)
+            launch_pair_sym<4, 1, 12, false>(c, set, st);
         else
-            launch_pair_sym<4, 4, 2>(c, set, st);
+            launch_pair_sym<4, 4, 2, false>(c, set, st);
     } else if (c->ipt == 2)
         mask ? launch_pair_fp64<2, 4, 4, true>(c, set, st) : launch_pair_fp64<2, 4, 4, false>(c, set, st);
     else
@@ -469,10 +482,11 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA(dalloc(&ctx->v0, 3 * np));
     CREATE_CUDA(dalloc(&ctx->sx, 3 * np));
     CREATE_CUDA(dalloc(&ctx->sv, 3 * np));
-    CREATE_CUDA((prepare_sym<2, 1, 16>()));
-    CREATE_CUDA((prepare_sym<4, 1, 8>()));
-    CREATE_CUDA((prepare_sym<4, 4, 2>()));
-    CREATE_CUDA((prepare_sym<4, 4, 3>()));
+    CREATE_CUDA((prepare_sym<4, 1, 12, false>()));
+    CREATE_CUDA((prepare_sym<4, 4, 3, true>()));
+    CREATE_CUDA((prepare_sym<4, 4, 2, false>()));
+    CREATE_CUDA((prepare_sym32<4, 1, 8>()));
+    CREATE_CUDA((prepare_sym32<4, 4, 3>()));
     CREATE_CUDA(dalloc(&ctx->part, (size_t)std::max(ctx->max_split, ctx->sym_G) * 3 * np));
     CREATE_CUDA(dalloc(&ctx->bh_part, 3 * (np / kEpiStars)));
     CREATE_CUDA(dalloc(&ctx->ticket, 1));
@@ -842,7 +856,7 @@ int pn_get_pair_config(pn_ctx* c, int32_t* cfg)
         return PN_OK;
     }
     if (use_sym(c)) {
-        cfg[0] = 32 * c->sym_W, cfg[1] = c->sym_I, cfg[2] = c->sym_U, cfg[3] = c->sym_G;
+        cfg[0] = (c->precision == PN_FP32_PAIR && c->sym_U == 128) ? 32 : 32 * c->sym_W, cfg[1] = c->sym_I, cfg[2] = c->sym_U, cfg[3] = c->sym_G;
         cfg[4] = c->sym_G * (c->sym_G + 1) / 2, cfg[5] = c->np;
         cfg[6] = (c->precision == PN_FP32_PAIR) ? (use_eqm(c) ? 10 : 11) : (use_eqm(c) ? 9 : 10);
         cfg[7] = (c->precision == PN_FP32_PAIR) ? 3 : (use_eqm(c) ? 4 : 2);

@@ -252,6 +252,7 @@ __device__ __forceinline__ void sym_step(const double2 xy, const double2 zm, con
         t[k] = t[k] * p[k];              // K = rho^-3
         if (MASK) t[k] = (k == self_k) ? 0.0 : t[k];
     }
+
     if (EQM) {  // all stars have the same mass: accumulate K d on both sides, the common G m is applied at the flush
 #pragma unroll
         for (int k = 0; k < I; ++k) {
@@ -289,18 +290,17 @@ __device__ __forceinline__ void sym_step(const double2 xy, const double2 zm, con
     }
 }
 
-template <int I, int W, bool SYM, bool MASK, bool EQM>
+template <int I, int U, bool SYM, bool MASK, bool EQM, int UNR = 32 / I>
 __device__ __forceinline__ void sym_unit_tile(const double2* __restrict__ sxy, const double2* __restrict__ szm,
-                                              double* __restrict__ cw /* this warp's [3][U] column sums */,
+                                              double* __restrict__ cw /* [3][U] column sums this warp writes into */,
                                               const double (&xi)[I], const double (&yi)[I], const double (&zi)[I],
                                               const double (&ngi)[I], double (&ax)[I], double (&ay)[I],
-                                              double (&az)[I], double eps2, int lane, int i_local0)
+                                              double (&az)[I], double eps2, int lane, int i_local0, int jb0, int jb1)
 {
-    constexpr int U = W * 32 * I;
 #pragma unroll 1
-    for (int jb = 0; jb < U; jb += 32) {
+    for (int jb = jb0; jb < jb1; jb += 32) {
         double bx = 0.0, by = 0.0, bz = 0.0;
-        constexpr int kUnr = 32 / I;  // rotation steps unrolled: 32 independent pairs per trip (16: -1 %, 8: -4 %, 128: -9 %, measured)
+        constexpr int kUnr = UNR;  // rotation steps unrolled: 32 independent pairs per trip (16: -1 %, 8: -4 %, 128: -9 %, measured)
 #pragma unroll kUnr
         for (int r = 0; r < 32; ++r) {
             const int jj = jb + ((lane + r) & 31);
@@ -360,31 +360,44 @@ __device__ __forceinline__ void sym_flush(const double* __restrict__ cacc, doubl
     }
 }
 
-template <int I, int W>
-constexpr int kSymSmemBytes = (W * 32 * I) * (2 * 16 + W * 3 * 8);
+// unit tile of the symmetric kernels: W warps of I i-stars per lane each (JS = false), or -- j-split form, JS = true,
+// W == I -- I i-stars per lane held by EVERY warp, warp w sweeping rotation group w of the j tile
+template <int I, int W, bool JS>
+constexpr int kSymU = JS ? 32 * I : W * 32 * I;
+
+template <int I, int W, bool JS = false>
+constexpr int kSymSmemBytes = kSymU<I, W, JS> * (2 * 16 + W * 3 * 8);
 
 // EQM: every star has the same mass (true of every BASELINE.json config and of the paper's own model):
 // both sides accumulate K d and the common G m = gm_eq multiplies the sums once, at the flush: 18 instead of 20 FP64
 // instructions per unordered pair.
-template <int I, int W, int MINB, bool MASK, bool EQM>
+// JS (j-split form, W == I warps, U = 32 I): all warps of the block hold the SAME I i-stars per lane and each sweeps one
+// rotation group (32 j-stars) of the j tile, so a unit-tile pair costs a quarter (1 / W) of the time it costs a one-warp
+// block of the same U while the partial-sum slots stay those of U = 32 I: W times more, W times shorter work items for
+// the same slot layout -- this is what shortens the launch tail at N_s ~ 10^4.  The column sums
+// of a warp are complete for its 32 j-stars; the row sums of the W warps are added in fixed warp order at the flush.
+template <int I, int W, int MINB, bool MASK, bool EQM, bool JS = false, int UNR = 32 / I>
 __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp64_kernel(const JRec* __restrict__ jrec,
                                                                      double* __restrict__ part, int np, int n_tiles,
                                                                      int m, double eps2, double gm_eq)
 {
-    constexpr int U = W * 32 * I;
+    static_assert(!JS || W == I, "j-split form: one rotation group of the j tile per warp");
+    constexpr int U = kSymU<I, W, JS>;
     constexpr int NT = W * 32;
-    extern __shared__ double2 sym_smem[];  // kSymSmemBytes<I, W>: dynamic, U = 512 needs more than 48 KB
+    extern __shared__ double2 sym_smem[];  // kSymSmemBytes<I, W, JS>: dynamic, U = 512 needs more than 48 KB
     const int item = blockIdx.x;
     double2* sxy = sym_smem;                                                   // [U] x, y of the j tile
     double2* szm = sym_smem + U;                                               // [U] z, G m
-    double(*cacc)[3][U] = reinterpret_cast<double(*)[3][U]>(sym_smem + 2 * U);  // [W][3][U] per-warp column sums
+    double(*cacc)[3][U] = reinterpret_cast<double(*)[3][U]>(sym_smem + 2 * U);  // [W][3][U] per-warp sums
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
     int A, B;
     sym_decode_block(item, A, B);
 
     const int ta0 = A * m, ta1 = min(ta0 + m, n_tiles);
     const int tb0 = B * m, tb1 = min(tb0 + m, n_tiles);
-    const int i_local0 = w * 32 * I + lane;  // this lane's k-th i-star is i_local0 + 32 k inside the unit tile
+    const int i_local0 = JS ? lane : w * 32 * I + lane;  // this lane's k-th i-star is i_local0 + 32 k inside the unit tile
+    const int jb0 = JS ? 32 * w : 0, jb1 = JS ? 32 * w + 32 : U;  // rotation groups of the j tile this warp sweeps
+    double* cw = JS ? &cacc[0][0][0] : &cacc[w][0][0];            // where this warp's column sums go
 
     auto flush = [&](int slot, int tile, bool first, int n_src) {
         sym_flush<U, NT>(&cacc[0][0][0], part + (size_t)slot * 3 * np + (size_t)tile * U, np, first, n_src, tid, EQM ? gm_eq : 1.0);
@@ -407,22 +420,25 @@ __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp64_kernel(const JRec*
             }
             sym_sync<W>();
             if (ta == tb) {
-                sym_unit_tile<I, W, false, MASK, EQM>(sxy, szm, &cacc[w][0][0], xi, yi, zi, ngi, ax, ay, az, eps2, lane, i_local0);
+                sym_unit_tile<I, U, false, MASK, EQM, UNR>(sxy, szm, cw, xi, yi, zi, ngi, ax, ay, az, eps2, lane, i_local0, jb0, jb1);
             } else {
-                sym_unit_tile<I, W, true, false, EQM>(sxy, szm, &cacc[w][0][0], xi, yi, zi, ngi, ax, ay, az, eps2, lane, i_local0);
+                sym_unit_tile<I, U, true, false, EQM, UNR>(sxy, szm, cw, xi, yi, zi, ngi, ax, ay, az, eps2, lane, i_local0, jb0, jb1);
                 sym_sync<W>();
-                flush(A, tb, ta == ta0, W);  // column sums: the i-stars of tile ta acting on the j-stars of tile tb
+                flush(A, tb, ta == ta0, JS ? 1 : W);  // column sums: the i-stars of tile ta acting on the j-stars of tile tb
             }
         }
         sym_sync<W>();
+        {
+            double(*rw)[U] = JS ? cacc[w] : cacc[0];  // JS: every warp holds partial row sums of all U i-stars
 #pragma unroll
-        for (int k = 0; k < I; ++k) {
-            cacc[0][0][i_local0 + 32 * k] = ax[k];
-            cacc[0][1][i_local0 + 32 * k] = ay[k];
-            cacc[0][2][i_local0 + 32 * k] = az[k];
+            for (int k = 0; k < I; ++k) {
+                rw[0][i_local0 + 32 * k] = ax[k];
+                rw[1][i_local0 + 32 * k] = ay[k];
+                rw[2][i_local0 + 32 * k] = az[k];
+            }
         }
         sym_sync<W>();
-        flush(B, ta, (A < B) || (ta == ta0), 1);  // row sums: the j-stars of group B acting on the i-stars of tile ta
+        flush(B, ta, (A < B) || (ta == ta0), JS ? W : 1);  // row sums: the j-stars of group B acting on the i-stars of tile ta
     }
 }
 
