@@ -39,10 +39,54 @@ PAIR_KERNELS = {0: ("pair_fp64_kernel", 15, 24.0), 2: ("pair_sym_fp64_kernel", 1
                 4: ("pair_sym_fp64_kernel<EQM>", 9, 15.0), 5: ("pair_cross_fp64_kernel", 54, 85.0),
                 6: ("pair_cross_fp64_kernel<BHX>", 59, 93.0)}
 SMS, FP64_LANES_PER_SM = 148, 64
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu --set full
-# captures (profiles/), keyed by (variant, N_s); null when no capture exists for the workload
-NCU_DRAM_BYTES_PER_PAIR_LAUNCH = {(0, 16383): 793344, (2, 16383): 800000 + 943872, (4, 16383): 805120 + 237312,
-                                  (4, 65535): 3248640 + 142522368}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed `ncu --set full`
+# captures (per launch, cold L2: ncu flushes the caches before every replay), keyed by (variant, N_s); each entry names the
+# profiles/ file (which states the command and the kernel build) it was read from.  No entry -> "traffic": null.
+NCU_DRAM_BYTES_PER_PAIR_LAUNCH = {
+    (4, 16383): (805120 + 237312, "profiles/r1_ncu_summary.md section 2 (prof_r1c, pair_sym_fp64_kernel<4,1,8,0,1>, commit 32e2d05)"),
+    (4, 65535): (3248640 + 142522368, "profiles/r1_ncu_summary.md section 12 (prof_r1_c3, pair_sym_fp64_kernel<4,4,2,0,1>)"),
+}
+
+
+def algorithmic_bytes_per_pair_launch(cfg: dict) -> dict:
+    """What one launch of the star-star kernel has to move: every j record once (48 B per padded star) and the partial
+    sums it hands to the epilogue (24 B per star and slot)."""
+    npad, slots = cfg["padded_stars"], cfg["j_splits"]
+    return {"jrec_read": 48 * npad, "partial_sums_written": 24 * slots * npad, "total": 48 * npad + 24 * slots * npad}
+
+
+_BENCH_LIB = None
+
+
+def bench_lib():
+    """libpn_bench.so (include/pn_bench.h): pipe-peak probes; not part of the product library."""
+    global _BENCH_LIB
+    if _BENCH_LIB is None:
+        import ctypes
+
+        from paper_1801_07986_b200 import build
+
+        lib = ctypes.CDLL(str(build.BENCH_LIB))
+        lib.pn_bench_fp64_peak.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_double)]
+        lib.pn_bench_fp32_peak.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
+        _BENCH_LIB = lib
+    return _BENCH_LIB
+
+
+def measure_fp64_peak(stream) -> float:
+    import ctypes
+
+    t = ctypes.c_double(0.0)
+    rc = bench_lib().pn_bench_fp64_peak(ctypes.c_void_p(stream.cuda_stream), ctypes.byref(t))
+    return t.value if rc == 0 else None
+
+
+def measure_fp32_peak(stream, packed: bool) -> float:
+    import ctypes
+
+    t = ctypes.c_double(0.0)
+    rc = bench_lib().pn_bench_fp32_peak(ctypes.c_void_p(stream.cuda_stream), int(packed), ctypes.byref(t))
+    return t.value if rc == 0 else None
 
 
 def load_peaks() -> dict:
@@ -214,6 +258,9 @@ def cpu_baseline(p, target_s=12.0, max_steps=200, terms=0) -> dict:
     dt = time.perf_counter() - t0
     out = {"value": pairs / dt, "unit": "pair-interactions/s", "cores": o.max_threads, "kind": "oracle",
            "build": "oracle/pn_oracle.c -DORACLE_FAST (double, -O3 -march=native, OpenMP over i)",
+           "note": "the parity oracle as it stands: plain scalar loops over every ORDERED pair, array-of-structures data, a sqrt and "
+                   "three divisions per pair, no use of Newton's third law -- a reported baseline, not a tuned CPU code; a ratio "
+                   "against it says nothing about kernel quality (the roofline fraction does)",
            "sample": f"{n} x {what}; {dt:.1f} s", "steps_per_s": (n / dt) if rows is None else None}
     # the like-for-like counterpart of the paper's single-core CPU column (Table 3.2): the same oracle on
     # ONE thread, on a seeded subset of i-rows (rows are independent), about 5 s
@@ -368,7 +415,7 @@ def run_ours(args) -> None:
     ms_total = ms_energy + ms_steps
     pair_ms, pair_n = pn.pn_get_pair_time(reset=True)
     pn.pn_set_option(binding.PN_OPT_TIME_PAIR, 0)
-    dfma_peak = pn.pn_measure_fp64_peak()  # register-only DFMA chains on this device, TFLOP/s
+    dfma_peak = measure_fp64_peak(stream)  # register-only DFMA chains on this device, TFLOP/s (libpn_bench.so)
 
     # ---------------- same K steps through the CUDA-graph path (information: what a user gets by default)
     pn.pn_set_state(pos_d, vel_d)
@@ -416,7 +463,9 @@ def run_ours(args) -> None:
         roof = {
             "bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
             "frac": (achieved / peak_tflops) if achieved else None,
-            "traffic": NCU_DRAM_BYTES_PER_PAIR_LAUNCH.get((cfg["variant"], p.n_stars)),
+            "traffic": NCU_DRAM_BYTES_PER_PAIR_LAUNCH.get((cfg["variant"], p.n_stars), (None, None))[0],
+            "traffic_source": NCU_DRAM_BYTES_PER_PAIR_LAUNCH.get((cfg["variant"], p.n_stars), (None, "no ncu capture of this kernel at this size"))[1],
+            "algorithmic_bytes": algorithmic_bytes_per_pair_launch(cfg),
             "convention": f"{instr} FP64-pipe instructions per ordered pair in the shipped SASS, each counted as an "
                           f"FMA (2 flops) = FP64-pipe issue-slot utilisation; peak = {SMS} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x "
                           f"{sm_max:.0f} MHz (clocks.max.sm; no measured fp64 peak in MEASURED_PEAKS.json)",
@@ -429,6 +478,7 @@ def run_ours(args) -> None:
             "peak_measured_dfma": dfma_peak,
             "frac_of_measured_dfma": (achieved / dfma_peak) if achieved and dfma_peak else None,
         }
+        bar = bar_leg(args, stream, flush, local, peak_tflops, sm_max) if (world == 1 and args.workload == "config2" and not args.cross and not args.no_bar) else None
         base = cpu_baseline(p, terms=cross_mask(args)) if not args.no_cpu_baseline else None
         line = {
             "metric": "fp64 pair-interactions/s", "value": value, "unit": "pair-interactions/s", "n_gpus": world,
@@ -442,12 +492,52 @@ def run_ours(args) -> None:
             "e2e": {"value": e2e_val, "unit": "pair-interactions/s", "h2d_bytes_per_step": 2 * p.N * 24,
                     "d2h_bytes_per_step": 2 * p.N * 24, "ms_per_step": 1e3 * e2e_m / K,
                     "api": "pn_set_state_host + pn_step + pn_get_state_host per step, pinned host buffers"},
-            "gpu_launches": launches, "roofline": roof, "cpu_baseline": base,
+            "gpu_launches": launches, "roofline": roof, "bar": bar, "cpu_baseline": base,
         }
         print(json.dumps(line), flush=True)
     pn.pn_destroy()
     if world > 1:
         dist.destroy_process_group()
+
+
+def bar_leg(args, stream, flush, local, peak_tflops, sm_max, steps: int = 3) -> dict:
+    """The configuration the >= 70 % bar of north_star is defined on (BASELINE.json configs[2], N = 1+65535): a short leg of
+    the same measurement (RK4 steps on the CUDA graph, the pair stage of the first force evaluation of every step bracketed
+    by event-record nodes, L2 flushed between steps, clocks sampled), so that the driver's own run observes it."""
+    import torch
+
+    from paper_1801_07986_b200 import PN, binding
+
+    p = make_problem("config3")
+    pn = PN(p.mass, p.G, p.c, p.softening, stream=stream)
+    cfg = pn.pn_get_pair_config()
+    kname, instr, _ = PAIR_KERNELS[cfg["variant"]]
+    pn.pn_set_option(binding.PN_OPT_TIME_PAIR, 2)
+    pn.pn_set_state(torch.from_numpy(p.pos).cuda(), torch.from_numpy(p.vel).cuda())
+    pn.pn_step(p.dt, 3)
+    torch.cuda.synchronize()
+    pn.pn_get_pair_time(reset=True)
+    sampler = make_sampler(local)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    t0 = time.perf_counter()
+    for a, b in ev:
+        flush.zero_()
+        a.record(stream)
+        pn.pn_step(p.dt, 1)
+        b.record(stream)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    clocks = sampler.stop(t0, t1)
+    ms_steps = [a.elapsed_time(b) for a, b in ev]
+    pair_ms, pair_n = pn.pn_get_pair_time(reset=True)
+    pn.pn_destroy()
+    avg = pair_ms / max(1, pair_n)
+    rate = p.pairs_per_eval / (avg * 1e-3)
+    return {"workload": p.name, "N": p.N, "kernel": kname, "pair_config": cfg, "steps": steps, "ms_per_step": float(np.mean(ms_steps)),
+            "pairs_per_s": 4 * p.pairs_per_eval / (float(np.mean(ms_steps)) * 1e-3), "avg_launch_ms": avg, "launches_timed": pair_n,
+            "kernel_pairs_per_s": rate, "frac": rate * 2 * instr / 1e12 / peak_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
+            "convention": f"{instr} FP64-pipe instructions per ordered pair, issue-slot convention, as roofline.frac", "clocks": clocks}
 
 
 def run_sweep(args) -> None:
@@ -589,6 +679,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-bar", action="store_true", help="skip the short config-3 leg (the >= 70 %% bar's configuration)")
     ap.add_argument("--cross", nargs="?", const="star", default=None, choices=["star", "full"],
                     help="add the Cross terms (NEXT rows of the scope table): star = [a_i]_Cross, Eq. 2.6; "
                          "full = also [a_1]_Cross, Eq. 2.3 (the paper's full limited-1PN force)")

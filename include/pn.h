@@ -23,6 +23,15 @@
  *   - All work is enqueued on the context's stream (pn_set_stream; default: the legacy default
  *     stream).  Calls with only device arguments are asynchronous; calls that take or return host
  *     data synchronise that stream before returning.
+ *   - A context is single-stream and single-threaded: pn_accel, pn_step, pn_energy and pn_momentum share
+ *     the context's scratch buffers (partial sums, the block partials of a_1 and their ticket counter),
+ *     so calls on one context must not run concurrently -- one stream at a time, one host thread at a
+ *     time.  pn_set_stream orders the new stream after everything already enqueued on the old one.
+ *     Use one context per stream for concurrent work.
+ *   - A context belongs to the CUDA device that was current in pn_create; every later call must be made
+ *     with that device current (PN_EINVAL otherwise; pn_destroy switches to it by itself).
+ *   - Size limit: 2 <= N <= 2^24 bodies (PN_EINVAL beyond; star indices and tile counts are 32-bit, the
+ *     partial-sum buffer grows as 3 KB per star: 12.9 GB at N = 2^22, 51.5 GB at N = 2^24).
  *   - There is no CPU fallback: without a CUDA device pn_create fails with PN_ECUDA.
  *   - Coincident bodies (BH-star distance 0, or two stars at distance 0 with eps = 0) give
  *     inf/NaN, propagated, not trapped.  With eps = 0 the self term j = i is skipped by index.
@@ -37,7 +46,7 @@ extern "C" {
 #endif
 
 #define PN_OK 0
-#define PN_EINVAL (-1) /* bad argument: N < 2, null pointer, non-finite/negative mass, M <= 0, G <= 0, c <= 0 or NaN,
+#define PN_EINVAL (-1) /* bad argument: N < 2 or N > 2^24, wrong current device, null pointer, non-finite/negative mass, M <= 0, G <= 0, c <= 0 or NaN,
                           eps < 0 or NaN, non-finite dt, nsteps < 0, unknown option/value */
 #define PN_ECUDA (-2)  /* a CUDA call failed (text in pn_last_error) or no device */
 #define PN_ESTATE (-3) /* pn_step / pn_energy / pn_get_state before any pn_set_state */
@@ -75,7 +84,7 @@ extern "C" {
 #define PN_FP32_PAIR 1 /* fp32 pair arithmetic on two-float positions, fp64 accumulation (parity 1e-5) */
 
 /* PN_OPT_PAIR_KERNEL values (either pair precision) */
-#define PN_PAIR_AUTO 0      /* symmetric for N - 1 >= 3072 stars, tiled below */
+#define PN_PAIR_AUTO 0      /* symmetric for N - 1 >= 3072 stars (unit tiles of 128 stars, 512 from 40000 stars on), tiled below */
 #define PN_PAIR_TILED 1     /* every ordered pair (i, j): 15 FP64 (18 FP32) instructions per ordered pair */
 #define PN_PAIR_SYMMETRIC 2 /* every unordered pair once, applied to both stars (Newton's third law, exact for the
                                softened Newtonian term of Eq. 2.4): 10 FP64 (11 FP32) instructions per ordered pair */
@@ -83,12 +92,14 @@ extern "C" {
 typedef struct pn_ctx pn_ctx; /* opaque; owns all internal device buffers */
 
 /* Problem statement of the paper: one massive object + N-1 stars, constants G, c and
- * the star-star Plummer softening eps.  masses_host: N host doubles, copied; masses_host[0] = M > 0, stars >= 0.
- * c may be +inf (pure Newtonian).  Uses the current CUDA device.  *out is set to NULL on failure. */
+ * the star-star Plummer softening eps.  2 <= N <= 2^24.  masses_host: N host doubles, copied; masses_host[0] = M > 0,
+ * stars >= 0.  c may be +inf (pure Newtonian).  Uses the current CUDA device, and stays on it.  *out is set to NULL on
+ * failure (pn_last_error(NULL) has the text). */
 int pn_create(pn_ctx** out, int64_t N, const double* masses_host, double G, double c, double softening);
 int pn_destroy(pn_ctx* ctx); /* synchronises, frees everything; NULL is allowed */
 
-int pn_set_stream(pn_ctx* ctx, void* cuda_stream); /* a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) */
+int pn_set_stream(pn_ctx* ctx, void* cuda_stream); /* a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); the new
+                                                      stream waits for the work already enqueued on the old one */
 int pn_set_option(pn_ctx* ctx, int key, int value);
 
 /* Integrator state (x, v) of all N bodies.  [N][3] each. */
@@ -118,8 +129,9 @@ int pn_momentum(pn_ctx* ctx, double* P_host);
 
 /* Bookkeeping for benchmarks. */
 int pn_get_launch_count(pn_ctx* ctx, int64_t* n_kernels_host);          /* kernels launched (graph nodes count) */
-int pn_get_pair_time(pn_ctx* ctx, double* ms_total_host, int64_t* n_launches_host, int reset); /* PN_OPT_TIME_PAIR;
-                                                                            synchronises the stream */
+int pn_get_pair_time(pn_ctx* ctx, double* ms_total_host, int64_t* n_launches_host, int reset); /* PN_OPT_TIME_PAIR: sum of
+                                                                            the bracketed pair-stage times and their count
+                                                                            since the last reset; synchronises the stream */
 int pn_get_pair_config(pn_ctx* ctx, int32_t* cfg_host); /* 8 ints: threads/block, i per thread, j-tile, partial-sum
                                                            slots (j-splits / groups), grid blocks, padded N_s, pipe
                                                            instructions per ordered pair, variant (0 fp64 tiled,
@@ -127,10 +139,6 @@ int pn_get_pair_config(pn_ctx* ctx, int32_t* cfg_host); /* 8 ints: threads/block
                                                            4 fp64 symmetric, equal-mass form,
                                                            5 fp64 ordered pairs with the Cross terms of Eq. 2.6,
                                                            6 the same with the O(N^2) sum of Eq. 2.3) */
-
-int pn_measure_fp64_peak(pn_ctx* ctx, double* tflops_host); /* sustained FP64 FMA rate of this device from a register-only
-                                                              DFMA-chain kernel (2 flops per FMA), best of 3: the measured
-                                                              roofline denominator of the pair kernel.  Synchronous. */
 
 const char* pn_last_error(pn_ctx* ctx); /* ctx may be NULL: last error of a failed pn_create in this thread */
 const char* pn_version(void);

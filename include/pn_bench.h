@@ -1,0 +1,29 @@
+/*
+ * pn_bench.h -- C-ABI of libpn_bench.so: roofline-denominator probes for bench.py.  NOT part of the product library
+ * (libpn.so, include/pn.h): nothing of the hot path lives here, and nothing in libpn.so depends on it.
+ *
+ * Each probe runs register-only chains of one arithmetic instruction on every SM of the current CUDA device and
+ * returns the best of three timed launches (CUDA events on `cuda_stream`) as TFLOP/s, counting an FMA as 2 flops per
+ * lane.  They give the measured counterpart of the nominal pipe peaks that DESIGN.md section 6 derives from the unit
+ * counts (FP64: 64 lanes per SM; FP32: 128 lanes per SM) and the SM clock.
+ *
+ * Return value: 0 on success, -2 on a CUDA error (no device, launch failure).  Synchronous.
+ */
+#ifndef PN_BENCH_H_
+#define PN_BENCH_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* sustained DFMA rate: the roofline denominator of the fp64 star-star pair kernels */
+int pn_bench_fp64_peak(void* cuda_stream, double* tflops_host);
+
+/* sustained FP32 FMA rate; packed = 0: scalar FFMA, packed = 1: the packed two-lane form fma.rn.f32x2 (FFMA2, one
+   instruction for two FMAs per thread), which the fp32-pair kernels use */
+int pn_bench_fp32_peak(void* cuda_stream, int packed, double* tflops_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PN_BENCH_H_ */

@@ -25,7 +25,7 @@ PN_PAIR_AUTO, PN_PAIR_TILED, PN_PAIR_SYMMETRIC = 0, 1, 2
 EXPORTS = (
     "pn_create", "pn_destroy", "pn_set_stream", "pn_set_option", "pn_set_state", "pn_get_state",
     "pn_set_state_host", "pn_get_state_host", "pn_accel", "pn_accel_host", "pn_step", "pn_energy", "pn_momentum",
-    "pn_get_launch_count", "pn_get_pair_time", "pn_get_pair_config", "pn_measure_fp64_peak", "pn_last_error",
+    "pn_get_launch_count", "pn_get_pair_time", "pn_get_pair_config", "pn_last_error",
     "pn_version",
 )
 
@@ -64,7 +64,6 @@ def load_library() -> ctypes.CDLL:
     lib.pn_get_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
     lib.pn_get_pair_time.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(i64), ci]
     lib.pn_get_pair_config.argtypes = [vp, ctypes.POINTER(ctypes.c_int32)]
-    lib.pn_measure_fp64_peak.argtypes = [vp, ctypes.POINTER(dbl)]
     lib.pn_last_error.argtypes = [vp]
     lib.pn_last_error.restype = ctypes.c_char_p
     lib.pn_version.argtypes = []
@@ -205,11 +204,6 @@ class PN:
         _check(self._lib, self._ctx, self._lib.pn_get_pair_config(self._ctx, cfg))
         keys = ("threads", "i_per_thread", "j_tile", "j_splits", "grid_blocks", "padded_stars", "fp64_instr_per_pair", "variant")
         return dict(zip(keys, list(cfg)))
-
-    def pn_measure_fp64_peak(self) -> float:
-        t = ctypes.c_double(0.0)
-        _check(self._lib, self._ctx, self._lib.pn_measure_fp64_peak(self._ctx, ctypes.byref(t)))
-        return t.value
 
     def pn_destroy(self):
         if self._ctx:

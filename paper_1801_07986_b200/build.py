@@ -1,4 +1,5 @@
-"""Build libpn.so (the C-ABI CUDA library) in-tree for sm_100a with nvcc.
+"""Build libpn.so (the C-ABI CUDA library) and libpn_bench.so (bench.py's pipe-peak probes, include/pn_bench.h) in-tree
+for sm_100a with nvcc.
 
     python -m paper_1801_07986_b200.build [--force] [--verbose]
 
@@ -19,6 +20,9 @@ INCLUDE = PKG.parent / "include"
 LIB = PKG / "libpn.so"
 SOURCES = [CSRC / "pn_api.cu"]
 HEADERS = [CSRC / "pn_kernels.cuh", INCLUDE / "pn.h"]
+BENCH_LIB = PKG / "libpn_bench.so"  # roofline-denominator probes for bench.py; not linked into or loaded by the product
+BENCH_SOURCES = [CSRC / "pn_bench.cu"]
+BENCH_HEADERS = [INCLUDE / "pn_bench.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -36,23 +40,32 @@ def nvcc_path() -> str:
     raise RuntimeError("nvcc not found; the CUDA library cannot be built (there is no CPU fallback)")
 
 
-def needs_build() -> bool:
-    if not LIB.exists():
+def _stale(lib: Path, deps) -> bool:
+    if not lib.exists():
         return True
-    t = LIB.stat().st_mtime
-    return any(p.stat().st_mtime > t for p in SOURCES + HEADERS + [Path(__file__)])
+    t = lib.stat().st_mtime
+    return any(p.stat().st_mtime > t for p in list(deps) + [Path(__file__)])
 
 
-def build(force: bool = False, verbose: bool = False) -> Path:
-    if not force and not needs_build():
-        return LIB
-    tmp = LIB.with_suffix(f".tmp{os.getpid()}.so")
+def needs_build() -> bool:
+    return _stale(LIB, SOURCES + HEADERS) or _stale(BENCH_LIB, BENCH_SOURCES + BENCH_HEADERS)
+
+
+def _nvcc(sources, out: Path, verbose: bool) -> None:
+    tmp = out.with_suffix(f".tmp{os.getpid()}.so")
     cmd = [nvcc_path(), *NVCC_FLAGS, f"-I{INCLUDE}", *(["-Xptxas", "-v"] if verbose else []),
-           *map(str, SOURCES), "-o", str(tmp)]
+           *map(str, sources), "-o", str(tmp)]
     if verbose:
         print(" ".join(cmd), file=sys.stderr)
     subprocess.run(cmd, check=True)
-    os.replace(tmp, LIB)
+    os.replace(tmp, out)
+
+
+def build(force: bool = False, verbose: bool = False) -> Path:
+    if force or _stale(LIB, SOURCES + HEADERS):
+        _nvcc(SOURCES, LIB, verbose)
+    if force or _stale(BENCH_LIB, BENCH_SOURCES + BENCH_HEADERS):
+        _nvcc(BENCH_SOURCES, BENCH_LIB, verbose)
     return LIB
 
 

@@ -19,7 +19,6 @@ namespace {
 constexpr int kNT = 128;        // threads per block of the pair / energy / epilogue kernels
 constexpr int kTJ = 128;        // j records per shared-memory tile
 constexpr int kGraphBatch = 16; // RK4 steps captured in the batched graph
-constexpr int kSMs = 148;       // B200
 constexpr int kCrossI = 2;      // i-stars per thread of pair_cross_fp64_kernel
 constexpr int kCrossTJ = 64;    // its j tile (96 B records)
 
@@ -31,8 +30,10 @@ struct pn_ctx {
     int64_t N = 0;
     int n_stars = 0, np = 0;
     double G = 0, c = 0, eps = 0, M = 0, GM = 0, inv_c2 = 0, eps2 = 0;
+    int device = 0, n_sm = 148;  // the CUDA device the context was created on, its SM count
     cudaStream_t stream = nullptr;
     cudaStream_t cap_stream = nullptr;
+    cudaEvent_t stream_ev = nullptr;  // orders a new stream after the old one in pn_set_stream
     std::string err;
 
     // options
@@ -79,8 +80,10 @@ struct pn_ctx {
     int graph_split = -1, graph_precision = -1, graph_sym = -1, graph_eqm = -1;
 
     int64_t n_launch = 0;
-    std::vector<cudaEvent_t> ev;  // pairs (start, stop)
+    std::vector<cudaEvent_t> ev;  // pairs (start, stop); a bounded pool, folded into the two sums below when it fills
     size_t ev_used = 0;
+    double pair_ms_folded = 0;
+    int64_t pair_n_folded = 0;
 };
 
 namespace {
@@ -117,7 +120,7 @@ void choose_split(pn_ctx* c)
     int s = c->j_split_opt;
     if (s <= 0) {
         // ~28 blocks per SM (4 resident) keeps the tail of the last wave small; at least one tile per block
-        s = (kSMs * 28 + c->n_itiles - 1) / c->n_itiles;
+        s = (c->n_sm * 28 + c->n_itiles - 1) / c->n_itiles;
     }
     if (s > c->n_tiles) s = c->n_tiles;
     if (s > c->max_split) s = c->max_split;
@@ -245,8 +248,27 @@ void launch_pair_sym(pn_ctx* c, int set, cudaStream_t st)
         eqm ? launch_pair_sym_v<I, W, MINB, JS, false, true>(c, set, st) : launch_pair_sym_v<I, W, MINB, JS, false, false>(c, set, st);
 }
 
+constexpr size_t kMaxEvents = 4096;  // PN_OPT_TIME_PAIR event pool: 2048 timed launches between folds
+
+// adds the elapsed times of the recorded event pairs to the running sums and recycles the pool (synchronises the stream)
+int fold_events(pn_ctx* c)
+{
+    if (c->ev_used == 0) return PN_OK;
+    PN_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (size_t q = 0; q + 1 < c->ev_used; q += 2) {
+        float ms = 0;
+        PN_CUDA(c, cudaEventElapsedTime(&ms, c->ev[q], c->ev[q + 1]));
+        c->pair_ms_folded += ms;
+    }
+    c->pair_n_folded += (int64_t)(c->ev_used / 2);
+    c->ev_used = 0;
+    return PN_OK;
+}
+
 int reserve_events(pn_ctx* c, size_t n)
 {
+    if (c->ev_used + n > kMaxEvents)
+        if (int rc = fold_events(c)) return rc;
     while (c->ev_used + n > c->ev.size()) {
         cudaEvent_t e;
         PN_CUDA(c, cudaEventCreate(&e));
@@ -368,18 +390,9 @@ int build_graph(pn_ctx* c, int nrep, cudaGraphExec_t* out)
     return PN_OK;
 }
 
-// One RK4 step with event-record nodes around the pair stage of each of the 4 force evaluations.
-int build_timed_graph(pn_ctx* c)
+// the event-record nodes of the captured timed graph, by template event
+int find_timed_nodes(pn_ctx* c)
 {
-    for (int q = 0; q < 8; ++q)
-        if (!c->tev[q]) PN_CUDA(c, cudaEventCreate(&c->tev[q]));
-    PN_CUDA(c, cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
-    c->cap_ev = 0;
-    int rc = enqueue_rk4_step(c, c->cap_stream, true);
-    c->cap_ev = -1;
-    cudaError_t e = cudaStreamEndCapture(c->cap_stream, &c->graphT_src);
-    if (rc != PN_OK) return rc;
-    if (e != cudaSuccess) return fail(c, PN_ECUDA, "cudaStreamEndCapture (timed graph) failed: %s", cudaGetErrorString(e));
     size_t n = 0;
     PN_CUDA(c, cudaGraphGetNodes(c->graphT_src, nullptr, &n));
     std::vector<cudaGraphNode_t> nodes(n);
@@ -396,14 +409,45 @@ int build_timed_graph(pn_ctx* c)
     }
     const int want = (c->time_pair == 2) ? 2 : 8;
     if (found != want) return fail(c, PN_ECUDA, "timed graph: %d of %d event-record nodes found", found, want);
-    e = cudaGraphInstantiate(&c->graphT, c->graphT_src, 0);
-    if (e != cudaSuccess) return fail(c, PN_ECUDA, "cudaGraphInstantiate (timed graph) failed: %s", cudaGetErrorString(e));
     return PN_OK;
 }
 
+// One RK4 step with event-record nodes around the pair stage of each of the 4 force evaluations.
+int build_timed_graph(pn_ctx* c)
+{
+    for (int q = 0; q < 8; ++q)
+        if (!c->tev[q]) PN_CUDA(c, cudaEventCreate(&c->tev[q]));
+    PN_CUDA(c, cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+    c->cap_ev = 0;
+    int rc = enqueue_rk4_step(c, c->cap_stream, true);
+    c->cap_ev = -1;
+    cudaError_t e = cudaStreamEndCapture(c->cap_stream, &c->graphT_src);
+    if (rc == PN_OK && e != cudaSuccess) rc = fail(c, PN_ECUDA, "cudaStreamEndCapture (timed graph) failed: %s", cudaGetErrorString(e));
+    if (rc == PN_OK) rc = find_timed_nodes(c);
+    if (rc == PN_OK) {
+        e = cudaGraphInstantiate(&c->graphT, c->graphT_src, 0);
+        if (e != cudaSuccess) rc = fail(c, PN_ECUDA, "cudaGraphInstantiate (timed graph) failed: %s", cudaGetErrorString(e));
+    }
+    if (rc != PN_OK) {  // nothing half-built survives a failure: the next call starts from scratch
+        destroy_graphs(c);
+        for (cudaGraphNode_t& nd : c->tnode) nd = nullptr;
+    }
+    return rc;
+}
+
+// every entry point: the context must exist and its device must be the calling thread's current device (device
+// pointers and kernel launches of a context belong to the device it was created on)
 int check_ctx(pn_ctx* c)
 {
-    return c ? PN_OK : fail(nullptr, PN_EINVAL, "null context");
+    if (!c) return fail(nullptr, PN_EINVAL, "null context");
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, PN_ECUDA, "cudaGetDevice failed");
+    }
+    if (dev != c->device)
+        return fail(c, PN_EINVAL, "the context lives on CUDA device %d but the current device is %d (cudaSetDevice first)", c->device, dev);
+    return PN_OK;
 }
 
 }  // namespace
@@ -437,6 +481,12 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
 
     pn_ctx* ctx = new (std::nothrow) pn_ctx;
     if (!ctx) return fail(nullptr, PN_ENOMEM, "pn_create: out of host memory");
+    if (cudaGetDevice(&ctx->device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, ctx->device) != cudaSuccess || ctx->n_sm < 1) {
+        cudaGetLastError();
+        delete ctx;
+        return fail(nullptr, PN_ECUDA, "pn_create: cannot query the current CUDA device");
+    }
     ctx->N = N;
     ctx->n_stars = (int)(N - 1);
     ctx->G = G, ctx->c = c, ctx->eps = softening, ctx->M = masses[0];
@@ -471,6 +521,7 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
 
     const size_t np = ctx->np;
     CREATE_CUDA(cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
+    CREATE_CUDA(cudaEventCreateWithFlags(&ctx->stream_ev, cudaEventDisableTiming));
     for (int s = 0; s < 2; ++s) {
         CREATE_CUDA(dalloc(&ctx->jrec[s], np));
         CREATE_CUDA(dalloc(&ctx->v[s], 3 * np));
@@ -501,7 +552,7 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
         const int n_it = (int)(np / kNT);
         // the energy pair kernel runs n_it / 2 mirrored i-tile pairs per j-split, all of equal work: aim at one full wave
         // (7 blocks of 72 registers x 128 threads per SM) rather than a full wave plus a short one
-        int s = (kSMs * 7) / (n_it / 2);
+        int s = (ctx->n_sm * 7) / (n_it / 2);
         s = std::max(1, std::min(s, std::min(ctx->n_tiles, 64)));
         ctx->e_split = s;  // each i-tile splits its own range of j-tiles into e_split chunks inside the kernel
         CREATE_CUDA(dalloc(&ctx->blk_prep, 4 * (size_t)n_it));
@@ -530,9 +581,15 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
 int pn_destroy(pn_ctx* c)
 {
     if (!c) return PN_OK;
+    int prev = -1;
+    cudaGetDevice(&prev);
+    if (prev != c->device) cudaSetDevice(c->device);
     cudaDeviceSynchronize();
     destroy_graphs(c);
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->tev)
+        if (e) cudaEventDestroy(e);
+    if (c->stream_ev) cudaEventDestroy(c->stream_ev);
     for (int s = 0; s < 2; ++s) cudaFree(c->jrec[s]), cudaFree(c->v[s]), cudaFree(c->bh[s]);
     cudaFree(c->x0), cudaFree(c->v0), cudaFree(c->sx), cudaFree(c->sv);
     cudaFree(c->part), cudaFree(c->bh_part), cudaFree(c->ticket), cudaFree(c->prm);
@@ -541,6 +598,7 @@ int pn_destroy(pn_ctx* c)
     cudaFree(c->frec), cudaFree(c->erec), cudaFree(c->blk_prep), cudaFree(c->blk_pair), cudaFree(c->d_energy);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     cudaGetLastError();
+    if (prev >= 0 && prev != c->device) cudaSetDevice(prev);
     delete c;
     return PN_OK;
 }
@@ -548,7 +606,14 @@ int pn_destroy(pn_ctx* c)
 int pn_set_stream(pn_ctx* c, void* s)
 {
     if (int rc = check_ctx(c)) return rc;
-    c->stream = static_cast<cudaStream_t>(s);
+    cudaStream_t ns = static_cast<cudaStream_t>(s);
+    if (ns != c->stream) {
+        // pn_accel and pn_step share the context's scratch (partial sums, the a_1 block partials and their ticket):
+        // work already enqueued on the old stream must finish before anything enqueued on the new one touches it
+        PN_CUDA(c, cudaEventRecord(c->stream_ev, c->stream));
+        PN_CUDA(c, cudaStreamWaitEvent(ns, c->stream_ev, 0));
+        c->stream = ns;
+    }
     return PN_OK;
 }
 
@@ -582,7 +647,7 @@ int pn_set_option(pn_ctx* c, int key, int value)
                 c->crec = nullptr, c->cblk = nullptr, c->csum = nullptr;
                 const size_t np = c->np;
                 const int n_it = c->np / (kCrossI * kNT), n_t = c->np / kCrossTJ;
-                int s = std::max(1, std::min(std::min((kSMs * 16 + n_it - 1) / n_it, n_t), 64));
+                int s = std::max(1, std::min(std::min((c->n_sm * 16 + n_it - 1) / n_it, n_t), 64));
                 c->c_tiles_per_split = (n_t + s - 1) / s;
                 c->c_split = (n_t + c->c_tiles_per_split - 1) / c->c_tiles_per_split;
                 PN_CUDA(c, dalloc(&c->crec, np));
@@ -804,44 +869,10 @@ int pn_get_pair_time(pn_ctx* c, double* ms_total, int64_t* n_launches, int reset
 {
     if (int rc = check_ctx(c)) return rc;
     if (!ms_total || !n_launches) return fail(c, PN_EINVAL, "pn_get_pair_time: null pointer");
-    PN_CUDA(c, cudaStreamSynchronize(c->stream));
-    double tot = 0;
-    for (size_t q = 0; q + 1 < c->ev_used; q += 2) {
-        float ms = 0;
-        PN_CUDA(c, cudaEventElapsedTime(&ms, c->ev[q], c->ev[q + 1]));
-        tot += ms;
-    }
-    *ms_total = tot;
-    *n_launches = (int64_t)(c->ev_used / 2);
-    if (reset) c->ev_used = 0;
-    return PN_OK;
-}
-
-int pn_measure_fp64_peak(pn_ctx* c, double* tflops)
-{
-    if (int rc = check_ctx(c)) return rc;
-    if (!tflops) return fail(c, PN_EINVAL, "pn_measure_fp64_peak: null pointer");
-    const int blocks = kSMs * 8, iters = 8192;
-    double* out = nullptr;
-    PN_CUDA(c, dalloc(&out, (size_t)blocks * 128));
-    cudaEvent_t a, b;
-    PN_CUDA(c, cudaEventCreate(&a));
-    PN_CUDA(c, cudaEventCreate(&b));
-    float best = 0;
-    fp64_peak_kernel<<<blocks, 128, 0, c->stream>>>(out, 64);
-    for (int rep = 0; rep < 3; ++rep) {
-        PN_CUDA(c, cudaEventRecord(a, c->stream));
-        fp64_peak_kernel<<<blocks, 128, 0, c->stream>>>(out, iters);
-        PN_CUDA(c, cudaEventRecord(b, c->stream));
-        PN_CUDA(c, cudaEventSynchronize(b));
-        float ms = 0;
-        PN_CUDA(c, cudaEventElapsedTime(&ms, a, b));
-        const float tf = (float)((double)blocks * 128 * iters * 64 * 2 / (ms * 1e-3) / 1e12);
-        if (tf > best) best = tf;
-    }
-    c->n_launch += 4;
-    cudaEventDestroy(a), cudaEventDestroy(b), cudaFree(out);
-    *tflops = best;
+    if (int rc = fold_events(c)) return rc;
+    *ms_total = c->pair_ms_folded;
+    *n_launches = c->pair_n_folded;
+    if (reset) c->pair_ms_folded = 0, c->pair_n_folded = 0;
     return PN_OK;
 }
 

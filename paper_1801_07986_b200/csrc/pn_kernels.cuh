@@ -9,7 +9,7 @@
 //   S2-S4  epilogue_kernel        partial-sum reduction, BH <-> star Newtonian + 1PN, a_1 reduction, fused RK4 stage update
 //   S5  energy_prep / energy_pair / energy_final   Eq. 2.7, compensated
 //   NEXT-3  momentum_prep / momentum_pair / momentum_final   Eq. 2.8, compensated
-//   pack / unpack (AoS <-> internal layout), fp64_peak_kernel (DFMA-chain probe)
+//   pack / unpack (AoS <-> internal layout)
 //
 // Internal data layout (all fp64, star index s = body index - 1, padded to NP):
 //   JRec  jrec[NP]      : stage position + mass constants of star s, 48 B, 16 B aligned.  This is the record the
@@ -854,25 +854,6 @@ __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp32_kernel(const FRec*
         sym_sync<W>();
         flush(B, ta, (A < B) || (ta == ta0), 1);
     }
-}
-
-// Register-only DFMA chains: measures the sustained FP64 FMA rate of the device (roofline denominator).
-__global__ void __launch_bounds__(128) fp64_peak_kernel(double* out, int iters)
-{
-    double a[8];
-#pragma unroll
-    for (int q = 0; q < 8; ++q) a[q] = threadIdx.x * 1e-9 + q;
-    const double m = 1.0000001, c = 1e-9;
-    for (int i = 0; i < iters; ++i) {
-#pragma unroll
-        for (int u = 0; u < 8; ++u)
-#pragma unroll
-            for (int q = 0; q < 8; ++q) a[q] = fma(a[q], m, c);
-    }
-    double s = 0;
-#pragma unroll
-    for (int q = 0; q < 8; ++q) s += a[q];
-    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
 // ---------------------------------------------------------------------------------------------------------

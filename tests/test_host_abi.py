@@ -94,3 +94,45 @@ def test_product_path_does_not_reference_oracle():
             for line in p.read_text().splitlines():
                 if re.match(r"\s*(#\s*include|import|from)\b", line):
                     assert "paper_1801_07986_b200" not in line and "csrc" not in line and "pn.h" not in line, (p, line)
+
+
+# ------------------------------------------------------------------ the header as a C header; the bench-only probe library
+def _build_abi_smoke(tmp_path):
+    """gcc -std=c11 -pedantic: pn.h must be a self-sufficient C header; linking checks the symbols a C client needs."""
+    import subprocess
+
+    from paper_1801_07986_b200 import build
+
+    build.build()
+    exe = tmp_path / "abi_smoke"
+    cmd = ["gcc", "-std=c11", "-Wall", "-Wextra", "-Werror", "-pedantic", f"-I{ROOT / 'include'}", str(ROOT / "tests" / "abi_smoke.c"),
+           f"-L{build.LIB.parent}", "-lpn", f"-Wl,-rpath,{build.LIB.parent}", "-lm", "-o", str(exe)]
+    subprocess.run(cmd, check=True)
+    return exe
+
+
+def test_c_client_compiles_links_and_refuses_to_run_without_a_gpu(tmp_path):
+    import subprocess
+
+    import torch
+
+    exe = _build_abi_smoke(tmp_path)
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present: tests/test_gpu_abi_smoke.py runs the client")
+    r = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert r.returncode == 3 and "no CUDA device" in r.stderr  # no CPU fallback behind the C entry points either
+
+
+def test_bench_probe_library_is_separate_and_exports_its_header():
+    from paper_1801_07986_b200 import build
+
+    build.build()
+    text = re.sub(r"/\*.*?\*/", "", (ROOT / "include" / "pn_bench.h").read_text(), flags=re.S)
+    declared = sorted(set(re.findall(r"\b(pn_bench_[a-z_0-9]+)\s*\(", text)))
+    assert declared == ["pn_bench_fp32_peak", "pn_bench_fp64_peak"]
+    blib = ctypes.CDLL(str(build.BENCH_LIB))
+    for name in declared:
+        assert hasattr(blib, name)
+    plib = ctypes.CDLL(str(build.LIB))
+    for name in declared + ["pn_measure_fp64_peak"]:
+        assert not hasattr(plib, name), f"{name} must not be part of the product library"
