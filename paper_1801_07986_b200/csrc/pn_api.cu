@@ -62,7 +62,8 @@ struct pn_ctx {
     StepParams* prm = nullptr;
     double *io_pos = nullptr, *io_vel = nullptr, *io_acc = nullptr;  // staging for the *_host entry points
     ERec* erec = nullptr;
-    FRec* frec = nullptr;  // two-float records of the fp32-pair variant, rebuilt before every pair launch
+    FRec* frec = nullptr;  // two-float records of the fp32-pair variant, rebuilt before every pair launch (tiled kernel)
+    FPair* fpair = nullptr;  // the same for pairs of consecutive stars: packed operands of the symmetric f32x2 kernel
     double *blk_prep = nullptr, *blk_pair = nullptr, *d_energy = nullptr;
     int e_split = 1;
 
@@ -201,33 +202,33 @@ cudaError_t prepare_sym()
     return e;
 }
 
-template <int I, int W, int MINB>
+template <int W, int MINB>
 cudaError_t prepare_sym32()
 {
-    const int bytes = kSymSmemBytes<I, W>;
-    cudaError_t e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<I, W, MINB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    const int bytes = kSym32SmemBytes<W>;
+    cudaError_t e = cudaFuncSetAttribute(pair_sym_fp32_kernel<W, MINB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<W, MINB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<W, MINB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pair_sym_fp32_kernel<W, MINB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     return e;
 }
 
-template <int I, int W, int MINB, bool MASK, bool EQM>
+template <int W, int MINB, bool MASK, bool EQM>
 void launch_pair_sym32_v(pn_ctx* c, cudaStream_t st)
 {
     const int items = c->sym_G * (c->sym_G + 1) / 2;
-    pair_sym_fp32_kernel<I, W, MINB, MASK, EQM><<<items, 32 * W, kSymSmemBytes<I, W>, st>>>(c->frec, c->part, c->np, c->sym_T, c->sym_m,
-                                                                                           (float)c->eps2, c->gm_eq);
+    pair_sym_fp32_kernel<W, MINB, MASK, EQM><<<items, 32 * W, kSym32SmemBytes<W>, st>>>(c->fpair, c->part, c->np, c->sym_T, c->sym_m,
+                                                                                      (float)c->eps2, c->gm_eq);
 }
 
-template <int I, int W, int MINB>
+template <int W, int MINB>
 void launch_pair_sym32(pn_ctx* c, cudaStream_t st)
 {
     const bool mask = (c->eps2 == 0.0), eqm = use_eqm(c);
     if (mask)
-        eqm ? launch_pair_sym32_v<I, W, MINB, true, true>(c, st) : launch_pair_sym32_v<I, W, MINB, true, false>(c, st);
+        eqm ? launch_pair_sym32_v<W, MINB, true, true>(c, st) : launch_pair_sym32_v<W, MINB, true, false>(c, st);
     else
-        eqm ? launch_pair_sym32_v<I, W, MINB, false, true>(c, st) : launch_pair_sym32_v<I, W, MINB, false, false>(c, st);
+        eqm ? launch_pair_sym32_v<W, MINB, false, true>(c, st) : launch_pair_sym32_v<W, MINB, false, false>(c, st);
 }
 
 template <int I, int W, int MINB, bool JS, bool MASK, bool EQM>
@@ -298,15 +299,18 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
             pair_cross_fp64_kernel<kCrossI, 2, kNT, kCrossTJ, false><<<grid, kNT, 0, st>>>(c->crec, c->bh[set], c->part6, c->np,
                                                                                           c->c_tiles_per_split, c->eps2, c->GM);
     } else if (c->precision == PN_FP32_PAIR) {
-        split_kernel<<<(c->np + 255) / 256, 256, 0, st>>>(c->jrec[set], c->frec, c->n_stars, c->np);
+        if (use_sym(c))
+            split_pair_kernel<<<(c->np + 255) / 256, 256, 0, st>>>(c->jrec[set], c->fpair, c->n_stars, c->np);
+        else
+            split_kernel<<<(c->np + 255) / 256, 256, 0, st>>>(c->jrec[set], c->frec, c->n_stars, c->np);
         PN_CUDA(c, cudaGetLastError());
         dim3 grid(c->n_itiles, c->n_split);
         const float e2 = (float)c->eps2;
         if (use_sym(c)) {
             if (c->sym_U == 128)
-                launch_pair_sym32<4, 1, 8>(c, st);
+                launch_pair_sym32<1, 8>(c, st);
             else
-                launch_pair_sym32<4, 4, 3>(c, st);
+                launch_pair_sym32<4, 3>(c, st);
         } else if (c->ipt == 2)
             mask ? pair_fp32_kernel<2, kNT, kTJ, 32, true><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2)
                  : pair_fp32_kernel<2, kNT, kTJ, 32, false><<<grid, kNT, 0, st>>>(c->frec, c->part, c->np, c->tiles_per_split, e2);
@@ -536,8 +540,8 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA((prepare_sym<4, 1, 12, false>()));
     CREATE_CUDA((prepare_sym<4, 4, 3, true>()));
     CREATE_CUDA((prepare_sym<4, 4, 2, false>()));
-    CREATE_CUDA((prepare_sym32<4, 1, 8>()));
-    CREATE_CUDA((prepare_sym32<4, 4, 3>()));
+    CREATE_CUDA((prepare_sym32<1, 8>()));
+    CREATE_CUDA((prepare_sym32<4, 3>()));
     CREATE_CUDA(dalloc(&ctx->part, (size_t)std::max(ctx->max_split, ctx->sym_G) * 3 * np));
     CREATE_CUDA(dalloc(&ctx->bh_part, 3 * (np / kEpiStars)));
     CREATE_CUDA(dalloc(&ctx->ticket, 1));
@@ -548,6 +552,7 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA(dalloc(&ctx->io_acc, 3 * (size_t)N));
     CREATE_CUDA(dalloc(&ctx->erec, np));
     CREATE_CUDA(dalloc(&ctx->frec, np));
+    CREATE_CUDA(dalloc(&ctx->fpair, np / 2));
     {
         const int n_it = (int)(np / kNT);
         // the energy pair kernel runs n_it / 2 mirrored i-tile pairs per j-split, all of equal work: aim at one full wave
@@ -595,7 +600,7 @@ int pn_destroy(pn_ctx* c)
     cudaFree(c->part), cudaFree(c->bh_part), cudaFree(c->ticket), cudaFree(c->prm);
     cudaFree(c->io_pos), cudaFree(c->io_vel), cudaFree(c->io_acc);
     cudaFree(c->crec), cudaFree(c->cblk), cudaFree(c->csum), cudaFree(c->part6), cudaFree(c->blk_mom);
-    cudaFree(c->frec), cudaFree(c->erec), cudaFree(c->blk_prep), cudaFree(c->blk_pair), cudaFree(c->d_energy);
+    cudaFree(c->frec), cudaFree(c->fpair), cudaFree(c->erec), cudaFree(c->blk_prep), cudaFree(c->blk_pair), cudaFree(c->d_energy);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     cudaGetLastError();
     if (prev >= 0 && prev != c->device) cudaSetDevice(prev);
