@@ -236,7 +236,7 @@ void launch_pair_sym_v(pn_ctx* c, int set, cudaStream_t st)
 {
     const int items = c->sym_G * (c->sym_G + 1) / 2;
     pair_sym_fp64_kernel<I, W, MINB, MASK, EQM, JS><<<items, 32 * W, kSymSmemBytes<I, W, JS>, st>>>(c->jrec[set], c->part, c->np, c->sym_T,
-                                                                                                   c->sym_m, c->eps2, c->gm_eq);
+                                                                                                   c->sym_m, c->eps2, c->gm_eq, 0);
 }
 
 template <int I, int W, int MINB, bool JS>
@@ -308,7 +308,7 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
         const float e2 = (float)c->eps2;
         if (use_sym(c)) {
             if (c->sym_U == 128)
-                launch_pair_sym32<1, 8>(c, st);
+                launch_pair_sym32<1, 12>(c, st);
             else
                 launch_pair_sym32<4, 3>(c, st);
         } else if (c->ipt == 2)
@@ -323,7 +323,7 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
         else if (c->sym_kind == SYM_W1_U128)
             launch_pair_sym<4, 1, 12, false>(c, set, st);
         else
-            launch_pair_sym<4, 4, 2, false>(c, set, st);
+            launch_pair_sym<4, 4, 3, false>(c, set, st);
     } else if (c->ipt == 2)
         mask ? launch_pair_fp64<2, 4, 4, true>(c, set, st) : launch_pair_fp64<2, 4, 4, false>(c, set, st);
     else
@@ -539,8 +539,8 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA(dalloc(&ctx->sv, 3 * np));
     CREATE_CUDA((prepare_sym<4, 1, 12, false>()));
     CREATE_CUDA((prepare_sym<4, 4, 3, true>()));
-    CREATE_CUDA((prepare_sym<4, 4, 2, false>()));
-    CREATE_CUDA((prepare_sym32<1, 8>()));
+    CREATE_CUDA((prepare_sym<4, 4, 3, false>()));
+    CREATE_CUDA((prepare_sym32<1, 12>()));
     CREATE_CUDA((prepare_sym32<4, 3>()));
     CREATE_CUDA(dalloc(&ctx->part, (size_t)std::max(ctx->max_split, ctx->sym_G) * 3 * np));
     CREATE_CUDA(dalloc(&ctx->bh_part, 3 * (np / kEpiStars)));

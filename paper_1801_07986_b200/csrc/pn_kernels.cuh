@@ -325,6 +325,53 @@ __device__ __forceinline__ void sym_unit_tile(const double2* __restrict__ sxy, c
     }
 }
 
+// Gray-code traversal of a rotation group (the default of the symmetric kernels): lane l meets j-star l ^ g(r) at step r,
+// g(r) = r ^ (r >> 1), so consecutive steps differ in ONE bit and the j-side sums move on with a butterfly shuffle whose
+// lane mask is an immediate (SHFL.BFLY: one register read, measured free next to the FP64 stream), where the rotation
+// (lane + r) mod 32 needs SHFL.IDX with the source lane in a register (two register reads: measured 1.9 FP64-pipe
+// cycles each on sm_100a, profiles/r2_ncu_summary.md section 2) and four integer instructions per step for the index.
+// The 32 steps are two identical halves of 16 (g(16 + q) = 24 ^ g(q); masks 1 2 1 4 1 2 1 8 1 2 1 4 1 2 1 16, the last
+// one brings the sums to the next half's first lane or, after step 31, home), so the unrolled body is 16 steps long and
+// every mask and every index offset in it is a compile-time constant.
+template <int I, int U, bool EQM, int STEPS>
+__device__ __forceinline__ void sym_unit_tile_gray(const double2* __restrict__ sxy, const double2* __restrict__ szm,
+                                                   double* __restrict__ cw, const double (&xi)[I], const double (&yi)[I],
+                                                   const double (&zi)[I], const double (&ngi)[I], double (&ax)[I],
+                                                   double (&ay)[I], double (&az)[I], double eps2, int lane, int jb0, int jb1)
+{
+    static_assert(STEPS == 8 || STEPS == 16, "unrolled steps of the Gray-code walk");
+#pragma unroll 1
+    for (int jb = jb0; jb < jb1; jb += 32) {
+        double bx = 0.0, by = 0.0, bz = 0.0;
+#pragma unroll 1
+        for (int c = 0; c < 32 / STEPS; ++c) {
+            // first j index of chunk c: l ^ g(STEPS c); g(8) = 12, g(16) = 24, g(24) = 20
+            const int off = (STEPS == 16) ? (c ? 24 : 0) : ((c & 1 ? 12 : 0) ^ (c & 2 ? 24 : 0));
+            const int base = jb + (lane ^ off);
+            // mask of the chunk's last move: g(STEPS c + STEPS - 1) ^ g(STEPS (c + 1)); 16 for both halves, 8 / 16 for quarters
+            const int last_mask = (STEPS == 16) ? 16 : ((c & 1) ? 16 : 8);
+#pragma unroll
+            for (int q = 0; q < STEPS; ++q) {
+                const int jj = base ^ (q ^ (q >> 1));
+                sym_step<I, true, false, EQM>(sxy[jj], szm[jj], xi, yi, zi, ngi, ax, ay, az, bx, by, bz, eps2, -1);
+                if (q + 1 < STEPS) {
+                    const int mask = (q + 1) & -(q + 1);  // lowest set bit of q + 1: the bit in which g(q) and g(q + 1) differ
+                    bx = __shfl_xor_sync(0xffffffffu, bx, mask);
+                    by = __shfl_xor_sync(0xffffffffu, by, mask);
+                    bz = __shfl_xor_sync(0xffffffffu, bz, mask);
+                } else {
+                    bx = __shfl_xor_sync(0xffffffffu, bx, last_mask);
+                    by = __shfl_xor_sync(0xffffffffu, by, last_mask);
+                    bz = __shfl_xor_sync(0xffffffffu, bz, last_mask);
+                }
+            }
+        }
+        cw[jb + lane] = bx;  // after 32 steps lane l holds the complete sums of j-star jb + l again
+        cw[U + jb + lane] = by;
+        cw[2 * U + jb + lane] = bz;
+    }
+}
+
 // triangular decode of a work-item index: (A <= B), id = B (B + 1) / 2 + A
 __device__ __forceinline__ void sym_decode_block(int id, int& A, int& B)
 {
@@ -376,16 +423,16 @@ constexpr int kSymSmemBytes = kSymU<I, W, JS> * (2 * 16 + W * 3 * 8);
 // block of the same U while the partial-sum slots stay those of U = 32 I: W times more, W times shorter work items for
 // the same slot layout -- this is what shortens the launch tail at N_s ~ 10^4.  The column sums
 // of a warp are complete for its 32 j-stars; the row sums of the W warps are added in fixed warp order at the flush.
-template <int I, int W, int MINB, bool MASK, bool EQM, bool JS = false, int UNR = 32 / I>
+template <int I, int W, int MINB, bool MASK, bool EQM, bool JS = false, int UNR = 32 / I, int TRAV = 16>
 __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp64_kernel(const JRec* __restrict__ jrec,
                                                                      double* __restrict__ part, int np, int n_tiles,
-                                                                     int m, double eps2, double gm_eq)
+                                                                     int m, double eps2, double gm_eq, int item0)
 {
     static_assert(!JS || W == I, "j-split form: one rotation group of the j tile per warp");
     constexpr int U = kSymU<I, W, JS>;
     constexpr int NT = W * 32;
     extern __shared__ double2 sym_smem[];  // kSymSmemBytes<I, W, JS>: dynamic, U = 512 needs more than 48 KB
-    const int item = blockIdx.x;
+    const int item = item0 + blockIdx.x;
     double2* sxy = sym_smem;                                                   // [U] x, y of the j tile
     double2* szm = sym_smem + U;                                               // [U] z, G m
     double(*cacc)[3][U] = reinterpret_cast<double(*)[3][U]>(sym_smem + 2 * U);  // [W][3][U] per-warp sums
@@ -422,7 +469,10 @@ __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp64_kernel(const JRec*
             if (ta == tb) {
                 sym_unit_tile<I, U, false, MASK, EQM, UNR>(sxy, szm, cw, xi, yi, zi, ngi, ax, ay, az, eps2, lane, i_local0, jb0, jb1);
             } else {
-                sym_unit_tile<I, U, true, false, EQM, UNR>(sxy, szm, cw, xi, yi, zi, ngi, ax, ay, az, eps2, lane, i_local0, jb0, jb1);
+                if (TRAV)
+                    sym_unit_tile_gray<I, U, EQM, TRAV ? TRAV : 16>(sxy, szm, cw, xi, yi, zi, ngi, ax, ay, az, eps2, lane, jb0, jb1);
+                else
+                    sym_unit_tile<I, U, true, false, EQM, UNR>(sxy, szm, cw, xi, yi, zi, ngi, ax, ay, az, eps2, lane, i_local0, jb0, jb1);
                 sym_sync<W>();
                 flush(A, tb, ta == ta0, JS ? 1 : W);  // column sums: the i-stars of tile ta acting on the j-stars of tile tb
             }
@@ -886,6 +936,68 @@ __device__ __forceinline__ void sym32_unit_tile(const Sym32Tile& tj, float* __re
     }
 }
 
+// the same unit tile walked in Gray-code order (see sym_unit_tile_gray): butterfly shuffles with immediate masks
+template <int U, bool EQM>
+__device__ __forceinline__ void sym32_unit_tile_gray(const Sym32Tile& tj, float* __restrict__ cw, const f32x2 (&xh)[2],
+                                                     const f32x2 (&yh)[2], const f32x2 (&zh)[2], const f32x2 (&xl)[2],
+                                                     const f32x2 (&yl)[2], const f32x2 (&zl)[2], const f32x2 (&ngi)[2],
+                                                     double (&ax)[4], double (&ay)[4], double (&az)[4], f32x2 eps2, int lane,
+                                                     int jb0, int jb1)
+{
+#pragma unroll 1
+    for (int jb = jb0; jb < jb1; jb += 32) {
+        f32x2 fx[2], fy[2], fz[2];
+#pragma unroll
+        for (int g = 0; g < 2; ++g) fx[g] = fy[g] = fz[g] = 0ull;
+        f32x2 bx = 0ull, by = 0ull, bz = 0ull;
+#pragma unroll 1
+        for (int c = 0; c < 2; ++c) {
+            const int base = jb + (lane ^ (c ? 24 : 0));
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                const int jj = base ^ (q ^ (q >> 1));
+                const ulonglong2 ja = tj.a[jj], jbv = tj.b[jj], jc = tj.c[jj];
+                f32x2 gmj = 0ull;
+                if (!EQM) gmj = tj.g[jj];
+#pragma unroll
+                for (int g = 0; g < 2; ++g) {
+                    const f32x2 dx = add2(sub2(ja.x, xh[g]), sub2(jbv.y, xl[g]));
+                    const f32x2 dy = add2(sub2(ja.y, yh[g]), sub2(jc.x, yl[g]));
+                    const f32x2 dz = add2(sub2(jbv.x, zh[g]), sub2(jc.y, zl[g]));
+                    const f32x2 r2 = fma2(dx, dx, fma2(dy, dy, fma2(dz, dz, eps2)));
+                    float r2a, r2b;
+                    unpack2(r2, r2a, r2b);
+                    const f32x2 y = pack2(rsqrt_seed_f32(r2a), rsqrt_seed_f32(r2b));
+                    const f32x2 K = mul2(mul2(y, y), y);
+                    const f32x2 sj = EQM ? K : mul2(K, gmj);
+                    fx[g] = fma2(sj, dx, fx[g]);
+                    fy[g] = fma2(sj, dy, fy[g]);
+                    fz[g] = fma2(sj, dz, fz[g]);
+                    const f32x2 si = EQM ? K : mul2(K, ngi[g]);
+                    bx = fma2(si, dx, bx);
+                    by = fma2(si, dy, by);
+                    bz = fma2(si, dz, bz);
+                }
+                const int mask = (q + 1 < 16) ? ((q + 1) & -(q + 1)) : 16;
+                bx = __shfl_xor_sync(0xffffffffu, bx, mask);
+                by = __shfl_xor_sync(0xffffffffu, by, mask);
+                bz = __shfl_xor_sync(0xffffffffu, bz, mask);
+            }
+        }
+#pragma unroll
+        for (int g = 0; g < 2; ++g) {
+            float lo, hi;
+            unpack2(fx[g], lo, hi), ax[2 * g] += (double)lo, ax[2 * g + 1] += (double)hi;
+            unpack2(fy[g], lo, hi), ay[2 * g] += (double)lo, ay[2 * g + 1] += (double)hi;
+            unpack2(fz[g], lo, hi), az[2 * g] += (double)lo, az[2 * g + 1] += (double)hi;
+        }
+        float lo, hi;
+        unpack2(bx, lo, hi), cw[jb + lane] = EQM ? -(lo + hi) : (lo + hi);
+        unpack2(by, lo, hi), cw[U + jb + lane] = EQM ? -(lo + hi) : (lo + hi);
+        unpack2(bz, lo, hi), cw[2 * U + jb + lane] = EQM ? -(lo + hi) : (lo + hi);
+    }
+}
+
 // column sums of the packed kernels: n_src per-warp [3][U] float tiles, added in fp64 in fixed warp order
 template <int U, int NT>
 __device__ __forceinline__ void sym32_flush_cols(const float* __restrict__ cw, double* __restrict__ dst, int np, bool first, int n_src,
@@ -905,7 +1017,7 @@ __device__ __forceinline__ void sym32_flush_cols(const float* __restrict__ cw, d
 template <int W>
 constexpr int kSym32SmemBytes = (W * 128) * (56 + 12 * W + 24);
 
-template <int W, int MINB, bool MASK, bool EQM>
+template <int W, int MINB, bool MASK, bool EQM, bool GRAY = true>
 __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp32_kernel(const FPair* __restrict__ fpair,
                                                                      double* __restrict__ part, int np, int n_tiles,
                                                                      int m, float eps2, double gm_eq)
@@ -959,7 +1071,10 @@ __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp32_kernel(const FPair
             if (ta == tb) {
                 sym32_unit_tile<U, false, MASK, EQM>(tj, cwf + w * 3 * U, xh, yh, zh, xl, yl, zl, ngi, ax, ay, az, eps2p, lane, i_local0, 0, U);
             } else {
-                sym32_unit_tile<U, true, false, EQM>(tj, cwf + w * 3 * U, xh, yh, zh, xl, yl, zl, ngi, ax, ay, az, eps2p, lane, i_local0, 0, U);
+                if (GRAY)
+                    sym32_unit_tile_gray<U, EQM>(tj, cwf + w * 3 * U, xh, yh, zh, xl, yl, zl, ngi, ax, ay, az, eps2p, lane, 0, U);
+                else
+                    sym32_unit_tile<U, true, false, EQM>(tj, cwf + w * 3 * U, xh, yh, zh, xl, yl, zl, ngi, ax, ay, az, eps2p, lane, i_local0, 0, U);
                 sym_sync<W>();
                 sym32_flush_cols<U, NT>(cwf, part + (size_t)A * 3 * np + (size_t)tb * U, np, ta == ta0, W, tid, scale);
             }
