@@ -50,6 +50,11 @@ struct pn_ctx {
     int ipt = 1, n_itiles = 0, n_tiles = 0, n_split = 1, tiles_per_split = 0, max_split = 1;
     // symmetric pair kernel: unit tile U = 32 W I stars, T unit tiles in G groups of m
     int sym_kind = 0, sym_I = 0, sym_W = 0, sym_U = 0, sym_T = 0, sym_m = 0, sym_G = 0;
+    // small-system path (small_path_kernel, one cooperative launch per pn_step / pn_accel call): i-stars per warp, blocks
+    int small_ok = 0, small_IW = 0, small_blocks = 0;
+    double* small_part = nullptr;      // [2][4 small_blocks][3] per-warp partials of a_1
+    unsigned int* small_bar = nullptr; // arrival counter of the grid barrier
+    unsigned int small_bar_base = 0;   // its value when the next launch starts
 
     // device buffers.  Two stage sets: [0] integrator state, [1] scratch for pn_accel.
     JRec* jrec[2] = {nullptr, nullptr};
@@ -167,7 +172,14 @@ bool use_sym(const pn_ctx* c)
     return c->n_stars >= 3072;
 }
 
-bool use_eqm(const pn_ctx* c) { return c->equal_mass && c->eqm_opt && use_sym(c); }
+// small systems: the whole call in one cooperative launch (fp64 hot path only; PN_PAIR_TILED / PN_PAIR_SYMMETRIC ask for
+// the multi-kernel path by name)
+bool use_small(const pn_ctx* c)
+{
+    return c->small_ok && c->kernel_opt == PN_PAIR_AUTO && c->precision == PN_FP64 && !c->cross;
+}
+
+bool use_eqm(const pn_ctx* c) { return c->equal_mass && c->eqm_opt && use_sym(c) && !use_small(c); }
 
 // kernels of the pair stage of one force evaluation (the epilogue is counted by the callers)
 int kernels_per_eval(const pn_ctx* c) { return c->cross ? 3 : (c->precision == PN_FP32_PAIR ? 2 : 1); }
@@ -180,6 +192,83 @@ void destroy_graphs(pn_ctx* c)
     if (c->graphB) cudaGraphExecDestroy(c->graphB), c->graphB = nullptr;
     if (c->graphT) cudaGraphExecDestroy(c->graphT), c->graphT = nullptr;
     if (c->graphT_src) cudaGraphDestroy(c->graphT_src), c->graphT_src = nullptr;
+}
+
+// ---- small-system path ------------------------------------------------------------------------------------------
+constexpr int kSmallMaxStars = 3071;
+constexpr int kSmallMaxIW = 6;
+
+template <int MODE, int IW, bool MASK>
+const void* small_kernel_ptr()
+{
+    constexpr int JU = IW == 1 ? 8 : (IW == 2 ? 4 : 2);
+    return reinterpret_cast<const void*>(small_path_kernel<MODE, IW, JU, MASK>);
+}
+
+template <int MODE>
+const void* small_kernel(int iw, bool mask)
+{
+    switch (iw) {
+        case 1: return mask ? small_kernel_ptr<MODE, 1, true>() : small_kernel_ptr<MODE, 1, false>();
+        case 2: return mask ? small_kernel_ptr<MODE, 2, true>() : small_kernel_ptr<MODE, 2, false>();
+        case 3: return mask ? small_kernel_ptr<MODE, 3, true>() : small_kernel_ptr<MODE, 3, false>();
+        case 4: return mask ? small_kernel_ptr<MODE, 4, true>() : small_kernel_ptr<MODE, 4, false>();
+        case 5: return mask ? small_kernel_ptr<MODE, 5, true>() : small_kernel_ptr<MODE, 5, false>();
+        default: return mask ? small_kernel_ptr<MODE, 6, true>() : small_kernel_ptr<MODE, 6, false>();
+    }
+}
+
+// one cooperative launch: mode MODE_RK4 runs nsteps classical RK4 steps on the integrator state (stage set 0, with stage
+// set 1 as the second position buffer), MODE_ACCEL one force evaluation on stage set 1
+int launch_small(pn_ctx* c, int mode, double dt, int64_t nsteps, double* acc_out)
+{
+    SmallArgs a;
+    const int set = (mode == MODE_RK4) ? 0 : 1;
+    a.jrec[0] = c->jrec[set], a.jrec[1] = c->jrec[1];
+    a.v = c->v[set];
+    a.x0 = c->x0, a.v0 = c->v0, a.sx = c->sx, a.sv = c->sv;
+    a.bh = c->bh[set];
+    a.bh_part = c->small_part;
+    a.bar = c->small_bar;
+    a.acc_out = acc_out;
+    a.n_stars = c->n_stars, a.np = c->np;
+    a.GM = c->GM, a.inv_c2 = c->inv_c2, a.eps2 = c->eps2, a.dt = dt;
+    a.nsteps = nsteps;
+    a.bar_base = c->small_bar_base;
+    const bool mask = (c->eps2 == 0.0);
+    const void* fn = (mode == MODE_RK4) ? small_kernel<MODE_RK4>(c->small_IW, mask) : small_kernel<MODE_ACCEL>(c->small_IW, mask);
+    const size_t smem = (size_t)c->np * sizeof(JRec);
+    void* args[] = {&a};
+    PN_CUDA(c, cudaLaunchCooperativeKernel(fn, dim3(c->small_blocks), dim3(kSmallNT), args, smem, c->stream));
+    const int64_t n_eval = (mode == MODE_RK4) ? 4 * nsteps : 1;
+    c->small_bar_base += (unsigned int)((uint64_t)n_eval * (uint64_t)c->small_blocks);  // modulo 2^32, like the counter
+    return PN_OK;
+}
+
+// sizes the small-system path and checks that the device can run it (cooperative launch, shared memory, residency)
+cudaError_t prepare_small(pn_ctx* c)
+{
+    c->small_ok = 0;
+    if (c->n_stars > kSmallMaxStars) return cudaSuccess;
+    int coop = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device);
+    if (e != cudaSuccess || !coop) return e;
+    const int warps = 4 * c->n_sm;
+    c->small_IW = std::min(kSmallMaxIW, std::max(1, (c->n_stars + warps - 1) / warps));
+    c->small_blocks = (c->n_stars + 4 * c->small_IW - 1) / (4 * c->small_IW);
+    if (c->small_blocks > c->n_sm) return cudaSuccess;  // one block per SM: every block must be resident
+    const int smem = c->np * (int)sizeof(JRec);
+    for (int mode = 0; mode < 2; ++mode)
+        for (int mask = 0; mask < 2; ++mask) {
+            const void* fn = mode ? small_kernel<MODE_RK4>(c->small_IW, mask != 0) : small_kernel<MODE_ACCEL>(c->small_IW, mask != 0);
+            e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            if (e != cudaSuccess) return e;
+        }
+    e = dalloc(&c->small_part, 2 * 3 * (size_t)4 * c->small_blocks);
+    if (e == cudaSuccess) e = dalloc(&c->small_bar, 1);
+    if (e == cudaSuccess) e = cudaMemset(c->small_bar, 0, sizeof(unsigned int));
+    if (e == cudaSuccess) c->small_ok = 1;
+    return e;
 }
 
 // ---- launches ---------------------------------------------------------------------------------------------
@@ -542,6 +631,7 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA((prepare_sym<4, 4, 3, false>()));
     CREATE_CUDA((prepare_sym32<1, 12>()));
     CREATE_CUDA((prepare_sym32<4, 3>()));
+    CREATE_CUDA(prepare_small(ctx));
     CREATE_CUDA(dalloc(&ctx->part, (size_t)std::max(ctx->max_split, ctx->sym_G) * 3 * np));
     CREATE_CUDA(dalloc(&ctx->bh_part, 3 * (np / kEpiStars)));
     CREATE_CUDA(dalloc(&ctx->ticket, 1));
@@ -600,6 +690,7 @@ int pn_destroy(pn_ctx* c)
     cudaFree(c->part), cudaFree(c->bh_part), cudaFree(c->ticket), cudaFree(c->prm);
     cudaFree(c->io_pos), cudaFree(c->io_vel), cudaFree(c->io_acc);
     cudaFree(c->crec), cudaFree(c->cblk), cudaFree(c->csum), cudaFree(c->part6), cudaFree(c->blk_mom);
+    cudaFree(c->small_part), cudaFree(c->small_bar);
     cudaFree(c->frec), cudaFree(c->fpair), cudaFree(c->erec), cudaFree(c->blk_prep), cudaFree(c->blk_pair), cudaFree(c->d_energy);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     cudaGetLastError();
@@ -733,6 +824,11 @@ int pn_accel(pn_ctx* c, const double* pos, const double* vel, double* acc)
     const int grid_pack = (c->n_stars + 255) / 256;
     pack_kernel<<<grid_pack, 256, 0, c->stream>>>(pos, vel, c->jrec[1], c->v[1], nullptr, nullptr, c->bh[1], c->n_stars, c->np, 0);
     PN_CUDA(c, cudaGetLastError());
+    if (use_small(c)) {
+        if (int rc = launch_small(c, MODE_ACCEL, 0.0, 0, acc)) return rc;
+        c->n_launch += 2;
+        return PN_OK;
+    }
     if (int rc = launch_pair(c, 1, c->stream, c->time_pair != 0)) return rc;
     const EpiArgs a = epi_args(c, 1, acc);
     if (c->cross & PN_CROSS_BH)
@@ -766,6 +862,11 @@ int pn_step(pn_ctx* c, double dt, int64_t nsteps)
     if (nsteps < 0) return fail(c, PN_EINVAL, "pn_step: nsteps must be >= 0");
     if (!c->have_state) return fail(c, PN_ESTATE, "pn_step: no state set (call pn_set_state first)");
     if (nsteps == 0) return PN_OK;
+    if (use_small(c)) {  // every stage of every step in one cooperative launch (PN_OPT_USE_GRAPH / PN_OPT_TIME_PAIR do not apply)
+        if (int rc = launch_small(c, MODE_RK4, dt, nsteps, nullptr)) return rc;
+        c->n_launch += 1;
+        return PN_OK;
+    }
     if (!(dt == c->dt_dev)) {
         StepParams p;
         p.dt = dt;
@@ -885,6 +986,10 @@ int pn_get_pair_config(pn_ctx* c, int32_t* cfg)
 {
     if (int rc = check_ctx(c)) return rc;
     if (!cfg) return fail(c, PN_EINVAL, "pn_get_pair_config: null pointer");
+    if (use_small(c)) {
+        cfg[0] = kSmallNT, cfg[1] = c->small_IW, cfg[2] = 32, cfg[3] = 1, cfg[4] = c->small_blocks, cfg[5] = c->np, cfg[6] = 15, cfg[7] = 7;
+        return PN_OK;
+    }
     if (c->cross) {
         cfg[0] = kNT, cfg[1] = kCrossI, cfg[2] = kCrossTJ, cfg[3] = c->c_split;
         cfg[4] = (c->np / (kCrossI * kNT)) * c->c_split, cfg[5] = c->np;

@@ -74,14 +74,14 @@ __device__ __forceinline__ double rsqrt_seed(double x)
 // is hidden inside the warp and consecutive instructions share operands (x_j, g15, g1875, gm, s) in the same
 // slot, which the operand-reuse cache needs (a DFMA with three distinct register operands costs 3 issue cycles
 // on sm_100a instead of 2 -- measured).
-template <int I, int JU, bool MASK>
+template <int I, int JU, bool MASK, int JSTR = 1>
 __device__ __forceinline__ void pairs_fp64(const JRec* __restrict__ tile, int jj, int jglob, const double (&xi)[I],
                                            const double (&yi)[I], const double (&zi)[I], const int (&ii)[I],
                                            double (&ax)[I], double (&ay)[I], double (&az)[I], double eps2)
 {
     JRec r[JU];
 #pragma unroll
-    for (int u = 0; u < JU; ++u) r[u] = tile[jj + u];
+    for (int u = 0; u < JU; ++u) r[u] = tile[jj + u * JSTR];  // JSTR = 32: the lanes of a warp share out the j-stars
     double dx[JU][I], dy[JU][I], dz[JU][I], r2[JU][I], y0[JU][I], t[JU][I], e[JU][I], s[JU][I];
 #pragma unroll
     for (int u = 0; u < JU; ++u)
@@ -131,7 +131,7 @@ __device__ __forceinline__ void pairs_fp64(const JRec* __restrict__ tile, int jj
 #pragma unroll
         for (int k = 0; k < I; ++k) {
             s[u][k] = s[u][k] * t[u][k];  // G m_j / rho^3
-            if (MASK) s[u][k] = (jglob + u == ii[k]) ? 0.0 : s[u][k];
+            if (MASK) s[u][k] = (jglob + u * JSTR == ii[k]) ? 0.0 : s[u][k];
         }
 #pragma unroll
     for (int u = 0; u < JU; ++u)
@@ -1333,6 +1333,261 @@ __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
                     bh->xs[k] = bh->x0[k] + hh * kx;
                     bh->vs[k] = bh->v0[k] + hh * kv;
                 }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// S1 - S4 for small systems (N_s < 3072, where a force evaluation is a few microseconds of arithmetic and the multi-kernel
+// path is bound by launch latency): ONE cooperative launch runs a whole pn_step call (every stage of every RK4 step) or
+// one pn_accel.  Each warp of the grid owns IW consecutive i-stars for the whole launch; its lanes share out the j-stars
+// (lane l takes j = l, l + 32, ...: every ordered pair, the 15-instruction form of pair_fp64_kernel), a butterfly
+// reduction gives every lane the complete sums, and lane k < IW then does the per-star physics of star k (S2, S3) and its
+// RK4 stage update (S4) with that star's step state held in registers.  What the other blocks need of an evaluation --
+// the new stage positions and one a_1 partial per warp -- goes through global memory, followed by one grid-wide barrier
+// per evaluation (an atomic arrival counter; the launch is cooperative, so every block is resident).  After the barrier
+// every block copies the stage records into its shared memory and forms a_1 from the per-warp partials in the same fixed
+// order (so every block integrates the massive object identically); block 0 writes its state back at the end.
+// Every sum has a fixed order: results are bit-reproducible.
+// ---------------------------------------------------------------------------------------------------------
+struct SmallArgs {
+    JRec* jrec[2];       // stage records: evaluation e reads set e & 1 and writes the next stage positions into the other
+    double* v;           // [3][np] stage velocity
+    double *x0, *v0, *sx, *sv;
+    BhState* bh;
+    double* bh_part;     // [2][warps of the grid][3]: evaluation e writes set e & 1
+    unsigned int* bar;   // arrival counter of the grid barrier (monotonic; bar_base = its value at launch)
+    double* acc_out;     // MODE_ACCEL: [N][3]
+    int n_stars, np;
+    double GM, inv_c2, eps2, dt;
+    long long nsteps;
+    unsigned int bar_base;
+};
+
+// TMA bulk copy (cp.async.bulk, global -> shared, completion on an mbarrier): one thread moves a whole contiguous array
+// into shared memory without staging it through registers; the data comes from L2, never from a stale L1 line
+__device__ __forceinline__ unsigned int smem_u32(const void* p) { return (unsigned int)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_copy_g2s(void* dst_smem, const void* src_gmem, unsigned int bytes, unsigned long long* bar)
+{
+    asm volatile("fence.proxy.async;" ::: "memory");  // earlier generic-proxy accesses are ordered before the async-proxy copy
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned int parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tMBAR_WAIT:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@!p bra MBAR_WAIT;\n\t}" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+
+constexpr int kSmallNT = 128;  // threads per block of small_path_kernel (one warp per SM sub-partition)
+
+__device__ __forceinline__ void small_grid_barrier(unsigned int* ctr, unsigned int target)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();  // this block's global writes are visible before its arrival is
+        atomicAdd(ctr, 1u);
+        unsigned int seen;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(ctr) : "memory");
+        } while ((int)(seen - target) < 0);
+    }
+    __syncthreads();
+}
+
+template <int MODE, int IW, int JU, bool MASK>
+__global__ void __launch_bounds__(kSmallNT, 1) small_path_kernel(SmallArgs A)
+{
+    extern __shared__ double2 small_smem[];              // JRec[np]: this block's copy of the stage records
+    JRec* sj = reinterpret_cast<JRec*>(small_smem);
+    __shared__ double red[3 * (kSmallNT / 32)];
+    __shared__ BhState sbh;
+    __shared__ __align__(8) unsigned long long fill_bar;  // completion of the bulk copy of the stage records
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int np = A.np;
+    const int gw = blockIdx.x * (kSmallNT / 32) + w;     // warp of the grid
+    const int i0 = gw * IW;                              // its first i-star
+    const int my = i0 + lane;                            // lane k < IW owns star i0 + k
+    const bool own = (lane < IW) && (my < A.n_stars);
+    unsigned int target = A.bar_base;
+
+    double x0[3] = {0, 0, 0}, v0[3] = {0, 0, 0}, vs[3] = {0, 0, 0}, sx[3] = {0, 0, 0}, sv[3] = {0, 0, 0}, gm_me = 0;
+    if (own) {
+        gm_me = A.jrec[0][my].gm;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const size_t q = (size_t)k * np + my;
+            vs[k] = A.v[q];
+            if (MODE == MODE_RK4) x0[k] = A.x0[q], v0[k] = A.v0[q], sx[k] = A.sx[q], sv[k] = A.sv[q];
+        }
+    }
+    if (tid == 0) {
+        sbh = *A.bh;
+        mbar_init(&fill_bar, 1);
+    }
+    __syncthreads();
+
+    // a_1 of an evaluation from the per-warp partials (fixed order), then the massive object's RK4 stage update
+    const int n_part = (int)gridDim.x * (kSmallNT / 32);
+    auto finish_bh = [&](long long e) {  // e: the evaluation whose a_1 is formed
+        const int stage = (int)(e & 3);
+        const double* part = A.bh_part + (size_t)(e & 1) * 3 * n_part;
+        double c0 = 0, c1 = 0, c2 = 0;
+        for (int q = tid; q < n_part; q += kSmallNT) {
+            c0 += __ldcg(part + 3 * q), c1 += __ldcg(part + 3 * q + 1), c2 += __ldcg(part + 3 * q + 2);
+        }
+        __syncthreads();  // red is free again
+        block_sum3<kSmallNT>(c0, c1, c2, red);
+        if (tid == 0) {
+            const double a1[3] = {c0, c1, c2};
+            if (MODE == MODE_ACCEL) {
+                if (blockIdx.x == 0) A.acc_out[0] = a1[0], A.acc_out[1] = a1[1], A.acc_out[2] = a1[2];
+            } else {
+                const double dt = A.dt, hh = (stage == 2) ? dt : 0.5 * dt;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const double kx = sbh.vs[k], kv = a1[k];
+                    if (stage == 3) {
+                        sbh.x0[k] += dt / 6.0 * (sbh.sx[k] + kx);
+                        sbh.v0[k] += dt / 6.0 * (sbh.sv[k] + kv);
+                        sbh.xs[k] = sbh.x0[k], sbh.vs[k] = sbh.v0[k];
+                    } else {
+                        if (stage == 0) {
+                            sbh.sx[k] = kx, sbh.sv[k] = kv;
+                        } else {
+                            sbh.sx[k] += 2.0 * kx, sbh.sv[k] += 2.0 * kv;
+                        }
+                        sbh.xs[k] = sbh.x0[k] + hh * kx;
+                        sbh.vs[k] = sbh.v0[k] + hh * kv;
+                    }
+                }
+            }
+        }
+    };
+
+    const long long n_eval = (MODE == MODE_RK4) ? 4 * A.nsteps : 1;
+    for (long long ev = 0; ev < n_eval; ++ev) {
+        const int stage = (int)(ev & 3);
+        // (A) the stage records of all stars -> shared memory: one TMA bulk copy (other blocks wrote them before the barrier)
+        if (tid == 0) bulk_copy_g2s(small_smem, A.jrec[ev & 1], (unsigned int)(np * sizeof(JRec)), &fill_bar);
+        // (B) meanwhile, the massive object's stage state: a_1 of the previous evaluation
+        if (ev > 0) finish_bh(ev - 1);
+        mbar_wait(&fill_bar, (unsigned int)(ev & 1));
+        __syncthreads();
+
+        // (C) every ordered pair (i, j) of this warp's IW i-stars: lane l takes j = l + 32 q
+        double xi[IW], yi[IW], zi[IW], ax[IW], ay[IW], az[IW];
+        int ii[IW];
+#pragma unroll
+        for (int k = 0; k < IW; ++k) {
+            ii[k] = i0 + k;
+            const JRec* pi = sj + min(ii[k], np - 1);  // beyond the padded range: a pad star, result unused
+            xi[k] = pi->x, yi[k] = pi->y, zi[k] = pi->z;
+            ax[k] = ay[k] = az[k] = 0.0;
+        }
+#pragma unroll 1
+        for (int jq = lane; jq < np; jq += 32 * JU) pairs_fp64<IW, JU, MASK, 32>(sj, jq, jq, xi, yi, zi, ii, ax, ay, az, A.eps2);
+        double s0 = 0, s1 = 0, s2 = 0;
+#pragma unroll
+        for (int k = 0; k < IW; ++k) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                ax[k] += __shfl_xor_sync(0xffffffffu, ax[k], o);
+                ay[k] += __shfl_xor_sync(0xffffffffu, ay[k], o);
+                az[k] += __shfl_xor_sync(0xffffffffu, az[k], o);
+            }
+            if (lane == k) s0 = ax[k], s1 = ay[k], s2 = az[k];
+        }
+
+        // S2 + S3 + S4 for the lane's own star (same formulas as epilogue_kernel)
+        double b0 = 0, b1 = 0, b2 = 0;
+        if (own) {
+            const JRec rec = sj[my];
+            const double x[3] = {rec.x - sbh.xs[0], rec.y - sbh.xs[1], rec.z - sbh.xs[2]};  // x_i1 = x_i - x_1
+            const double r2 = x[0] * x[0] + x[1] * x[1] + x[2] * x[2];
+            const double r = sqrt(r2);
+            const double inv_r = 1.0 / r;
+            const double inv_r3 = inv_r * inv_r * inv_r;
+            const double v2 = vs[0] * vs[0] + vs[1] * vs[1] + vs[2] * vs[2];
+            const double vx = vs[0] * x[0] + vs[1] * x[1] + vs[2] * x[2];
+            const double GMr = A.GM * inv_r;
+            const double cs = A.GM * inv_r3;
+            const double fx = -1.0 + A.inv_c2 * (4.0 * GMr - v2);
+            const double fv = A.inv_c2 * 4.0 * vx;
+            const double cb = gm_me * inv_r3;
+            const double gx = 1.0 - A.inv_c2 * (5.0 * GMr - 2.0 * v2 + 1.5 * vx * vx * inv_r * inv_r);
+            const double gv = -A.inv_c2 * 3.0 * vx;
+            const double ss[3] = {s0, s1, s2};
+            double a[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) a[k] = ss[k] + cs * (fx * x[k] + fv * vs[k]);
+            b0 = cb * (gx * x[0] + gv * vs[0]);
+            b1 = cb * (gx * x[1] + gv * vs[1]);
+            b2 = cb * (gx * x[2] + gv * vs[2]);
+            if (MODE == MODE_ACCEL) {
+                double* o = A.acc_out + 3 * (size_t)(my + 1);
+                o[0] = a[0], o[1] = a[1], o[2] = a[2];
+            } else {
+                const double dt = A.dt, hh = (stage == 2) ? dt : 0.5 * dt;
+                double xn[3];
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const double kx = vs[k], kv = a[k];
+                    if (stage == 3) {
+                        x0[k] = x0[k] + dt / 6.0 * (sx[k] + kx);
+                        v0[k] = v0[k] + dt / 6.0 * (sv[k] + kv);
+                        xn[k] = x0[k], vs[k] = v0[k];
+                    } else {
+                        if (stage == 0) {
+                            sx[k] = kx, sv[k] = kv;
+                        } else {
+                            sx[k] += 2.0 * kx, sv[k] += 2.0 * kv;
+                        }
+                        xn[k] = x0[k] + hh * kx;
+                        vs[k] = v0[k] + hh * kv;
+                    }
+                }
+                JRec* g = A.jrec[(ev + 1) & 1] + my;  // the next evaluation's stage position, for every block
+                g->x = xn[0], g->y = xn[1], g->z = xn[2];
+            }
+        }
+        // this warp's a_1 partial: its stars in index order
+        {
+            double p0 = 0, p1 = 0, p2 = 0;
+#pragma unroll
+            for (int k = 0; k < IW; ++k) {
+                p0 += __shfl_sync(0xffffffffu, b0, k);
+                p1 += __shfl_sync(0xffffffffu, b1, k);
+                p2 += __shfl_sync(0xffffffffu, b2, k);
+            }
+            if (lane == 0) {
+                double* bp = A.bh_part + (size_t)(ev & 1) * 3 * n_part + 3 * (size_t)gw;
+                bp[0] = p0, bp[1] = p1, bp[2] = p2;
+            }
+        }
+        // (D) everything of this evaluation is in global memory before anyone starts the next one
+        target += gridDim.x;
+        small_grid_barrier(A.bar, target);
+    }
+    finish_bh(n_eval - 1);
+    __syncthreads();
+    if (MODE == MODE_RK4) {
+        if (blockIdx.x == 0 && tid == 0) *A.bh = sbh;
+        if (own) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const size_t q = (size_t)k * np + my;
+                A.v[q] = vs[k], A.x0[q] = x0[k], A.v0[q] = v0[k], A.sx[q] = sx[k], A.sv[q] = sv[k];
             }
         }
     }

@@ -109,15 +109,17 @@ def test_accel_parity_both_pair_kernels(n_stars, kernel):
 def test_pair_kernels_agree_and_auto_selection():
     from paper_1801_07986_b200 import binding
 
-    for n_stars, want in ((3071, 0), (3072, 4)):
+    for n_stars, want in ((3071, 7), (3072, 4)):  # 7: the one-launch small-system path (N_s < 3072)
         p = inputs.plummer_bh(n_stars, seed=12)
         with _pn(p) as pn:
             assert pn.pn_get_pair_config()["variant"] == want
-            acc = {}
+            acc = {binding.PN_PAIR_AUTO: _gpu_accel(pn, p.pos, p.vel)}
             for k in (binding.PN_PAIR_TILED, binding.PN_PAIR_SYMMETRIC):
                 pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, k)
+                assert pn.pn_get_pair_config()["variant"] == (0 if k == binding.PN_PAIR_TILED else 4)
                 acc[k] = _gpu_accel(pn, p.pos, p.vel)
             assert rel_err_rows(acc[binding.PN_PAIR_SYMMETRIC], acc[binding.PN_PAIR_TILED]).max() <= 1e-13
+            assert rel_err_rows(acc[binding.PN_PAIR_AUTO], acc[binding.PN_PAIR_TILED]).max() <= 1e-13
             with pytest.raises(binding.PNError):
                 pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, 7)
 
@@ -262,13 +264,18 @@ def test_config3_like_cusp_trajectory_and_energy_drift():
     print(f"cusp 4095: oracle drift after 20 steps {drift_ref:.3e}, worst trajectory error {worst_traj:.2e}")
 
 
-def test_step_graph_and_plain_launches_agree_bitwise():
+@pytest.mark.parametrize("kernel", ["auto", "tiled"])
+def test_step_graph_and_plain_launches_agree_bitwise(kernel):
+    """auto: N_s = 2500 takes the small-system path (one cooperative launch, PN_OPT_USE_GRAPH does not apply);
+    tiled: the multi-kernel path, as a 16-step batched graph + 3 single-step graphs against plain launches."""
     from paper_1801_07986_b200 import binding
 
     p = inputs.plummer_bh(2500, seed=12, dt=1e-3)
     out = []
     for use_graph in (1, 0):
         with _pn(p) as pn:
+            if kernel == "tiled":
+                pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, binding.PN_PAIR_TILED)
             pn.pn_set_option(binding.PN_OPT_USE_GRAPH, use_graph)
             pn.pn_set_state(_dev(p.pos), _dev(p.vel))
             pn.pn_step(p.dt, 19)  # 16-step batched graph + 3 single-step graphs
