@@ -35,9 +35,11 @@ if str(ROOT) not in sys.path:
 #     multiplications go: 3 DADD + 12 DFMA + 3 DMUL = 18 per unordered pair = 9 per ordered pair
 #   5 ordered pairs with the Cross terms of Eq. 2.6 (--cross): 36 DADD + 124 DFMA + 56 DMUL per 4 pairs = 54 per ordered pair
 #   6 the same plus the O(N^2) sum of Eq. 2.3 (--cross full): 59 per ordered pair
+#   7 small-system path (N_s < 3072): ONE cooperative launch per pn_step / pn_accel call, every ordered pair in the tiled
+#     kernel's 15-instruction form; there is no separate pair stage to time, the launch is the whole call
 PAIR_KERNELS = {0: ("pair_fp64_kernel", 15, 24.0), 2: ("pair_sym_fp64_kernel", 10, 16.0),
                 4: ("pair_sym_fp64_kernel<EQM>", 9, 15.0), 5: ("pair_cross_fp64_kernel", 54, 85.0),
-                6: ("pair_cross_fp64_kernel<BHX>", 59, 93.0)}
+                6: ("pair_cross_fp64_kernel<BHX>", 59, 93.0), 7: ("small_path_kernel", 15, 24.0)}
 SMS, FP64_LANES_PER_SM = 148, 64
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed `ncu --set full`
 # captures (per launch, cold L2: ncu flushes the caches before every replay), keyed by (variant, N_s); each entry names the
@@ -458,7 +460,10 @@ def run_ours(args) -> None:
         pair_avg_ms = pair_ms / max(1, pair_n)
         kname, instr, exec_flops = PAIR_KERNELS[cfg["variant"]]
         assert instr == cfg["fp64_instr_per_pair"]
-        kernel_pairs_per_s = p.pairs_per_eval / (pair_avg_ms * 1e-3) if pair_n else None
+        pairs_per_launch = p.pairs_per_eval
+        if cfg["variant"] == 7:  # one launch = one whole RK4 step (4 force evaluations): its time is the step's
+            pair_avg_ms, pair_n, pairs_per_launch = ms_steps / K, K, 4 * p.pairs_per_eval
+        kernel_pairs_per_s = pairs_per_launch / (pair_avg_ms * 1e-3) if pair_n else None
         achieved = kernel_pairs_per_s * 2 * instr / 1e12 if pair_n else None
         roof = {
             "bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
@@ -469,8 +474,9 @@ def run_ours(args) -> None:
             "convention": f"{instr} FP64-pipe instructions per ordered pair in the shipped SASS, each counted as an "
                           f"FMA (2 flops) = FP64-pipe issue-slot utilisation; peak = {SMS} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x "
                           f"{sm_max:.0f} MHz (clocks.max.sm; no measured fp64 peak in MEASURED_PEAKS.json)",
-            "pairs_per_launch": p.pairs_per_eval, "avg_launch_ms": pair_avg_ms, "launches_timed": pair_n,
-            "launches_in_timed_steps": 4 * K, "pair_kernel_share_of_steps": 4 * K * pair_avg_ms / ms_steps if ms_steps else None,
+            "pairs_per_launch": pairs_per_launch, "avg_launch_ms": pair_avg_ms, "launches_timed": pair_n,
+            "launches_in_timed_steps": K if cfg["variant"] == 7 else 4 * K,
+            "pair_kernel_share_of_steps": (1.0 if cfg["variant"] == 7 else 4 * K * pair_avg_ms / ms_steps) if ms_steps else None,
             "kernel_pairs_per_s": kernel_pairs_per_s,
             "frac_at_sampled_clock": (achieved / (peak_tflops * clocks["sm_mhz"] / sm_max)) if achieved and clocks.get("sm_mhz") else None,
             "executed_flops_frac": (kernel_pairs_per_s * exec_flops / 1e12 / peak_tflops) if achieved else None,
@@ -581,7 +587,7 @@ def run_sweep(args) -> None:
             torch.cuda.synchronize()
             ms = float(np.median([a.elapsed_time(b) for a, b in ev]))
             pair_ms, n = pn.pn_get_pair_time(reset=True)
-            pair_ms /= max(1, n)
+            pair_ms = pair_ms / n if n else ms  # small-system path: no separate pair stage, the evaluation is one launch
             tfl = p.pairs_per_eval * 2 * instr / (pair_ms * 1e-3) / 1e12
             print(json.dumps({
                 "workload": name, "N": p.N, "precision": pname, "pairs": p.pairs_per_eval, "accel_ms": ms,
