@@ -54,7 +54,8 @@ extern "C" {
 
 /* pn_set_option keys */
 #define PN_OPT_PAIR_PRECISION 1 /* PN_FP64 (default) | PN_FP32_PAIR: arithmetic of the O(N^2) star-star pair loop */
-#define PN_OPT_USE_GRAPH 2      /* 1 (default): pn_step replays a captured CUDA graph; 0: plain launches */
+#define PN_OPT_USE_GRAPH 2      /* 1 (default): pn_step replays a captured CUDA graph; 0: plain launches (neither applies to
+                                   the small-system path, see PN_PAIR_AUTO: that is one cooperative launch per call) */
 #define PN_OPT_TIME_PAIR 3      /* 1: bracket the pair stage of every force evaluation with CUDA events (pn_step: event-record
                                    nodes inside a one-step CUDA graph; plain launches when PN_OPT_USE_GRAPH is 0); read with
                                    pn_get_pair_time.  2: as 1, but in pn_step only the first of the four force evaluations
@@ -69,13 +70,15 @@ extern "C" {
 
 #define PN_OPT_CROSS_TERMS 7    /* 0 (default): the hot path of north_star; PN_CROSS_STAR: add [a_i]_Cross, Eq. 2.6
                                    (PAPER.md:70-86), to every star's acceleration -- the first NEXT row of the scope table:
-                                   its O(N^2) sums are fused into an fp64 ordered-pair kernel that also produces the
-                                   Newtonian star-star term (54 FP64 instructions per ordered pair), its O(N) parts go into
-                                   the epilogue.  PN_CROSS_STAR | PN_CROSS_BH: also [a_1]_Cross, Eq. 2.3, the
-                                   second NEXT row -- the paper's full limited-1PN force (one more O(N^2) sum per star in the
-                                   same kernel, 59 instructions per pair; the rest is O(N)).  Applies to pn_accel and
-                                   pn_step; pn_energy is Eq. 2.7 either way.  The Cross path is fp64 only: while it is on,
-                                   PN_OPT_PAIR_PRECISION, PN_OPT_PAIR_KERNEL and PN_OPT_EQUAL_MASS have no effect. */
+                                   its O(N^2) sums are fused into an fp64 pair kernel that also produces the Newtonian
+                                   star-star term, its O(N) parts go into the epilogue.  From 6144 stars on that kernel
+                                   evaluates every UNORDERED pair once for both stars (38 FP64 instructions per ordered
+                                   pair), below every ordered pair (54); PN_OPT_PAIR_KERNEL = PN_PAIR_SYMMETRIC /
+                                   PN_PAIR_TILED forces either.  PN_CROSS_STAR | PN_CROSS_BH: also [a_1]_Cross, Eq. 2.3
+                                   (PAPER.md:51-57), the second NEXT row -- the paper's full limited-1PN force (one more
+                                   O(N^2) sum per star in the same kernel, 42 / 59 instructions per pair; the rest is O(N)).
+                                   Applies to pn_accel and pn_step; pn_energy is Eq. 2.7 either way.  The Cross path is fp64
+                                   only: while it is on, PN_OPT_PAIR_PRECISION and PN_OPT_EQUAL_MASS have no effect. */
 #define PN_CROSS_STAR 1
 #define PN_CROSS_BH 2
 
@@ -84,7 +87,10 @@ extern "C" {
 #define PN_FP32_PAIR 1 /* fp32 pair arithmetic on two-float positions, fp64 accumulation (parity 1e-5) */
 
 /* PN_OPT_PAIR_KERNEL values (either pair precision) */
-#define PN_PAIR_AUTO 0      /* symmetric for N - 1 >= 3072 stars (unit tiles of 128 stars, 512 from 40000 stars on), tiled below */
+#define PN_PAIR_AUTO 0      /* symmetric for N - 1 >= 3072 stars (unit tiles of 128 stars, 512 from 40000 stars on).  Below
+                               (fp64, no Cross terms): the small-system path -- ONE cooperative kernel launch runs a whole
+                               pn_step call (every stage of every step) or one pn_accel, every ordered pair, 15 instructions;
+                               it needs a device with cooperative launch and as many SMs as blocks (else: tiled) */
 #define PN_PAIR_TILED 1     /* every ordered pair (i, j): 15 FP64 (18 FP32) instructions per ordered pair */
 #define PN_PAIR_SYMMETRIC 2 /* every unordered pair once, applied to both stars (Newton's third law, exact for the
                                softened Newtonian term of Eq. 2.4): 10 FP64 (11 FP32) instructions per ordered pair */

@@ -20,7 +20,13 @@ constexpr int kNT = 128;        // threads per block of the pair / energy / epil
 constexpr int kTJ = 128;        // j records per shared-memory tile
 constexpr int kGraphBatch = 16; // RK4 steps captured in the batched graph
 constexpr int kCrossI = 2;      // i-stars per thread of pair_cross_fp64_kernel
-constexpr int kCrossTJ = 64;    // its j tile (96 B records)
+constexpr int kCrossTJ = 64;    // its j tile (112 B records)
+#ifndef PN_CROSS_SYM_MINB
+#define PN_CROSS_SYM_MINB 8
+#endif
+constexpr int kCrossSymMinB = PN_CROSS_SYM_MINB;  // one-warp blocks per SM of pair_cross_sym_kernel
+constexpr int kCrossSymMinStars = 6144; // below: the ordered-pair kernel (too few work items for the triangular grid)
+constexpr int kCrossSymMaxGroups = 128; // its partial-sum slots
 
 thread_local std::string g_create_error;
 
@@ -39,9 +45,10 @@ struct pn_ctx {
     // options
     int precision = PN_FP64, use_graph = 1, time_pair = 0, j_split_opt = 0, kernel_opt = PN_PAIR_AUTO, eqm_opt = 1;
     int cross = 0;            // PN_OPT_CROSS_TERMS mask
-    CRec* crec = nullptr;     // cross mode: per-star records, block partials and totals of the O(N) sums, 6-component partials
+    CRec* crec = nullptr;     // cross mode: per-star records, block partials and totals of the O(N) sums, 7/8-component partials
     double *cblk = nullptr, *csum = nullptr, *part6 = nullptr;
     int c_split = 1, c_tiles_per_split = 0;
+    int c_T = 0, c_m = 0, c_G = 0;  // symmetric Cross kernel: unit tiles of 64 stars in c_G groups of c_m
     double* blk_mom = nullptr;  // pn_momentum scratch
     bool equal_mass = false;  // every star has the same mass > 0
     double gm_eq = 0;
@@ -184,7 +191,13 @@ bool use_eqm(const pn_ctx* c) { return c->equal_mass && c->eqm_opt && use_sym(c)
 // kernels of the pair stage of one force evaluation (the epilogue is counted by the callers)
 int kernels_per_eval(const pn_ctx* c) { return c->cross ? 3 : (c->precision == PN_FP32_PAIR ? 2 : 1); }
 
-int active_split(const pn_ctx* c) { return c->cross ? c->c_split : (use_sym(c) ? c->sym_G : c->n_split); }
+// Cross terms: every unordered pair once from kCrossSymMinStars stars on (PN_PAIR_TILED / PN_PAIR_SYMMETRIC force either kernel)
+bool cross_sym(const pn_ctx* c)
+{
+    return c->kernel_opt == PN_PAIR_SYMMETRIC || (c->kernel_opt == PN_PAIR_AUTO && c->n_stars >= kCrossSymMinStars);
+}
+
+int active_split(const pn_ctx* c) { return c->cross ? (cross_sym(c) ? c->c_G : c->c_split) : (use_sym(c) ? c->sym_G : c->n_split); }
 
 void destroy_graphs(pn_ctx* c)
 {
@@ -378,15 +391,26 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
     const bool mask = (c->eps2 == 0.0);
     if (c->cross) {  // NEXT-1: star-star Newtonian + pair part of [a_i]_Cross in one ordered-pair pass (fp64)
         const int nb = c->np / kNT;
-        cross_prep_kernel<kNT><<<nb, kNT, 0, st>>>(c->jrec[set], c->v[set], c->bh[set], c->crec, c->cblk, c->n_stars, c->np);
+        cross_prep_kernel<kNT><<<nb, kNT, 0, st>>>(c->jrec[set], c->v[set], c->bh[set], c->crec, c->cblk, c->n_stars, c->np, c->GM);
         cross_sum_kernel<<<1, 256, 0, st>>>(c->cblk, nb, c->csum);
-        dim3 grid(c->np / (kCrossI * kNT), c->c_split);
-        if (c->cross & PN_CROSS_BH)
-            pair_cross_fp64_kernel<kCrossI, 2, kNT, kCrossTJ, true><<<grid, kNT, 0, st>>>(c->crec, c->bh[set], c->part6, c->np,
-                                                                                         c->c_tiles_per_split, c->eps2, c->GM);
-        else
-            pair_cross_fp64_kernel<kCrossI, 2, kNT, kCrossTJ, false><<<grid, kNT, 0, st>>>(c->crec, c->bh[set], c->part6, c->np,
-                                                                                          c->c_tiles_per_split, c->eps2, c->GM);
+        const double GM4 = 4.0 * c->GM;
+        if (cross_sym(c)) {  // every unordered pair once
+            const int items = c->c_G * (c->c_G + 1) / 2;
+            if (c->cross & PN_CROSS_BH)
+                pair_cross_sym_kernel<kCrossSymMinB, true><<<items, 32, kCrossSymSmemBytes<true>, st>>>(c->crec, c->part6, c->np, c->c_T, c->c_m,
+                                                                                                         c->eps2, GM4);
+            else
+                pair_cross_sym_kernel<kCrossSymMinB, false><<<items, 32, kCrossSymSmemBytes<false>, st>>>(c->crec, c->part6, c->np, c->c_T, c->c_m,
+                                                                                                           c->eps2, GM4);
+        } else {
+            dim3 grid(c->np / (kCrossI * kNT), c->c_split);
+            if (c->cross & PN_CROSS_BH)
+                pair_cross_fp64_kernel<kCrossI, 2, kNT, kCrossTJ, true><<<grid, kNT, 0, st>>>(c->crec, c->part6, c->np, c->c_tiles_per_split,
+                                                                                             c->eps2, GM4);
+            else
+                pair_cross_fp64_kernel<kCrossI, 2, kNT, kCrossTJ, false><<<grid, kNT, 0, st>>>(c->crec, c->part6, c->np, c->c_tiles_per_split,
+                                                                                              c->eps2, GM4);
+        }
     } else if (c->precision == PN_FP32_PAIR) {
         if (use_sym(c))
             split_pair_kernel<<<(c->np + 255) / 256, 256, 0, st>>>(c->jrec[set], c->fpair, c->n_stars, c->np);
@@ -733,6 +757,7 @@ int pn_set_option(pn_ctx* c, int key, int value)
         case PN_OPT_PAIR_KERNEL:
             if (value != PN_PAIR_AUTO && value != PN_PAIR_TILED && value != PN_PAIR_SYMMETRIC)
                 return fail(c, PN_EINVAL, "pn_set_option: unknown pair kernel %d", value);
+            if (value != c->kernel_opt) destroy_graphs(c);
             c->kernel_opt = value;
             return PN_OK;
         case PN_OPT_CROSS_TERMS: {
@@ -746,10 +771,15 @@ int pn_set_option(pn_ctx* c, int key, int value)
                 int s = std::max(1, std::min(std::min((c->n_sm * 16 + n_it - 1) / n_it, n_t), 64));
                 c->c_tiles_per_split = (n_t + s - 1) / s;
                 c->c_split = (n_t + c->c_tiles_per_split - 1) / c->c_tiles_per_split;
+                c->c_T = c->np / kCrossSymU;
+                c->c_m = (c->c_T + kCrossSymMaxGroups - 1) / kCrossSymMaxGroups;
+                c->c_G = (c->c_T + c->c_m - 1) / c->c_m;
+                PN_CUDA(c, cudaFuncSetAttribute(pair_cross_sym_kernel<kCrossSymMinB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCrossSymSmemBytes<true>));
+                PN_CUDA(c, cudaFuncSetAttribute(pair_cross_sym_kernel<kCrossSymMinB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCrossSymSmemBytes<false>));
                 PN_CUDA(c, dalloc(&c->crec, np));
                 PN_CUDA(c, dalloc(&c->cblk, (np / kNT) * kCrossSums));
                 PN_CUDA(c, dalloc(&c->csum, kCrossSums));
-                PN_CUDA(c, dalloc(&c->part6, (size_t)c->c_split * 7 * np));
+                PN_CUDA(c, dalloc(&c->part6, (size_t)std::max(c->c_split, c->c_G) * 8 * np));
             }
             c->cross = value;
             destroy_graphs(c);
@@ -988,6 +1018,12 @@ int pn_get_pair_config(pn_ctx* c, int32_t* cfg)
     if (!cfg) return fail(c, PN_EINVAL, "pn_get_pair_config: null pointer");
     if (use_small(c)) {
         cfg[0] = kSmallNT, cfg[1] = c->small_IW, cfg[2] = 32, cfg[3] = 1, cfg[4] = c->small_blocks, cfg[5] = c->np, cfg[6] = 15, cfg[7] = 7;
+        return PN_OK;
+    }
+    if (c->cross && cross_sym(c)) {
+        cfg[0] = 32, cfg[1] = kCrossSymI, cfg[2] = kCrossSymU, cfg[3] = c->c_G;
+        cfg[4] = c->c_G * (c->c_G + 1) / 2, cfg[5] = c->np;
+        cfg[6] = (c->cross & PN_CROSS_BH) ? 42 : 38, cfg[7] = (c->cross & PN_CROSS_BH) ? 9 : 8;
         return PN_OK;
     }
     if (c->cross) {

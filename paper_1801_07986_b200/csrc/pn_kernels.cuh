@@ -506,21 +506,29 @@ __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp64_kernel(const JRec*
 // sum over all j != i of a per-j quantity, i.e. a global sum minus star i's own term: with
 //   P = sum_j G m_j v_j,  Q1 = sum_j G m_j / r_j1,  Q3 = sum_j G m_j / r_j1^3,  W = sum_j G m_j x_j1 / r_j1^3
 // (cross_prep_kernel + cross_sum_kernel, O(N)) L4 and parts of L1 and L3 are O(N) work in the epilogue.  What is left for
-// the O(N^2) loop, per ordered pair with d = x_ij, y = 1/rho_ij, s = G m_j y^3:
-//   a^SS -= s d                                                           (the Newtonian term of Eq. 2.4, 3 DFMA extra)
-//   A    += s g d,  g = GM f2 + v_i^2 - 2 |v_ij|^2 + (3/2)(v_j.d)^2 y^2,   f2 = 4/r_i1 + 5/(4 r_j1) + (rho^2 - r_i1^2)/(4 r_j1^3)
-//   S    += G m_j (4 y - rho^2 / (4 r_j1^3))           (L1: coefficient of GM x_i1 / r_i1^3)
-//   Y    += y (G m_j x_j1 / r_j1^3)                    (L3: times -(7/2) GM)
-//   H    += h,  V += h v_j,   h = s (4 v_i.d - 3 v_j.d) (L6 = H v_i - V)
-// = 54 FP64-pipe instructions + 1 MUFU.RSQ64H per ordered pair.  Tiled form (ordered pairs, j tiles of 96 B records
-// through double-buffered shared memory, I i-stars per thread); output part[S][6][np]: a^SS and the pair part of the
-// Cross term per j-chunk, reduced in fixed order by the epilogue.
+// the O(N^2) loop, per ordered pair (i <- j) with d = x_ij, u = v_ij, y = 1/rho_ij, s = G m_j y^3 and the per-star constants
+// of the record below (a5_j = GM 5/(4 r_j1), b_j = GM/(4 r_j1^3), w_j = -(7/2) GM G m_j x_j1/r_j1^3, kap_i = 4GM/r_i1 + v_i^2):
+//   n  -= s d                                                           (the Newtonian term of Eq. 2.4)
+//   X  += s g d + h u + y w_j                                            (pair parts of L2 + L5, L6, L3)
+//         g = (rho^2 - r_i1^2) b_j + a5_j + kap_i - 2 |u|^2 + (3/2)(v_j.d)^2 y^2,    h = s (4 v_i.d - 3 v_j.d)
+//   S  += G m_j (4 GM y - rho^2 b_j)                                     (L1: coefficient of x_i1 / r_i1^3, applied by the epilogue)
+//   U  += G m_j y (5/4 + (r_i1^2 - r_j1^2) y^2 / 4)                      (BHX: [a_1]_Cross, below)
+// Output part[S][7 or 8][np]: n (3), X (3), S, U per partial-sum slot, reduced in fixed order by the epilogue.
+//
+// Two kernels.  pair_cross_fp64_kernel walks every ORDERED pair (tiled: j tiles through double-buffered shared memory,
+// I i-stars per thread; used below kCrossSymMinStars).  pair_cross_sym_kernel evaluates every UNORDERED pair once, for
+// both stars: d, rho^-1, |u|^2, v_i.d and v_j.d are shared, the reversed pair (j <- i) has d -> -d, u -> -u,
+//   n_j += s_i d,   X_j += -s_i g' d - h' u + y w_i,   g' = (rho^2 - r_j1^2) b_i + a5_i + kap_j - 2|u|^2 + (3/2)(v_i.d)^2 y^2,
+//   h' = s_i (3 v_i.d - 4 v_j.d),   S_j += G m_i (4 GM y - rho^2 b_i),   U_j += G m_i y (5/4 - (r_i1^2 - r_j1^2) y^2 / 4),
+// and the eight j-side sums travel through the lanes of the warp with the j-star (Gray-code walk, butterfly shuffles) as
+// in pair_sym_fp64_kernel: 76 FP64-pipe instructions + 1 MUFU.RSQ64H per unordered pair (84 with U) = 38 (42) per ordered
+// pair instead of 54 (59).
 // ---------------------------------------------------------------------------------------------------------
 struct __align__(16) CRec {
     double x, y, z, gm;      // position, G m_j
-    double vx, vy, vz, a5;   // velocity, 5 / (4 r_j1)
-    double b, wx, wy, wz;    // 1 / (4 r_j1^3),  G m_j x_j1 / r_j1^3
-    double rj2, pad;         // r_j1^2 (used by the [a_1]_Cross sum only)
+    double vx, vy, vz, a5;   // velocity, GM 5 / (4 r_j1)
+    double b, wx, wy, wz;    // GM / (4 r_j1^3),  -(7/2) GM G m_j x_j1 / r_j1^3
+    double rj2, kap;         // r_j1^2,  4 GM / r_j1 + v_j^2
 };
 static_assert(sizeof(CRec) == 112, "CRec must be 112 bytes");
 
@@ -529,7 +537,7 @@ constexpr int kCrossSums = 8;  // P (3), Q1, Q3, W (3)
 template <int NT>
 __global__ void __launch_bounds__(NT) cross_prep_kernel(const JRec* __restrict__ jrec, const double* __restrict__ v,
                                                         const BhState* __restrict__ bh, CRec* __restrict__ crec,
-                                                        double* __restrict__ blk /* [grid][8] */, int n_stars, int np)
+                                                        double* __restrict__ blk /* [grid][8] */, int n_stars, int np, double GM)
 {
     __shared__ double red[kCrossSums][NT / 32];
     const int i = blockIdx.x * NT + threadIdx.x;
@@ -538,18 +546,20 @@ __global__ void __launch_bounds__(NT) cross_prep_kernel(const JRec* __restrict__
         const JRec r = jrec[i];
         CRec o;
         o.x = r.x, o.y = r.y, o.z = r.z, o.gm = r.gm;
-        o.vx = o.vy = o.vz = o.a5 = o.b = o.wx = o.wy = o.wz = o.rj2 = o.pad = 0.0;
+        o.vx = o.vy = o.vz = o.a5 = o.b = o.wx = o.wy = o.wz = o.rj2 = o.kap = 0.0;
         if (i < n_stars) {
             const double d[3] = {r.x - bh->xs[0], r.y - bh->xs[1], r.z - bh->xs[2]};  // x_j1
             const double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
             const double inv_r = 1.0 / sqrt(r2);
             const double inv_r3 = inv_r * inv_r * inv_r;
             o.vx = v[i], o.vy = v[np + i], o.vz = v[2 * np + i];
-            o.a5 = 1.25 * inv_r, o.b = 0.25 * inv_r3, o.rj2 = r2;
-            o.wx = r.gm * d[0] * inv_r3, o.wy = r.gm * d[1] * inv_r3, o.wz = r.gm * d[2] * inv_r3;
+            o.a5 = GM * 1.25 * inv_r, o.b = GM * 0.25 * inv_r3, o.rj2 = r2;
+            o.kap = 4.0 * GM * inv_r + (o.vx * o.vx + o.vy * o.vy + o.vz * o.vz);
+            const double w[3] = {r.gm * d[0] * inv_r3, r.gm * d[1] * inv_r3, r.gm * d[2] * inv_r3};
+            o.wx = -3.5 * GM * w[0], o.wy = -3.5 * GM * w[1], o.wz = -3.5 * GM * w[2];
             sums[0] = r.gm * o.vx, sums[1] = r.gm * o.vy, sums[2] = r.gm * o.vz;
             sums[3] = r.gm * inv_r, sums[4] = r.gm * inv_r3;
-            sums[5] = o.wx, sums[6] = o.wy, sums[7] = o.wz;
+            sums[5] = w[0], sums[6] = w[1], sums[7] = w[2];
         }
         crec[i] = o;
     }
@@ -583,18 +593,19 @@ __global__ void __launch_bounds__(256) cross_sum_kernel(const double* __restrict
 //   + sum_{j != k} G^2 m_j m_k x_1j / r_1j^3 ( 4/r_1k + 5/(4 rho_jk) + (r_1j^2 - r_1k^2)/(4 rho_jk^3) )
 //   - (7/2) sum_{j != k} G^2 m_j m_k x_jk / (rho_jk^3 r_1j)                  [= + (7/2) sum_j (G m_j / r_1j) a_j^SS]
 //   - sum_{j, k} (G m_j m_k / (M r_1j^3)) [ 4 (v_j.v_k) x_1j - 3 (v_j.x_1j) v_k - 4 (v_k.x_1j) v_j ]   [O(N) with P]
-// needs one more O(N^2) sum per star, U_i = sum_{j != i} G m_j ( 5/(4 rho) + (r_i1^2 - r_j1^2)/(4 rho^3) ) (5 more FP64
-// instructions per pair, 7th output component); everything else is O(N) work in the epilogue, summed over the stars by
-// the reduction that already builds a_1.
+// needs one more O(N^2) sum per star, U_i = sum_{j != i} G m_j ( 5/(4 rho) + (r_i1^2 - r_j1^2)/(4 rho^3) ) (last output
+// component); everything else is O(N) work in the epilogue, summed over the stars by the reduction that already builds a_1.
+template <bool BHX>
+constexpr int kCrossNC = BHX ? 8 : 7;
+
 template <int I, int MINB, int NT, int TJ, bool BHX>
-__global__ void __launch_bounds__(NT, MINB) pair_cross_fp64_kernel(const CRec* __restrict__ crec, const BhState* __restrict__ bh,
-                                                                   double* __restrict__ part /* [S][6 + BHX][np] */, int np,
-                                                                   int tiles_per_split, double eps2, double GM)
+__global__ void __launch_bounds__(NT, MINB) pair_cross_fp64_kernel(const CRec* __restrict__ crec, double* __restrict__ part /* [S][NC][np] */,
+                                                                   int np, int tiles_per_split, double eps2, double GM4)
 {
-    constexpr int NC = BHX ? 7 : 6;
+    constexpr int NC = kCrossNC<BHX>;
     __shared__ CRec sj[2][TJ];
     const int tid = threadIdx.x;
-    double xi[I], yi[I], zi[I], vxi[I], vyi[I], vzi[I], ri2[I], ci[I], vi2[I];
+    double xi[I], yi[I], zi[I], vxi[I], vyi[I], vzi[I], ri2[I], kapi[I];
     double nx[I], ny[I], nz[I], ax[I], ay[I], az[I], S[I], Yx[I], Yy[I], Yz[I], H[I], Vx[I], Vy[I], Vz[I], U[I];
     int ii[I];
 #pragma unroll
@@ -602,10 +613,7 @@ __global__ void __launch_bounds__(NT, MINB) pair_cross_fp64_kernel(const CRec* _
         ii[k] = blockIdx.x * (I * NT) + tid + k * NT;
         const CRec c = crec[ii[k]];
         xi[k] = c.x, yi[k] = c.y, zi[k] = c.z, vxi[k] = c.vx, vyi[k] = c.vy, vzi[k] = c.vz;
-        const double dx = c.x - bh->xs[0], dy = c.y - bh->xs[1], dz = c.z - bh->xs[2];
-        ri2[k] = dx * dx + dy * dy + dz * dz;
-        ci[k] = 4.0 / sqrt(ri2[k]);
-        vi2[k] = c.vx * c.vx + c.vy * c.vy + c.vz * c.vz;
+        ri2[k] = c.rj2, kapi[k] = c.kap;
         nx[k] = ny[k] = nz[k] = ax[k] = ay[k] = az[k] = S[k] = Yx[k] = Yy[k] = Yz[k] = H[k] = Vx[k] = Vy[k] = Vz[k] = U[k] = 0.0;
     }
     const int n_tiles = np / TJ;
@@ -644,13 +652,12 @@ __global__ void __launch_bounds__(NT, MINB) pair_cross_fp64_kernel(const CRec* _
                 const double uu = fma(ux, ux, fma(uy, uy, uz * uz));
                 const double vjx = fma(r.vx, dx, fma(r.vy, dy, r.vz * dz));
                 const double vix = fma(vxi[k], dx, fma(vyi[k], dy, vzi[k] * dz));
-                const double f2 = fma(r2 - ri2[k], r.b, r.a5) + ci[k];
-                double g = fma(GM, f2, vi2[k]);
+                double g = fma(r2 - ri2[k], r.b, r.a5) + kapi[k];
                 g = fma(-2.0, uu, g);
                 g = fma(1.5, (vjx * vjx) * y2, g);
                 const double sg = s * g;
                 ax[k] = fma(sg, dx, ax[k]), ay[k] = fma(sg, dy, ay[k]), az[k] = fma(sg, dz, az[k]);
-                S[k] = fma(gm, fma(-r2, r.b, 4.0 * y), S[k]);
+                S[k] = fma(gm, fma(-r2, r.b, GM4 * y), S[k]);
                 Yx[k] = fma(y, r.wx, Yx[k]), Yy[k] = fma(y, r.wy, Yy[k]), Yz[k] = fma(y, r.wz, Yz[k]);
                 const double h = s * fma(4.0, vix, -3.0 * vjx);
                 H[k] += h;
@@ -663,14 +670,186 @@ __global__ void __launch_bounds__(NT, MINB) pair_cross_fp64_kernel(const CRec* _
     double* out = part + (size_t)blockIdx.y * NC * np;
 #pragma unroll
     for (int k = 0; k < I; ++k) {
-        if (BHX) out[6 * np + ii[k]] = U[k];
-        const double dx = xi[k] - bh->xs[0], dy = yi[k] - bh->xs[1], dz = zi[k] - bh->xs[2];  // x_i1
-        const double inv_r = 0.25 * ci[k];
-        const double c1 = GM * inv_r * inv_r * inv_r * S[k];  // L1 pair part: GM x_i1 / r_i1^3 * S
         out[ii[k]] = nx[k], out[np + ii[k]] = ny[k], out[2 * np + ii[k]] = nz[k];
-        out[3 * np + ii[k]] = fma(c1, dx, ax[k]) - 3.5 * GM * Yx[k] + fma(H[k], vxi[k], -Vx[k]);
-        out[4 * np + ii[k]] = fma(c1, dy, ay[k]) - 3.5 * GM * Yy[k] + fma(H[k], vyi[k], -Vy[k]);
-        out[5 * np + ii[k]] = fma(c1, dz, az[k]) - 3.5 * GM * Yz[k] + fma(H[k], vzi[k], -Vz[k]);
+        out[3 * np + ii[k]] = ax[k] + Yx[k] + fma(H[k], vxi[k], -Vx[k]);
+        out[4 * np + ii[k]] = ay[k] + Yy[k] + fma(H[k], vyi[k], -Vy[k]);
+        out[5 * np + ii[k]] = az[k] + Yz[k] + fma(H[k], vzi[k], -Vz[k]);
+        out[6 * np + ii[k]] = S[k];
+        if (BHX) out[7 * np + ii[k]] = U[k];
+    }
+}
+
+// ---- the symmetric form: every unordered pair once.  One-warp blocks, I = 2 i-stars per lane, unit tiles of U = 64 stars,
+// the work-item / slot scheme of pair_sym_fp64_kernel (block (A <= B) of a triangular grid over G groups of m tiles: row
+// sums to slot B, column sums to slot A, one writer per (slot, star), nothing zeroed, no atomics).
+constexpr int kCrossSymI = 2;
+constexpr int kCrossSymU = 32 * kCrossSymI;
+template <bool BHX>
+constexpr int kCrossSymSmemBytes = kCrossSymU * ((int)sizeof(CRec) + kCrossNC<BHX> * 8);
+
+struct CrossAcc {  // the sums of one star: n (3), X (3), S, U
+    double n[3], X[3], S, U;
+};
+
+// one ordered or unordered pair: i-star (register state) against the j record r.  SYM: also the reversed pair into b.
+template <bool SYM, bool BHX>
+__device__ __forceinline__ void cross_pair(const CRec& r, const double (&xi)[3], const double (&vi)[3], double ri2, double kapi,
+                                           double gmi, double a5i, double bi, const double (&wi)[3], CrossAcc& a, CrossAcc& b,
+                                           double eps2, double GM4, bool self)
+{
+    const double d[3] = {xi[0] - r.x, xi[1] - r.y, xi[2] - r.z};  // x_ij
+    const double r2 = fma(d[0], d[0], fma(d[1], d[1], fma(d[2], d[2], eps2)));
+    const double y0 = rsqrt_seed(r2);
+    const double e = fma(-r2, y0 * y0, 1.0);
+    double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1 / rho to full fp64 accuracy
+    double gmj = r.gm;
+    if (!SYM) {  // diagonal unit tile, ordered pairs: j != i in every sum of Eq. 2.6 (eps > 0 does not cancel the self term here)
+        y = self ? 0.0 : y;
+        gmj = self ? 0.0 : gmj;
+    }
+    const double y2 = y * y, y3 = y2 * y;
+    const double u[3] = {vi[0] - r.vx, vi[1] - r.vy, vi[2] - r.vz};  // v_ij
+    const double uu = fma(u[0], u[0], fma(u[1], u[1], u[2] * u[2]));
+    const double vjx = fma(r.vx, d[0], fma(r.vy, d[1], r.vz * d[2]));
+    const double vix = fma(vi[0], d[0], fma(vi[1], d[1], vi[2] * d[2]));
+    const double da = vix - vjx;                 // u.d
+    const double y4 = GM4 * y;
+    const double yq = 1.2247448713915890 * y;    // sqrt(3/2) / rho
+    double dy2 = 0.0;
+    if (BHX) dy2 = (ri2 - r.rj2) * y2;
+    {   // i <- j
+        const double s = gmj * y3;
+        const double pj = vjx * yq;
+        const double g = fma(pj, pj, fma(r2 - ri2, r.b, r.a5) + fma(-2.0, uu, kapi));
+        const double sg = s * g;
+        const double h = s * fma(3.0, da, vix);  // s (4 v_i.d - 3 v_j.d)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) a.n[c] = fma(-s, d[c], a.n[c]);
+        a.X[0] = fma(y, r.wx, fma(h, u[0], fma(sg, d[0], a.X[0])));
+        a.X[1] = fma(y, r.wy, fma(h, u[1], fma(sg, d[1], a.X[1])));
+        a.X[2] = fma(y, r.wz, fma(h, u[2], fma(sg, d[2], a.X[2])));
+        a.S = fma(gmj, fma(-r2, r.b, y4), a.S);
+        if (BHX) a.U = fma(gmj * y, fma(dy2, 0.25, 1.25), a.U);
+    }
+    if (SYM) {  // j <- i: d -> -d, u -> -u
+        const double s = gmi * y3;
+        const double pi = vix * yq;
+        const double g = fma(pi, pi, fma(r2 - r.rj2, bi, a5i) + fma(-2.0, uu, r.kap));
+        const double sg = s * g;
+        const double h = s * fma(3.0, da, -vjx);  // s (3 v_i.d - 4 v_j.d)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) b.n[c] = fma(s, d[c], b.n[c]);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) b.X[c] = fma(y, wi[c], fma(-h, u[c], fma(-sg, d[c], b.X[c])));
+        b.S = fma(gmi, fma(-r2, bi, y4), b.S);
+        if (BHX) b.U = fma(gmi * y, fma(dy2, -0.25, 1.25), b.U);
+    }
+}
+
+__device__ __forceinline__ void cross_acc_zero(CrossAcc& a)
+{
+    a.n[0] = a.n[1] = a.n[2] = a.X[0] = a.X[1] = a.X[2] = a.S = a.U = 0.0;
+}
+
+template <bool BHX>
+__device__ __forceinline__ void cross_acc_shfl(CrossAcc& a, int mask)
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) a.n[c] = __shfl_xor_sync(0xffffffffu, a.n[c], mask), a.X[c] = __shfl_xor_sync(0xffffffffu, a.X[c], mask);
+    a.S = __shfl_xor_sync(0xffffffffu, a.S, mask);
+    if (BHX) a.U = __shfl_xor_sync(0xffffffffu, a.U, mask);
+}
+
+template <int MINB, bool BHX>
+__global__ void __launch_bounds__(32, MINB) pair_cross_sym_kernel(const CRec* __restrict__ crec, double* __restrict__ part /* [G][NC][np] */,
+                                                                  int np, int n_tiles, int m, double eps2, double GM4)
+{
+    constexpr int I = kCrossSymI, U = kCrossSymU, NC = kCrossNC<BHX>;
+    extern __shared__ double2 sym_smem[];
+    CRec* sj = reinterpret_cast<CRec*>(sym_smem);                                // [U] the j tile
+    double(*cacc)[U] = reinterpret_cast<double(*)[U]>(sym_smem + U * 7);         // [NC][U] column sums, then row sums
+    const int lane = threadIdx.x;
+    int A, B;
+    sym_decode_block(blockIdx.x, A, B);
+    const int ta0 = A * m, ta1 = min(ta0 + m, n_tiles);
+    const int tb0 = B * m, tb1 = min(tb0 + m, n_tiles);
+
+    auto store_acc = [&](const CrossAcc& a, int el) {
+        cacc[0][el] = a.n[0], cacc[1][el] = a.n[1], cacc[2][el] = a.n[2];
+        cacc[3][el] = a.X[0], cacc[4][el] = a.X[1], cacc[5][el] = a.X[2];
+        cacc[6][el] = a.S;
+        if (BHX) cacc[7][el] = a.U;
+    };
+    auto flush = [&](int slot, int tile, bool first) {  // cacc -> part[slot][NC][tile]; the same lane owns the same elements every time
+        double* dst = part + (size_t)slot * NC * np + (size_t)tile * U;
+#pragma unroll
+        for (int c = 0; c < NC; ++c)
+#pragma unroll
+            for (int q = lane; q < U; q += 32) {
+                double* p = dst + (size_t)c * np + q;
+                const double v = cacc[c][q];
+                *p = first ? v : *p + v;
+            }
+    };
+
+    for (int ta = ta0; ta < ta1; ++ta) {
+        double xi[I][3], vi[I][3], ri2[I], kapi[I], gmi[I], a5i[I], bi[I], wi[I][3];
+        CrossAcc acc[I];
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            const CRec c = crec[(size_t)ta * U + lane + 32 * k];
+            xi[k][0] = c.x, xi[k][1] = c.y, xi[k][2] = c.z, vi[k][0] = c.vx, vi[k][1] = c.vy, vi[k][2] = c.vz;
+            ri2[k] = c.rj2, kapi[k] = c.kap, gmi[k] = c.gm, a5i[k] = c.a5, bi[k] = c.b;
+            wi[k][0] = c.wx, wi[k][1] = c.wy, wi[k][2] = c.wz;
+            cross_acc_zero(acc[k]);
+        }
+        for (int tb = (A == B) ? ta : tb0; tb < tb1; ++tb) {
+            __syncwarp();
+            {
+                const double2* src = reinterpret_cast<const double2*>(crec + (size_t)tb * U);
+                for (int q = lane; q < U * 7; q += 32) sym_smem[q] = src[q];
+            }
+            __syncwarp();
+            if (ta == tb) {  // diagonal unit tile: ordered pairs, i-side only, j != i by index
+                CrossAcc dummy;
+                cross_acc_zero(dummy);
+#pragma unroll 1
+                for (int jj = 0; jj < U; ++jj) {
+                    const CRec r = sj[jj];
+#pragma unroll
+                    for (int k = 0; k < I; ++k)
+                        cross_pair<false, BHX>(r, xi[k], vi[k], ri2[k], kapi[k], gmi[k], a5i[k], bi[k], wi[k], acc[k], dummy, eps2, GM4,
+                                               jj == lane + 32 * k);
+                }
+            } else {
+#pragma unroll 1
+                for (int jb = 0; jb < U; jb += 32) {
+                    CrossAcc b;
+                    cross_acc_zero(b);
+#pragma unroll 1
+                    for (int c = 0; c < 4; ++c) {  // Gray-code walk in four chunks of 8 steps (see sym_unit_tile_gray)
+                        const int base = jb + (lane ^ ((c & 1 ? 12 : 0) ^ (c & 2 ? 24 : 0)));
+                        const int last_mask = (c & 1) ? 16 : 8;
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) {
+                            const CRec r = sj[base ^ (q ^ (q >> 1))];
+#pragma unroll
+                            for (int k = 0; k < I; ++k)
+                                cross_pair<true, BHX>(r, xi[k], vi[k], ri2[k], kapi[k], gmi[k], a5i[k], bi[k], wi[k], acc[k], b, eps2, GM4, false);
+                            cross_acc_shfl<BHX>(b, (q + 1 < 8) ? ((q + 1) & -(q + 1)) : last_mask);
+                        }
+                    }
+                    store_acc(b, jb + lane);
+                }
+                __syncwarp();
+                flush(A, tb, ta == ta0);  // column sums: the i-stars of tile ta acting on the j-stars of tile tb
+            }
+        }
+        __syncwarp();
+#pragma unroll
+        for (int k = 0; k < I; ++k) store_acc(acc[k], lane + 32 * k);
+        __syncwarp();
+        flush(B, ta, (A < B) || (ta == ta0));  // row sums: the j-stars of group B acting on the i-stars of tile ta
     }
 }
 
@@ -1146,14 +1325,14 @@ enum { MODE_ACCEL = 0, MODE_RK4 = 1 };
 
 constexpr int kEpiStars = 32;  // stars per epilogue block: lane = star, warp w sums the partial-sum slots w, w + NW, ...
 
-// CROSS: the partial sums carry 6 components (a^SS and the pair part of [a_i]_Cross, Eq. 2.6); the O(N) parts of the
-// Cross term are added here (see pair_cross_fp64_kernel).
-// CROSS = 2: additionally the star's share of [a_1]_Cross (Eq. 2.3), 7th component U (see pair_cross_fp64_kernel<BHX>).
+// CROSS: the partial sums carry 7 components (a^SS, the pair part X of [a_i]_Cross, Eq. 2.6, and the scalar S of its line
+// L1); the O(N) parts of the Cross term are added here (see the pair_cross kernels).
+// CROSS = 2: additionally the star's share of [a_1]_Cross (Eq. 2.3), 8th component U.
 template <int MODE, int NT, int CROSS>
 __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
 {
     constexpr int NW = NT / 32;
-    constexpr int NC = CROSS == 2 ? 7 : (CROSS ? 6 : 3);
+    constexpr int NC = CROSS == 2 ? 8 : (CROSS ? 7 : 3);
     static_assert(NW == 4, "the fixed-order cross-warp sum below is written for 4 warps");
     __shared__ double red[3 * NW];
     __shared__ double wsum[NW][NC][kEpiStars];
@@ -1168,7 +1347,7 @@ __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
 #pragma unroll
     for (int k = 0; k < NC; ++k) ss[k] = 0.0;
     if (i < A.n_stars) {
-        constexpr int UN = CROSS ? 2 : 4;  // slots in flight per thread (12 loads either way)
+        constexpr int UN = CROSS ? 2 : 4;  // slots in flight per thread (12 - 16 loads)
         const size_t stride = (size_t)NW * NC * np;
         const double* p = A.part + (size_t)w * NC * np + i;
         int s = w;
@@ -1231,7 +1410,8 @@ __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
             const double vP = vel[0] * P[0] + vel[1] * P[1] + vel[2] * P[2];
             const double xP = x[0] * P[0] + x[1] * P[1] + x[2] * P[2];
             // coefficient of x_i1: L0 (5 G m_i GM / r^4 - 4 G m_i v^2 / r^3) + L1 (GM/r^3)(5/4 Q1 + r^2/4 Q3) - L4 4 (v.P)/r^3
-            const double kx = inv_r3 * (5.0 * rec.gm * GMr - 4.0 * rec.gm * v2 + A.GM * (1.25 * Q1 + 0.25 * r2 * Q3) - 4.0 * vP);
+            // + the pair part of L1, S / r^3 (S = sum_j G m_j (4 GM / rho_ij - GM rho_ij^2 / (4 r_j1^3)), 7th component)
+            const double kx = inv_r3 * (5.0 * rec.gm * GMr - 4.0 * rec.gm * v2 + A.GM * (1.25 * Q1 + 0.25 * r2 * Q3) - 4.0 * vP + ss[6]);
             // coefficient of v_i: L0 7 G m_i (v.x)/r^3 + L4 3 (P.x)/r^3
             const double kv = inv_r3 * (7.0 * rec.gm * vx + 3.0 * xP);
             const double kp = 4.0 * vx * inv_r3;       // L4: + 4 (v_i.x_i1) P / r^3
@@ -1244,7 +1424,7 @@ __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
                 const double vPf = vel[0] * Pf[0] + vel[1] * Pf[1] + vel[2] * Pf[2];
                 const double xPf = x[0] * Pf[0] + x[1] * Pf[1] + x[2] * Pf[2];
                 const double gr3 = rec.gm * inv_r3, g_M = gr3 / A.GM;
-                const double tx = -(4.0 * rec.gm * gr3 * inv_r + gr3 * (4.0 * Q1 + ss[6])) + 4.0 * g_M * vPf;  // times x
+                const double tx = -(4.0 * rec.gm * gr3 * inv_r + gr3 * (4.0 * Q1 + ss[CROSS == 2 ? 7 : 0])) + 4.0 * g_M * vPf;  // times x
                 const double tP = -3.0 * g_M * vx;                                                             // times P
                 const double tv = -4.0 * g_M * xPf;                                                            // times v_j
                 const double ta = 3.5 * rec.gm * inv_r;                                                        // times a_j^SS

@@ -31,7 +31,9 @@ def _pn_cross(p, terms=CROSS_STAR):
 
 
 @pytest.mark.parametrize("terms", TERMS)
-@pytest.mark.parametrize("n_stars", [1, 2, 3, 129, 1023, 4099, 13001])
+# from 6144 stars on the Cross terms run in the symmetric kernel (every unordered pair once, variant 8 / 9): 64-star unit
+# tiles in up to 128 groups of m tiles (m = 1 up to 8192 stars, 2 up to 16384, 3 at 20000)
+@pytest.mark.parametrize("n_stars", [1, 2, 3, 129, 1023, 4099, 6143, 6144, 8200, 13001, 16383, 20000])
 def test_cross_accel_parity_sizes(n_stars, terms):
     if n_stars <= 3:
         p = inputs.random_small(n_stars, seed=700 + n_stars, M=1.0, m_scale=1e-2, c=10.0, softening=1e-3, bh_moving=True)
@@ -40,9 +42,12 @@ def test_cross_accel_parity_sizes(n_stars, terms):
     ref = Oracle(p.mass, p.G, p.c, p.softening, terms=terms).accel(p.pos, p.vel)
     hot = Oracle(p.mass, p.G, p.c, p.softening).accel(p.pos, p.vel)
     with _pn_cross(p, terms) as pn:
-        assert pn.pn_get_pair_config()["variant"] == (6 if terms & CROSS_BH else 5)
+        sym = n_stars >= 6144
+        assert pn.pn_get_pair_config()["variant"] == ((9 if sym else 6) if terms & CROSS_BH else (8 if sym else 5))
         acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
+        again = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
     assert rel_err_rows(acc, ref).max() <= TOL_ACC
+    assert np.array_equal(acc, again)  # fixed-order sums
     if n_stars >= 2:  # the Cross term is really there (with one star only the O(m_i) self line is left)
         assert rel_err_rows(hot[1:], ref[1:]).max() > 1e-9
     if terms & CROSS_BH:
@@ -52,20 +57,54 @@ def test_cross_accel_parity_sizes(n_stars, terms):
 
 
 @pytest.mark.parametrize("terms", TERMS)
-@pytest.mark.parametrize("gen", ["cusp", "unequal_eps0", "tracers"])
+@pytest.mark.parametrize("gen", ["cusp", "unequal_eps0", "tracers", "cusp_sym", "unequal_eps0_sym", "tracers_sym"])
 def test_cross_accel_parity_other_inputs(gen, terms):
+    """*_sym: sizes at which the symmetric Cross kernel runs (>= 6144 stars), compared on sampled rows + the massive object."""
     if gen == "cusp":
         p = inputs.cusp_bh(3000, seed=5)
     elif gen == "unequal_eps0":
         p = inputs.random_small(500, seed=8, M=1.0, m_scale=1e-3, c=10.0, softening=0.0, bh_moving=True)
-    else:
+    elif gen == "tracers":
         p = inputs.plummer_bh(700, seed=9, c=30.0)
         p.mass[10:200] = 0.0
-    ref = Oracle(p.mass, p.G, p.c, p.softening, terms=terms).accel(p.pos, p.vel)
+    elif gen == "cusp_sym":
+        p = inputs.cusp_bh(8000, seed=5)
+    elif gen == "unequal_eps0_sym":
+        p = inputs.random_small(7001, seed=8, M=1.0, m_scale=1e-4, c=10.0, softening=0.0, bh_moving=True)
+    else:
+        p = inputs.plummer_bh(6500, seed=9, c=30.0)
+        p.mass[10:3000:3] = 0.0
+    rows = np.arange(p.N) if p.N < 4000 else np.concatenate(
+        [[0, 1, p.N - 1], np.sort(np.random.default_rng(3).choice(np.arange(2, p.N - 1), 1500, replace=False))])
+    ref = Oracle(p.mass, p.G, p.c, p.softening, terms=terms).accel_rows(p.pos, p.vel, rows)
     with _pn_cross(p, terms) as pn:
+        assert (pn.pn_get_pair_config()["variant"] >= 8) == gen.endswith("_sym")
         acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
     assert np.isfinite(acc).all()
-    assert rel_err_rows(acc, ref).max() <= TOL_ACC
+    assert rel_err_rows(acc[rows], ref).max() <= TOL_ACC
+
+
+@pytest.mark.parametrize("terms", TERMS)
+def test_cross_symmetric_and_ordered_kernels_agree_and_track_the_oracle(terms):
+    """6500 stars: the symmetric Cross kernel (default from 6144 stars) against the ordered-pair kernel (PN_PAIR_TILED) on
+    every row, and three RK4 steps of each against the oracle with the same terms."""
+    from paper_1801_07986_b200 import PN, binding
+
+    p = inputs.plummer_bh(6500, seed=21, c=20.0, dt=1e-3)
+    xr, vr = Oracle(p.mass, p.G, p.c, p.softening, terms=terms).step(p.pos, p.vel, p.dt, 3)
+    acc, traj = {}, {}
+    for kernel in (binding.PN_PAIR_AUTO, binding.PN_PAIR_TILED):
+        with PN(p.mass, p.G, p.c, p.softening) as pn:
+            pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, kernel)  # before the Cross option: it sizes the Cross buffers
+            pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, terms)
+            assert (pn.pn_get_pair_config()["variant"] >= 8) == (kernel == binding.PN_PAIR_AUTO)
+            acc[kernel] = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
+            pn.pn_set_state_host(p.pos, p.vel)
+            pn.pn_step(p.dt, 3)
+            traj[kernel] = pn.pn_get_state_host()
+    assert rel_err_rows(acc[binding.PN_PAIR_AUTO], acc[binding.PN_PAIR_TILED]).max() <= 1e-13
+    for x, v in traj.values():
+        assert max(rel_err_rows(x, xr).max(), rel_err_rows(v, vr).max()) <= 1e-11
 
 
 def test_cross_switch_off_restores_the_hot_path_bitwise_and_is_deterministic():
