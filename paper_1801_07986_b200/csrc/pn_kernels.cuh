@@ -685,7 +685,7 @@ __global__ void __launch_bounds__(NT, MINB) pair_cross_fp64_kernel(const CRec* _
 constexpr int kCrossSymI = 2;
 constexpr int kCrossSymU = 32 * kCrossSymI;
 template <bool BHX>
-constexpr int kCrossSymSmemBytes = kCrossSymU * ((int)sizeof(CRec) + kCrossNC<BHX> * 8);
+constexpr int kCrossSymSmemBytes = kCrossSymU * (2 * (int)sizeof(CRec) + kCrossNC<BHX> * 8);
 
 struct CrossAcc {  // the sums of one star: n (3), X (3), S, U
     double n[3], X[3], S, U;
@@ -760,20 +760,34 @@ __device__ __forceinline__ void cross_acc_shfl(CrossAcc& a, int mask)
     if (BHX) a.U = __shfl_xor_sync(0xffffffffu, a.U, mask);
 }
 
+__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned int)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
 template <int MINB, bool BHX>
 __global__ void __launch_bounds__(32, MINB) pair_cross_sym_kernel(const CRec* __restrict__ crec, double* __restrict__ part /* [G][NC][np] */,
                                                                   int np, int n_tiles, int m, double eps2, double GM4)
 {
     constexpr int I = kCrossSymI, U = kCrossSymU, NC = kCrossNC<BHX>;
     extern __shared__ double2 sym_smem[];
-    CRec* sj = reinterpret_cast<CRec*>(sym_smem);                                // [U] the j tile
-    double(*cacc)[U] = reinterpret_cast<double(*)[U]>(sym_smem + U * 7);         // [NC][U] column sums, then row sums
+    // two j tiles (the next one is on its way, cp.async, while the current one is evaluated), then [NC][U] column / row sums
+    double(*cacc)[U] = reinterpret_cast<double(*)[U]>(sym_smem + 2 * U * 7);
     const int lane = threadIdx.x;
     int A, B;
     sym_decode_block(blockIdx.x, A, B);
     const int ta0 = A * m, ta1 = min(ta0 + m, n_tiles);
     const int tb0 = B * m, tb1 = min(tb0 + m, n_tiles);
 
+    auto fetch_tile = [&](int buf, int tile) {
+        const double2* src = reinterpret_cast<const double2*>(crec + (size_t)tile * U);
+        double2* dst = sym_smem + buf * (U * 7);
+#pragma unroll
+        for (int q = lane; q < U * 7; q += 32) cp_async16(dst + q, src + q);
+        cp_async_commit();
+    };
     auto store_acc = [&](const CrossAcc& a, int el) {
         cacc[0][el] = a.n[0], cacc[1][el] = a.n[1], cacc[2][el] = a.n[2];
         cacc[3][el] = a.X[0], cacc[4][el] = a.X[1], cacc[5][el] = a.X[2];
@@ -792,6 +806,8 @@ __global__ void __launch_bounds__(32, MINB) pair_cross_sym_kernel(const CRec* __
             }
     };
 
+    int buf = 0;
+    fetch_tile(0, (A == B) ? ta0 : tb0);
     for (int ta = ta0; ta < ta1; ++ta) {
         double xi[I][3], vi[I][3], ri2[I], kapi[I], gmi[I], a5i[I], bi[I], wi[I][3];
         CrossAcc acc[I];
@@ -804,12 +820,14 @@ __global__ void __launch_bounds__(32, MINB) pair_cross_sym_kernel(const CRec* __
             cross_acc_zero(acc[k]);
         }
         for (int tb = (A == B) ? ta : tb0; tb < tb1; ++tb) {
-            __syncwarp();
-            {
-                const double2* src = reinterpret_cast<const double2*>(crec + (size_t)tb * U);
-                for (int q = lane; q < U * 7; q += 32) sym_smem[q] = src[q];
+            cp_async_wait_all();
+            __syncwarp();  // the tile is there, and everyone is done with the other buffer
+            {   // the next tile of this item's walk, if any
+                int nt = tb + 1;
+                if (nt >= tb1) nt = (ta + 1 < ta1) ? ((A == B) ? ta + 1 : tb0) : -1;
+                if (nt >= 0) fetch_tile(buf ^ 1, nt);
             }
-            __syncwarp();
+            const CRec* sj = reinterpret_cast<const CRec*>(sym_smem + buf * (U * 7));
             if (ta == tb) {  // diagonal unit tile: ordered pairs, i-side only, j != i by index
                 CrossAcc dummy;
                 cross_acc_zero(dummy);
@@ -843,13 +861,15 @@ __global__ void __launch_bounds__(32, MINB) pair_cross_sym_kernel(const CRec* __
                 }
                 __syncwarp();
                 flush(A, tb, ta == ta0);  // column sums: the i-stars of tile ta acting on the j-stars of tile tb
+                __syncwarp();
             }
+            buf ^= 1;
         }
-        __syncwarp();
 #pragma unroll
         for (int k = 0; k < I; ++k) store_acc(acc[k], lane + 32 * k);
         __syncwarp();
         flush(B, ta, (A < B) || (ta == ta0));  // row sums: the j-stars of group B acting on the i-stars of tile ta
+        __syncwarp();
     }
 }
 
