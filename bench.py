@@ -48,8 +48,9 @@ SMS, FP64_LANES_PER_SM = 148, 64
 # captures (per launch, cold L2: ncu flushes the caches before every replay), keyed by (variant, N_s); each entry names the
 # profiles/ file (which states the command and the kernel build) it was read from.  No entry -> "traffic": null.
 NCU_DRAM_BYTES_PER_PAIR_LAUNCH = {
-    (4, 16383): (805120 + 237312, "profiles/r1_ncu_summary.md section 2 (prof_r1c, pair_sym_fp64_kernel<4,1,8,0,1>, commit 32e2d05)"),
-    (4, 65535): (3248640 + 142522368, "profiles/r1_ncu_summary.md section 12 (prof_r1_c3, pair_sym_fp64_kernel<4,4,2,0,1>)"),
+    (4, 16383): (826624 + 185856, "profiles/r2_ncu_summary.md section 6 (r2_bench_c2, pair_sym_fp64_kernel<4,1,12,0,1,0,8,16>, round-2 build)"),
+    (4, 65535): (3268864 + 142611968, "profiles/r2_ncu_summary.md section 6 (r2_bench_c3, pair_sym_fp64_kernel<4,4,3,0,1,0,8,16>, round-2 build)"),
+    (8, 16383): (1872384 + 62415872, "profiles/r2_ncu_summary.md section 8 (r2_cross_sym, pair_cross_sym_kernel<8,0>, before the cp.async prefetch)"),
 }
 
 
@@ -74,6 +75,7 @@ def bench_lib():
         lib = ctypes.CDLL(str(build.BENCH_LIB))
         lib.pn_bench_fp64_peak.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_double)]
         lib.pn_bench_fp32_peak.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
+        lib.pn_bench_operand_probe.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
         _BENCH_LIB = lib
     return _BENCH_LIB
 
@@ -92,6 +94,36 @@ def measure_fp32_peak(stream, packed: bool) -> float:
     t = ctypes.c_double(0.0)
     rc = bench_lib().pn_bench_fp32_peak(ctypes.c_void_p(stream.cuda_stream), int(packed), ctypes.byref(t))
     return t.value if rc == 0 else None
+
+
+def run_probes(args) -> None:
+    """--probes: the operand-bandwidth micro-probes behind DESIGN.md section 6.1 (libpn_bench.so), one JSON line each: SM cycles
+    per DFMA warp-instruction and sub-partition (issue limit 2.0) for FP64 operand patterns, and for a two-register DFMA stream
+    with other-pipe instructions mixed in (what a second register operand of a non-FP64 instruction costs the FP64 stream)."""
+    import ctypes
+
+    import torch
+
+    torch.cuda.set_device(0)
+    st = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    cases = [(0, 0, 0, "DFMA, 2 distinct register operands"), (0, 1, 0, "DFMA, 3 distinct register operands"),
+             (0, 2, 0, "pairs a += K d (3 reads), b -= K d (d, K from the reuse cache)"),
+             (0, 3, 0, "3-register DFMA alternating with a 1-register DMUL"), (0, 4, 0, "1, 1, 3, 3 register operands"),
+             (1, 0, 0, "2-register DFMA stream alone")]
+    for nx in (4, 8):
+        cases += [(1, 1, nx, "+ SHFL.IDX, lane in a register (2 reads)"), (1, 2, nx, "+ SHFL.BFLY, immediate mask (1 read)"),
+                  (1, 3, nx, "+ IMAD (3 reads)"), (1, 4, nx, "+ MOV immediate (0 reads)"), (1, 5, nx, "+ LOP3 with immediate (1 read)"),
+                  (1, 6, nx, "+ FADD (2 reads)"), (1, 7, nx, "+ LDS.128 (1 read)")]
+    base = None
+    for kind, mode, nx, what in cases:
+        c = ctypes.c_double(0.0)
+        rc = bench_lib().pn_bench_operand_probe(st, kind, mode, nx, ctypes.byref(c))
+        line = {"probe": what, "kind": kind, "mode": mode, "other_per_16_dfma": nx, "cycles_per_dfma_per_subpartition": c.value if rc == 0 else None}
+        if kind == 1 and nx == 0:
+            base = c.value
+        if kind == 1 and nx and base and rc == 0:
+            line["fp64_cycles_lost_per_other_instruction"] = (c.value - base) * 16.0 / nx
+        print(json.dumps(line), flush=True)
 
 
 def load_peaks() -> dict:
@@ -698,11 +730,14 @@ def main():
     ap.add_argument("--t-end", type=float, default=10.0)
     ap.add_argument("--collapse-every", type=float, default=0.25, help="output interval in time units")
     ap.add_argument("--collapse-hot-path", action="store_true", help="without the Cross terms")
+    ap.add_argument("--probes", action="store_true", help="operand-bandwidth micro-probes of DESIGN.md section 6.1 (JSON lines)")
     ap.add_argument("--paper-timing", action="store_true",
                     help="the paper's timing experiment (PAPER.md:130-144, Table 3.2): 32 RK4 steps + 2 energy evaluations of "
                          "the full limited-1PN force at N = 100 ... 30000, one JSON line per N")
     args = ap.parse_args()
-    if args.cold_collapse:
+    if args.probes:
+        run_probes(args)
+    elif args.cold_collapse:
         run_cold_collapse(args)
     elif args.paper_timing:
         run_paper_timing(args)

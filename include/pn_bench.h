@@ -23,6 +23,15 @@ int pn_bench_fp64_peak(void* cuda_stream, double* tflops_host);
    instruction for two FMAs per thread), which the fp32-pair kernels use */
 int pn_bench_fp32_peak(void* cuda_stream, int packed, double* tflops_host);
 
+/* Operand-bandwidth probes behind DESIGN.md section 6.1 (`python bench.py --probes`).  A stream of DFMAs in one-warp blocks,
+   12 per SM; *cycles_host = SM cycles per DFMA warp-instruction and sub-partition at the rated clock (the issue limit is 2).
+   kind 0: FP64 operand patterns, mode 0: two distinct register operands; 1: three; 2: pairs a += K d, b -= K d (d and K from
+           the operand reuse cache in the second); 3: a three-register DFMA next to a one-register DMUL; 4: 1, 1, 3, 3.
+   kind 1: a two-register DFMA stream with nx (0, 4 or 8) other-pipe instructions per 16 DFMA, mode 1: SHFL.IDX with the lane
+           in a register (2 register reads); 2: SHFL.BFLY with an immediate mask (1); 3: IMAD (3); 4: MOV immediate (0);
+           5: LOP3 with an immediate (1); 6: FADD (2); 7: LDS.128 (1). */
+int pn_bench_operand_probe(void* cuda_stream, int kind, int mode, int nx, double* cycles_host);
+
 #ifdef __cplusplus
 }
 #endif

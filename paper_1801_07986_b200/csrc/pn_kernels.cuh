@@ -470,7 +470,7 @@ __global__ void __launch_bounds__(W * 32, MINB) pair_sym_fp64_kernel(const JRec*
                 sym_unit_tile<I, U, false, MASK, EQM, UNR>(sxy, szm, cw, xi, yi, zi, ngi, ax, ay, az, eps2, lane, i_local0, jb0, jb1);
             } else {
                 if (TRAV)
-                    sym_unit_tile_gray<I, U, EQM, TRAV ? TRAV : 16>(sxy, szm, cw, xi, yi, zi, ngi, ax, ay, az, eps2, lane, jb0, jb1);
+                    sym_unit_tile_gray<I, U, EQM, (TRAV == 8) ? 8 : 16>(sxy, szm, cw, xi, yi, zi, ngi, ax, ay, az, eps2, lane, jb0, jb1);
                 else
                     sym_unit_tile<I, U, true, false, EQM, UNR>(sxy, szm, cw, xi, yi, zi, ngi, ax, ay, az, eps2, lane, i_local0, jb0, jb1);
                 sym_sync<W>();

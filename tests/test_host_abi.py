@@ -129,7 +129,7 @@ def test_bench_probe_library_is_separate_and_exports_its_header():
     build.build()
     text = re.sub(r"/\*.*?\*/", "", (ROOT / "include" / "pn_bench.h").read_text(), flags=re.S)
     declared = sorted(set(re.findall(r"\b(pn_bench_[a-z_0-9]+)\s*\(", text)))
-    assert declared == ["pn_bench_fp32_peak", "pn_bench_fp64_peak"]
+    assert declared == ["pn_bench_fp32_peak", "pn_bench_fp64_peak", "pn_bench_operand_probe"]
     blib = ctypes.CDLL(str(build.BENCH_LIB))
     for name in declared:
         assert hasattr(blib, name)
