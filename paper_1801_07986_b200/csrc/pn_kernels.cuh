@@ -391,8 +391,10 @@ __device__ __forceinline__ void sym_sync()
         __syncthreads();
 }
 
-// adds n_src block-owned [3][U] tiles (consecutive in shared memory) into one (slot, tile) of part; the same thread
-// handles the same elements on every call, so read-modify-write sequences of one block need no fence
+// adds n_src block-owned [3][U] tiles (consecutive in shared memory) into one (slot, tile) of part.  Every element of part
+// has one writer in the whole launch, the same thread of the same block on every call: the first contribution is a plain
+// store, later ones are reductions to the same address by the same thread (RED.ADD.F64, applied in program order, no
+// read-modify-write latency), so the order of the sum stays fixed
 template <int U, int NT>
 __device__ __forceinline__ void sym_flush(const double* __restrict__ cacc, double* __restrict__ dst, int np, bool first,
                                           int n_src, int tid, double scale = 1.0)
@@ -403,7 +405,10 @@ __device__ __forceinline__ void sym_flush(const double* __restrict__ cacc, doubl
         for (int s = 1; s < n_src; ++s) v += cacc[s * 3 * U + q];
         v *= scale;
         double* d = dst + (size_t)c * np + el;
-        *d = first ? v : *d + v;
+        if (first)
+            *d = v;
+        else
+            atomicAdd(d, v);
     }
 }
 
@@ -794,7 +799,10 @@ __global__ void __launch_bounds__(32, MINB) pair_cross_sym_kernel(const CRec* __
         cacc[6][el] = a.S;
         if (BHX) cacc[7][el] = a.U;
     };
-    auto flush = [&](int slot, int tile, bool first) {  // cacc -> part[slot][NC][tile]; the same lane owns the same elements every time
+    // cacc -> part[slot][NC][tile].  Every element of part has ONE writer in the whole launch -- the same lane of the same block every
+    // time -- so its first contribution is a plain store and the later ones are reductions to the same address by the same thread
+    // (RED.ADD.F64: applied in program order, nothing to wait for), which keeps the sum's order fixed without a read-modify-write
+    auto flush = [&](int slot, int tile, bool first) {
         double* dst = part + (size_t)slot * NC * np + (size_t)tile * U;
 #pragma unroll
         for (int c = 0; c < NC; ++c)
@@ -802,7 +810,10 @@ __global__ void __launch_bounds__(32, MINB) pair_cross_sym_kernel(const CRec* __
             for (int q = lane; q < U; q += 32) {
                 double* p = dst + (size_t)c * np + q;
                 const double v = cacc[c][q];
-                *p = first ? v : *p + v;
+                if (first)
+                    *p = v;
+                else
+                    atomicAdd(p, v);
             }
     };
 
@@ -1208,7 +1219,10 @@ __device__ __forceinline__ void sym32_flush_cols(const float* __restrict__ cw, d
         for (int s = 1; s < n_src; ++s) v += (double)cw[s * 3 * U + q];
         v *= scale;
         double* d = dst + (size_t)c * np + el;
-        *d = first ? v : *d + v;
+        if (first)
+            *d = v;
+        else
+            atomicAdd(d, v);
     }
 }
 
