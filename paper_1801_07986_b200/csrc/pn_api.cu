@@ -252,7 +252,15 @@ int launch_small(pn_ctx* c, int mode, double dt, int64_t nsteps, double* acc_out
     const void* fn = (mode == MODE_RK4) ? small_kernel<MODE_RK4>(c->small_IW, mask) : small_kernel<MODE_ACCEL>(c->small_IW, mask);
     const size_t smem = (size_t)c->np * sizeof(JRec);
     void* args[] = {&a};
-    PN_CUDA(c, cudaLaunchCooperativeKernel(fn, dim3(c->small_blocks), dim3(kSmallNT), args, smem, c->stream));
+    cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(c->small_blocks), dim3(kSmallNT), args, smem, c->stream);
+    if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorLaunchOutOfResources) {
+        // the blocks cannot all be resident (SMs taken by another client of the device): nothing was launched; the callers fall
+        // back to the multi-kernel path for the rest of this context's life
+        cudaGetLastError();
+        c->small_ok = 0;
+        return PN_ESTATE;
+    }
+    PN_CUDA(c, e);
     const int64_t n_eval = (mode == MODE_RK4) ? 4 * nsteps : 1;
     c->small_bar_base += (unsigned int)((uint64_t)n_eval * (uint64_t)c->small_blocks);  // modulo 2^32, like the counter
     return PN_OK;
@@ -855,9 +863,12 @@ int pn_accel(pn_ctx* c, const double* pos, const double* vel, double* acc)
     pack_kernel<<<grid_pack, 256, 0, c->stream>>>(pos, vel, c->jrec[1], c->v[1], nullptr, nullptr, c->bh[1], c->n_stars, c->np, 0);
     PN_CUDA(c, cudaGetLastError());
     if (use_small(c)) {
-        if (int rc = launch_small(c, MODE_ACCEL, 0.0, 0, acc)) return rc;
-        c->n_launch += 2;
-        return PN_OK;
+        const int rc = launch_small(c, MODE_ACCEL, 0.0, 0, acc);
+        if (rc == PN_OK) {
+            c->n_launch += 2;
+            return PN_OK;
+        }
+        if (c->small_ok) return rc;  // a real error; otherwise: cooperative launch not possible right now, multi-kernel path
     }
     if (int rc = launch_pair(c, 1, c->stream, c->time_pair != 0)) return rc;
     const EpiArgs a = epi_args(c, 1, acc);
@@ -893,9 +904,12 @@ int pn_step(pn_ctx* c, double dt, int64_t nsteps)
     if (!c->have_state) return fail(c, PN_ESTATE, "pn_step: no state set (call pn_set_state first)");
     if (nsteps == 0) return PN_OK;
     if (use_small(c)) {  // every stage of every step in one cooperative launch (PN_OPT_USE_GRAPH / PN_OPT_TIME_PAIR do not apply)
-        if (int rc = launch_small(c, MODE_RK4, dt, nsteps, nullptr)) return rc;
-        c->n_launch += 1;
-        return PN_OK;
+        const int rc = launch_small(c, MODE_RK4, dt, nsteps, nullptr);
+        if (rc == PN_OK) {
+            c->n_launch += 1;
+            return PN_OK;
+        }
+        if (c->small_ok) return rc;  // a real error; otherwise: cooperative launch not possible right now, multi-kernel path
     }
     if (!(dt == c->dt_dev)) {
         StepParams p;
