@@ -6,6 +6,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -60,7 +61,8 @@ struct pn_ctx {
     // small-system path (small_path_kernel, one cooperative launch per pn_step / pn_accel call): i-stars per warp, blocks
     int small_ok = 0, small_IW = 0, small_blocks = 0;
     double* small_part = nullptr;      // [2][4 small_blocks][3] per-warp partials of a_1
-    unsigned int* small_bar = nullptr; // arrival counter of the grid barrier
+    unsigned int* small_bar = nullptr; // [2]: arrival counter of the grid barrier, give-up flag (small_check)
+    bool small_used = false;           // a small-path launch since the last check
     unsigned int small_bar_base = 0;   // its value when the next launch starts
 
     // device buffers.  Two stage sets: [0] integrator state, [1] scratch for pn_accel.
@@ -252,6 +254,16 @@ int launch_small(pn_ctx* c, int mode, double dt, int64_t nsteps, double* acc_out
     const void* fn = (mode == MODE_RK4) ? small_kernel<MODE_RK4>(c->small_IW, mask) : small_kernel<MODE_ACCEL>(c->small_IW, mask);
     const size_t smem = (size_t)c->np * sizeof(JRec);
     void* args[] = {&a};
+    // blocks of two grids that both spin at their own barrier must never share the device half and half: cooperative launches
+    // of this process run one after the other (each waits for the event the previous one recorded, on whatever stream)
+    static std::mutex g_small_mu;
+    static cudaEvent_t g_small_ev[16] = {};
+    std::lock_guard<std::mutex> lock(g_small_mu);
+    cudaEvent_t& chain = g_small_ev[c->device & 15];
+    if (chain)
+        PN_CUDA(c, cudaStreamWaitEvent(c->stream, chain, 0));
+    else
+        PN_CUDA(c, cudaEventCreateWithFlags(&chain, cudaEventDisableTiming));
     cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(c->small_blocks), dim3(kSmallNT), args, smem, c->stream);
     if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorLaunchOutOfResources) {
         // the blocks cannot all be resident (SMs taken by another client of the device): nothing was launched; the callers fall
@@ -261,6 +273,8 @@ int launch_small(pn_ctx* c, int mode, double dt, int64_t nsteps, double* acc_out
         return PN_ESTATE;
     }
     PN_CUDA(c, e);
+    PN_CUDA(c, cudaEventRecord(chain, c->stream));
+    c->small_used = true;
     const int64_t n_eval = (mode == MODE_RK4) ? 4 * nsteps : 1;
     c->small_bar_base += (unsigned int)((uint64_t)n_eval * (uint64_t)c->small_blocks);  // modulo 2^32, like the counter
     return PN_OK;
@@ -286,8 +300,8 @@ cudaError_t prepare_small(pn_ctx* c)
             if (e != cudaSuccess) return e;
         }
     e = dalloc(&c->small_part, 2 * 3 * (size_t)4 * c->small_blocks);
-    if (e == cudaSuccess) e = dalloc(&c->small_bar, 1);
-    if (e == cudaSuccess) e = cudaMemset(c->small_bar, 0, sizeof(unsigned int));
+    if (e == cudaSuccess) e = dalloc(&c->small_bar, 2);
+    if (e == cudaSuccess) e = cudaMemset(c->small_bar, 0, 2 * sizeof(unsigned int));
     if (e == cudaSuccess) c->small_ok = 1;
     return e;
 }
@@ -575,6 +589,21 @@ int check_ctx(pn_ctx* c)
     return PN_OK;
 }
 
+// after a synchronisation of the context's stream: did a grid barrier of the small-system path give up?  (one 4-byte read)
+int small_check(pn_ctx* c)
+{
+    if (!c->small_used) return PN_OK;
+    c->small_used = false;
+    unsigned int flag = 0;
+    PN_CUDA(c, cudaMemcpy(&flag, c->small_bar + 1, sizeof flag, cudaMemcpyDeviceToHost));
+    if (!flag) return PN_OK;
+    cudaMemset(c->small_bar, 0, 2 * sizeof(unsigned int));
+    c->small_bar_base = 0;
+    c->small_ok = 0;
+    return fail(c, PN_ECUDA, "small-system path: a grid barrier timed out (the results of the last pn_step / pn_accel are invalid); "
+                             "the context uses the multi-kernel path from now on");
+}
+
 }  // namespace
 
 // =================================================================================================== C-ABI ==
@@ -852,6 +881,7 @@ int pn_get_state_host(pn_ctx* c, double* pos, double* vel)
     PN_CUDA(c, cudaMemcpyAsync(pos, c->io_pos, bytes, cudaMemcpyDeviceToHost, c->stream));
     PN_CUDA(c, cudaMemcpyAsync(vel, c->io_vel, bytes, cudaMemcpyDeviceToHost, c->stream));
     PN_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (int rc = small_check(c)) return rc;
     return PN_OK;
 }
 
@@ -893,6 +923,7 @@ int pn_accel_host(pn_ctx* c, const double* pos, const double* vel, double* acc)
     if (int rc = pn_accel(c, c->io_pos, c->io_vel, c->io_acc)) return rc;
     PN_CUDA(c, cudaMemcpyAsync(acc, c->io_acc, bytes, cudaMemcpyDeviceToHost, c->stream));
     PN_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (int rc = small_check(c)) return rc;
     return PN_OK;
 }
 
@@ -978,6 +1009,7 @@ int pn_energy(pn_ctx* c, double* E)
     c->n_launch += 3;
     PN_CUDA(c, cudaMemcpyAsync(E, c->d_energy, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     PN_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (int rc = small_check(c)) return rc;
     return PN_OK;
 }
 
@@ -1004,6 +1036,7 @@ int pn_momentum(pn_ctx* c, double* P)
     c->n_launch += 4;
     PN_CUDA(c, cudaMemcpyAsync(P, d_out, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     PN_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (int rc = small_check(c)) return rc;
     return PN_OK;
 }
 

@@ -1571,7 +1571,7 @@ struct SmallArgs {
     double *x0, *v0, *sx, *sv;
     BhState* bh;
     double* bh_part;     // [2][warps of the grid][3]: evaluation e writes set e & 1
-    unsigned int* bar;   // arrival counter of the grid barrier (monotonic; bar_base = its value at launch)
+    unsigned int* bar;   // [2]: arrival counter of the grid barrier (monotonic; bar_base = its value at launch), give-up flag
     double* acc_out;     // MODE_ACCEL: [N][3]
     int n_stars, np;
     double GM, inv_c2, eps2, dt;
@@ -1605,15 +1605,22 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned int 
 
 constexpr int kSmallNT = 128;  // threads per block of small_path_kernel (one warp per SM sub-partition)
 
+// ctr[0]: arrivals (monotonic); ctr[1]: set if a wait ever gave up.  The wait is bounded (about half a minute of polling) so
+// that a broken invariant -- blocks not all resident, a counter out of step with the host's copy -- ends in an error the host
+// reports (pn_api.cu: small_check) instead of a hung device.
 __device__ __forceinline__ void small_grid_barrier(unsigned int* ctr, unsigned int target)
 {
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();  // this block's global writes are visible before its arrival is
         atomicAdd(ctr, 1u);
-        unsigned int seen;
+        unsigned int seen, polls = 0;
         do {
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(ctr) : "memory");
+            if (++polls == (1u << 26)) {
+                atomicExch(ctr + 1, 1u);
+                break;
+            }
         } while ((int)(seen - target) < 0);
     }
     __syncthreads();

@@ -96,3 +96,31 @@ def test_small_path_accel_between_steps_does_not_disturb_the_state():
         pn.pn_step(p.dt, 3)
         got = pn.pn_get_state_host()
     assert np.array_equal(ref[0], got[0]) and np.array_equal(ref[1], got[1])
+
+
+def test_two_small_contexts_on_two_streams():
+    """Cooperative launches of two contexts never share the device half and half (each spins at its own grid barrier):
+    the library chains them; interleaved stepping on two streams gives each context its sequential result."""
+    from paper_1801_07986_b200 import PN
+
+    ps = [inputs.plummer_bh(900, seed=41, dt=1e-3), inputs.plummer_bh(2100, seed=42, dt=1e-3)]
+    ref = []
+    for p in ps:
+        with PN(p.mass, p.G, p.c, p.softening) as pn:
+            pn.pn_set_state_host(p.pos, p.vel)
+            pn.pn_step(p.dt, 12)
+            ref.append(pn.pn_get_state_host())
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    pns = [PN(p.mass, p.G, p.c, p.softening, stream=s) for p, s in zip(ps, streams)]
+    try:
+        for pn, p in zip(pns, ps):
+            pn.pn_set_state_host(p.pos, p.vel)
+        for _ in range(4):  # 4 x 3 steps each, enqueued alternately without synchronising in between
+            for pn, p in zip(pns, ps):
+                pn.pn_step(p.dt, 3)
+        got = [pn.pn_get_state_host() for pn in pns]
+    finally:
+        for pn in pns:
+            pn.pn_destroy()
+    for (x, v), (xr, vr) in zip(got, ref):
+        assert np.array_equal(x, xr) and np.array_equal(v, vr)
