@@ -79,7 +79,8 @@ struct pn_ctx {
     FRec* frec = nullptr;  // two-float records of the fp32-pair variant, rebuilt before every pair launch (tiled kernel)
     FPair* fpair = nullptr;  // the same for pairs of consecutive stars: packed operands of the symmetric f32x2 kernel
     double *blk_prep = nullptr, *blk_pair = nullptr, *d_energy = nullptr;
-    int e_split = 1;
+    int e_blocks = 1;            // blocks of the energy / momentum pair kernels
+    long long e_per_block = 1;   // tile pairs (it <= jt) each of them walks
 
     bool have_state = false;
     double dt_dev = NAN;
@@ -706,13 +707,14 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses, double G, double c,
     CREATE_CUDA(dalloc(&ctx->fpair, np / 2));
     {
         const int n_it = (int)(np / kNT);
-        // the energy pair kernel runs n_it / 2 mirrored i-tile pairs per j-split, all of equal work: aim at one full wave
-        // (7 blocks of 72 registers x 128 threads per SM) rather than a full wave plus a short one
-        int s = (ctx->n_sm * 7) / (n_it / 2);
-        s = std::max(1, std::min(s, std::min(ctx->n_tiles, 64)));
-        ctx->e_split = s;  // each i-tile splits its own range of j-tiles into e_split chunks inside the kernel
+        // the energy / momentum pair kernels share out the n_it (n_it + 1) / 2 tile pairs (it <= jt) evenly: one full wave of
+        // blocks (7 of 72 registers x 128 threads per SM), every block the same number of consecutive pairs
+        const long long n_pairs = (long long)n_it * (n_it + 1) / 2;
+        const long long want = (long long)ctx->n_sm * 7;
+        ctx->e_per_block = std::max(1LL, (n_pairs + want - 1) / want);
+        ctx->e_blocks = (int)((n_pairs + ctx->e_per_block - 1) / ctx->e_per_block);
         CREATE_CUDA(dalloc(&ctx->blk_prep, 4 * (size_t)n_it));
-        CREATE_CUDA(dalloc(&ctx->blk_pair, 2 * (size_t)n_it * ctx->e_split));
+        CREATE_CUDA(dalloc(&ctx->blk_pair, 2 * (size_t)ctx->e_blocks));
         CREATE_CUDA(dalloc(&ctx->d_energy, 1));
     }
 
@@ -999,11 +1001,10 @@ int pn_energy(pn_ctx* c, double* E)
     energy_prep_kernel<kNT><<<n_it, kNT, 0, c->stream>>>(c->jrec[0], c->v[0], c->bh[0], c->erec, c->blk_prep, c->n_stars, c->np,
                                                         c->GM, c->G, c->inv_c2);
     PN_CUDA(c, cudaGetLastError());
-    dim3 grid(n_it / 2, c->e_split);
-    energy_pair_kernel<kNT, kTJ><<<grid, kNT, 0, c->stream>>>(c->erec, c->blk_pair, c->n_stars, c->np, c->eps2, c->G,
+    energy_pair_kernel<kNT, kTJ><<<c->e_blocks, kNT, 0, c->stream>>>(c->erec, c->blk_pair, c->n_stars, c->np, c->e_per_block, c->eps2, c->G,
                                                               c->inv_c2);
     PN_CUDA(c, cudaGetLastError());
-    energy_final_kernel<256><<<1, 256, 0, c->stream>>>(c->blk_prep, n_it, c->blk_pair, (n_it / 2) * c->e_split, c->bh[0], c->M, c->GM,
+    energy_final_kernel<256><<<1, 256, 0, c->stream>>>(c->blk_prep, n_it, c->blk_pair, c->e_blocks, c->bh[0], c->M, c->GM,
                                                        c->G, c->inv_c2, c->d_energy);
     PN_CUDA(c, cudaGetLastError());
     c->n_launch += 3;
@@ -1019,19 +1020,18 @@ int pn_momentum(pn_ctx* c, double* P)
     if (!P) return fail(c, PN_EINVAL, "pn_momentum: null pointer");
     if (!c->have_state) return fail(c, PN_ESTATE, "pn_momentum: no state set");
     const int n_it = c->np / kNT;
-    if (!c->blk_mom) {  // [n_it][6] + [n_it * e_split][6] + 3 results, on first use
-        PN_CUDA(c, dalloc(&c->blk_mom, 6 * (size_t)n_it * (1 + c->e_split) + 3));
+    if (!c->blk_mom) {  // [n_it][6] + [e_blocks][6] + 3 results, on first use
+        PN_CUDA(c, dalloc(&c->blk_mom, 6 * ((size_t)n_it + c->e_blocks) + 3));
     }
     double* blk_prep = c->blk_mom;
     double* blk_pair = c->blk_mom + 6 * (size_t)n_it;
-    double* d_out = blk_pair + 6 * (size_t)n_it * c->e_split;
+    double* d_out = blk_pair + 6 * (size_t)c->e_blocks;
     energy_prep_kernel<kNT><<<n_it, kNT, 0, c->stream>>>(c->jrec[0], c->v[0], c->bh[0], c->erec, c->blk_prep, c->n_stars, c->np,
                                                         c->GM, c->G, c->inv_c2);  // builds the ERec stream
     momentum_prep_kernel<kNT><<<n_it, kNT, 0, c->stream>>>(c->jrec[0], c->v[0], c->bh[0], blk_prep, c->n_stars, c->np, c->GM, c->G,
                                                           c->inv_c2);
-    dim3 grid(n_it, c->e_split);
-    momentum_pair_kernel<kNT, kTJ><<<grid, kNT, 0, c->stream>>>(c->erec, blk_pair, c->n_stars, c->np, c->eps2, c->G);
-    momentum_final_kernel<256><<<1, 256, 0, c->stream>>>(blk_prep, n_it, blk_pair, n_it * c->e_split, c->bh[0], c->M, c->inv_c2, d_out);
+    momentum_pair_kernel<kNT, kTJ><<<c->e_blocks, kNT, 0, c->stream>>>(c->erec, blk_pair, c->n_stars, c->np, c->e_per_block, c->eps2, c->G);
+    momentum_final_kernel<256><<<1, 256, 0, c->stream>>>(blk_prep, n_it, blk_pair, c->e_blocks, c->bh[0], c->M, c->inv_c2, d_out);
     PN_CUDA(c, cudaGetLastError());
     c->n_launch += 4;
     PN_CUDA(c, cudaMemcpyAsync(P, d_out, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));

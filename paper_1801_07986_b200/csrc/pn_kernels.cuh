@@ -1954,11 +1954,26 @@ __global__ void __launch_bounds__(NT) energy_prep_kernel(const JRec* __restrict_
     }
 }
 
-// O(N^2) part: Epair is symmetric in (i, j), so only the unordered pairs i < j are visited: thread i walks the
-// j-tiles from its own tile upwards and skips j <= i.  grid = (i-tiles, j-splits of that i-tile's own range).
+// The upper-triangular list of tile pairs (it <= jt), row by row: row it holds the n_tiles - it pairs (it, it), ..., (it, n_tiles - 1).
+// Every block of the energy / momentum pair kernels takes the same number of consecutive entries of that list, so all blocks
+// carry the same work to within one tile pair (the mirrored i-tile scheme of round 1 left a 12 % spread between blocks).
+__device__ __forceinline__ void tri_decode(long long p, int n_tiles, int& it, int& jt)
+{
+    // offset(it) = it n_tiles - it (it - 1) / 2 <= p
+    const double b = 2.0 * n_tiles + 1.0;
+    int r = (int)((b - sqrt(b * b - 8.0 * (double)p)) * 0.5);
+    r = max(0, min(r, n_tiles - 1));
+    auto off = [&](int q) { return (long long)q * n_tiles - (long long)q * (q - 1) / 2; };
+    while (r > 0 && off(r) > p) --r;
+    while (r + 1 < n_tiles && off(r + 1) <= p) ++r;
+    it = r, jt = r + (int)(p - off(r));
+}
+
+// O(N^2) part: Epair is symmetric in (i, j), so only the unordered pairs i < j are visited: tile pairs (it <= jt), thread = i-star
+// of tile it, j records of tile jt broadcast from shared memory; inside the diagonal tile j <= i is masked.
 template <int NT, int TJ>
 __global__ void __launch_bounds__(NT) energy_pair_kernel(const ERec* __restrict__ erec, double* __restrict__ blk /* [grid][2] */,
-                                                         int n_stars, int np, double eps2, double G, double inv_c2)
+                                                         int n_stars, int np, long long per_block, double eps2, double G, double inv_c2)
 {
     __shared__ ERec sj[TJ];
     __shared__ double red[2 * (NT / 32)];
@@ -1967,67 +1982,75 @@ __global__ void __launch_bounds__(NT) energy_pair_kernel(const ERec* __restrict_
     static_assert(TJ % kEGroup == 0, "tile must be a multiple of the summation group");
     static_assert(NT == TJ, "i-tiles and j-tiles share one index space");
     const double c35 = 3.5 * inv_c2, c05 = 0.5 * inv_c2;
-    const int n_tiles = np / TJ;  // even (np is a multiple of 2 NT)
-    double hi = 0, lo = 0;
-
-    // i-tile `it` has n_tiles - it j-tiles to walk: a block takes tile blockIdx.x and its mirror n_tiles - 1 - blockIdx.x,
-    // so every block of the grid (n_tiles / 2, j-splits) has the same amount of work
-    for (int half = 0; half < 2; ++half) {
-        const int it = half ? n_tiles - 1 - (int)blockIdx.x : (int)blockIdx.x;
-        const int i = it * NT + tid;
-        const ERec me = erec[i];
-        const double wi1 = me.w - 1.0;
-        double h_hi = 0, h_lo = 0;
-        const int per = (n_tiles - it + (int)gridDim.y - 1) / (int)gridDim.y;
-        const int t_begin = it + blockIdx.y * per;
-        const int t_end = min(n_tiles, t_begin + per);
-        for (int t = t_begin; t < t_end; ++t) {
-            __syncthreads();
-            {
-                const double2* src = reinterpret_cast<const double2*>(erec + (size_t)t * TJ);
-                double2* dst = reinterpret_cast<double2*>(sj);
-                for (int q = tid; q < TJ * 4; q += NT) dst[q] = src[q];
-            }
-            __syncthreads();
-            const int j0 = t * TJ;
-#pragma unroll 1
-            for (int jb = 0; jb < TJ; jb += kEGroup) {
-                // kEGroup terms are added plainly (their sum is tiny next to the running total), then the group sum
-                // goes into the compensated accumulator: one TwoSum per kEGroup pairs instead of one per pair
-                double g = 0.0;
-#pragma unroll
-                for (int u = 0; u < kEGroup; ++u) {
-                    const int jj = jb + u;
-                    const ERec r = sj[jj];
-                    const double dx = me.x - r.x, dy = me.y - r.y, dz = me.z - r.z;  // x_ij
-                    const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
-                    const double y0 = rsqrt_seed(r2);
-                    const double t2 = y0 * y0;
-                    const double e = fma(-r2, t2, 1.0);
-                    const double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1/rho to full fp64 accuracy
-                    const double vv = fma(me.vx, r.vx, fma(me.vy, r.vy, me.vz * r.vz));
-                    const double xvi = fma(dx, me.vx, fma(dy, me.vy, dz * me.vz));
-                    const double xvj = fma(dx, r.vx, fma(dy, r.vy, dz * r.vz));
-                    // q = -1 + (1/c^2)[w_i + w_j - 7/2 v_i.v_j - 1/2 (x_ij.v_i)(x_ij.v_j)/rho^2]; me.w, r.w carry the 1/c^2
-                    double q = wi1 + r.w;
-                    q = fma(-c35, vv, q);
-                    q = fma(-c05, (xvi * xvj) * (y * y), q);
-                    double term = (r.gm * y) * q;
-                    term = (j0 + jj <= i) ? 0.0 : term;  // i < j only (false only inside the diagonal tile)
-                    g += term;
-                }
-                two_sum_acc(h_hi, h_lo, g);
-            }
-        }
-        if (i < n_stars) {  // the factor m_i is common to all of star i's pairs
+    const int n_tiles = np / TJ;
+    const long long n_pairs = (long long)n_tiles * (n_tiles + 1) / 2;
+    const long long p0 = (long long)blockIdx.x * per_block, p1 = min(n_pairs, p0 + per_block);
+    double hi = 0, lo = 0;      // this thread's total: sum over its i-stars of m_i * (their pair sums)
+    double h_hi = 0, h_lo = 0;  // pair sum of the current i-star
+    int it = 0, jt = 0;
+    if (p0 < p1) tri_decode(p0, n_tiles, it, jt);
+    int i = it * NT + tid;
+    ERec me = erec[i];
+    double wi1 = me.w - 1.0;
+    auto close_row = [&]() {  // the factor m_i is common to all of star i's pairs
+        if (i < n_stars) {
             const double mi = me.gm / G;
             two_sum_acc(hi, lo, h_hi * mi);
             lo += h_lo * mi;
         }
+        h_hi = h_lo = 0;
+    };
+    for (long long p = p0; p < p1; ++p) {
+        __syncthreads();
+        {
+            const double2* src = reinterpret_cast<const double2*>(erec + (size_t)jt * TJ);
+            double2* dst = reinterpret_cast<double2*>(sj);
+            for (int q = tid; q < TJ * 4; q += NT) dst[q] = src[q];
+        }
+        __syncthreads();
+        const int j0 = jt * TJ;
+#pragma unroll 1
+        for (int jb = 0; jb < TJ; jb += kEGroup) {
+            // kEGroup terms are added plainly (their sum is tiny next to the running total), then the group sum
+            // goes into the compensated accumulator: one TwoSum per kEGroup pairs instead of one per pair
+            double g = 0.0;
+#pragma unroll
+            for (int u = 0; u < kEGroup; ++u) {
+                const int jj = jb + u;
+                const ERec r = sj[jj];
+                const double dx = me.x - r.x, dy = me.y - r.y, dz = me.z - r.z;  // x_ij
+                const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+                const double y0 = rsqrt_seed(r2);
+                const double t2 = y0 * y0;
+                const double e = fma(-r2, t2, 1.0);
+                const double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1/rho to full fp64 accuracy
+                const double vv = fma(me.vx, r.vx, fma(me.vy, r.vy, me.vz * r.vz));
+                const double xvi = fma(dx, me.vx, fma(dy, me.vy, dz * me.vz));
+                const double xvj = fma(dx, r.vx, fma(dy, r.vy, dz * r.vz));
+                // q = -1 + (1/c^2)[w_i + w_j - 7/2 v_i.v_j - 1/2 (x_ij.v_i)(x_ij.v_j)/rho^2]; me.w, r.w carry the 1/c^2
+                double q = wi1 + r.w;
+                q = fma(-c35, vv, q);
+                q = fma(-c05, (xvi * xvj) * (y * y), q);
+                double term = (r.gm * y) * q;
+                term = (j0 + jj <= i) ? 0.0 : term;  // i < j only (false only inside the diagonal tile)
+                g += term;
+            }
+            two_sum_acc(h_hi, h_lo, g);
+        }
+        if (++jt == n_tiles) {  // next row of the list: the next i-tile, starting at its diagonal pair
+            close_row();
+            ++it, jt = it;
+            if (p + 1 < p1) {
+                i = it * NT + tid;
+                me = erec[i];
+                wi1 = me.w - 1.0;
+            }
+        }
     }
+    close_row();
     block_sum_dd<NT>(hi, lo, red);
     if (tid == 0) {
-        double* b = blk + 2 * ((size_t)blockIdx.y * gridDim.x + blockIdx.x);
+        double* b = blk + 2 * (size_t)blockIdx.x;
         b[0] = hi, b[1] = lo;
     }
 }
@@ -2109,29 +2132,43 @@ __global__ void __launch_bounds__(NT) momentum_prep_kernel(const JRec* __restric
 
 template <int NT, int TJ>
 __global__ void __launch_bounds__(NT) momentum_pair_kernel(const ERec* __restrict__ erec, double* __restrict__ blk /* [grid][6] */,
-                                                           int n_stars, int np, double eps2, double G)
+                                                           int n_stars, int np, long long per_block, double eps2, double G)
 {
     static_assert(NT == TJ, "i-tiles and j-tiles share one index space");
     constexpr int kGroup = 8;
     __shared__ ERec sj[TJ];
     __shared__ double red[2 * (NT / 32)];
     const int tid = threadIdx.x;
-    const int i = blockIdx.x * NT + tid;
-    const ERec me = erec[i];
-    double hi[3] = {0, 0, 0}, lo[3] = {0, 0, 0};
     const int n_tiles = np / TJ;
-    const int per = (n_tiles - (int)blockIdx.x + (int)gridDim.y - 1) / (int)gridDim.y;
-    const int t_begin = blockIdx.x + blockIdx.y * per;
-    const int t_end = min(n_tiles, t_begin + per);
-    for (int t = t_begin; t < t_end; ++t) {
+    const long long n_pairs = (long long)n_tiles * (n_tiles + 1) / 2;
+    const long long p0 = (long long)blockIdx.x * per_block, p1 = min(n_pairs, p0 + per_block);
+    double tot_hi[3] = {0, 0, 0}, tot_lo[3] = {0, 0, 0};  // this thread's total over its i-stars, m_i applied
+    double hi[3] = {0, 0, 0}, lo[3] = {0, 0, 0};          // the current i-star's pair sums
+    int it = 0, jt = 0;
+    if (p0 < p1) tri_decode(p0, n_tiles, it, jt);
+    int i = it * NT + tid;
+    ERec me = erec[i];
+    auto close_row = [&]() {
+        if (i < n_stars) {  // pad stars (coincident, massless) may hold NaN with eps = 0
+            const double mi = me.gm / G;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                two_sum_acc(tot_hi[k], tot_lo[k], hi[k] * mi);
+                tot_lo[k] += lo[k] * mi;
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) hi[k] = lo[k] = 0;
+    };
+    for (long long p = p0; p < p1; ++p) {
         __syncthreads();
         {
-            const double2* src = reinterpret_cast<const double2*>(erec + (size_t)t * TJ);
+            const double2* src = reinterpret_cast<const double2*>(erec + (size_t)jt * TJ);
             double2* dst = reinterpret_cast<double2*>(sj);
             for (int q = tid; q < TJ * 4; q += NT) dst[q] = src[q];
         }
         __syncthreads();
-        const int j0 = t * TJ;
+        const int j0 = jt * TJ;
 #pragma unroll 1
         for (int jb = 0; jb < TJ; jb += kGroup) {
             double g[3] = {0, 0, 0};
@@ -2155,13 +2192,20 @@ __global__ void __launch_bounds__(NT) momentum_pair_kernel(const ERec* __restric
 #pragma unroll
             for (int k = 0; k < 3; ++k) two_sum_acc(hi[k], lo[k], g[k]);
         }
+        if (++jt == n_tiles) {
+            close_row();
+            ++it, jt = it;
+            if (p + 1 < p1) {
+                i = it * NT + tid;
+                me = erec[i];
+            }
+        }
     }
-    const bool real_star = i < n_stars;  // pad stars (coincident, massless) may hold NaN with eps = 0
-    const double mi = me.gm / G;
-    double* b = blk + 6 * ((size_t)blockIdx.y * gridDim.x + blockIdx.x);
+    close_row();
+    double* b = blk + 6 * (size_t)blockIdx.x;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        double h = real_star ? hi[k] * mi : 0.0, l = real_star ? lo[k] * mi : 0.0;
+        double h = tot_hi[k], l = tot_lo[k];
         block_sum_dd<NT>(h, l, red);
         if (tid == 0) b[2 * k] = h, b[2 * k + 1] = l;
     }
