@@ -87,7 +87,7 @@ extern "C" {
 #define PN_FP32_PAIR 1 /* fp32 pair arithmetic on two-float positions, fp64 accumulation (parity 1e-5) */
 
 /* PN_OPT_PAIR_KERNEL values (either pair precision) */
-#define PN_PAIR_AUTO 0      /* symmetric for N - 1 >= 3072 stars (unit tiles of 128 stars, 512 from 40000 stars on).  Below
+#define PN_PAIR_AUTO 0      /* symmetric for N - 1 >= 3072 stars (unit tiles of 128 stars, 512 from 36000 stars on).  Below
                                (fp64, no Cross terms): the small-system path -- ONE cooperative kernel launch runs a whole
                                pn_step call (every stage of every step) or one pn_accel, every ordered pair, 15 instructions;
                                it needs a device with cooperative launch and as many SMs as blocks (else: tiled) */

@@ -155,11 +155,14 @@ enum { SYM_W1_U128 = 0, SYM_JS_U128 = 1, SYM_W4_U512 = 2 };
 
 void choose_sym(pn_ctx* c)
 {
-    if (c->n_stars < 12288)
+    // measured with the Gray-code walk (profiles/r2_ncu_summary.md section 4): one-warp blocks win only where 120 - 128 one-tile
+    // groups give 7260 - 8256 items of one 128 x 128 tile pair (N_s = 16383: 0.763 against 0.756); below and above (two-tile
+    // groups from 16385 stars on) the j-split form, whose items are a quarter as long; 512-star tiles from 36000 stars on
+    if (c->n_stars < 15360)
         c->sym_kind = SYM_JS_U128;
-    else if (c->n_stars < 20000)
+    else if (c->n_stars <= 16384)
         c->sym_kind = SYM_W1_U128;
-    else if (c->n_stars < 40000)
+    else if (c->n_stars < 36000)
         c->sym_kind = SYM_JS_U128;
     else
         c->sym_kind = SYM_W4_U512;
