@@ -36,13 +36,15 @@ if str(ROOT) not in sys.path:
 #   5 ordered pairs with the Cross terms of Eq. 2.6 (--cross): 36 DADD + 124 DFMA + 56 DMUL per 4 pairs = 54 per ordered pair
 #   6 the same plus the O(N^2) sum of Eq. 2.3 (--cross full): 59 per ordered pair
 #   8 / 9 the Cross terms on every UNORDERED pair (pair_cross_sym_kernel, N_s >= 6144): 768 DFMA + 176 DADD + 272 DMUL per 16
-#     unordered pairs = 38 per ordered pair (42 with the sum of Eq. 2.3: 832 + 192 + 320)
+#     unordered pairs = 38 per ordered pair (42 with the sum of Eq. 2.3: 832 + 192 + 320); 10 / 11: the equal-mass form of the
+#     same kernel (the common G m applied at the flush): 736 + 208 + 240 = 37 per ordered pair (800 + 224 + 256 = 40)
 #   7 small-system path (N_s < 3072): ONE cooperative launch per pn_step / pn_accel call, every ordered pair in the tiled
 #     kernel's 15-instruction form; there is no separate pair stage to time, the launch is the whole call
 PAIR_KERNELS = {0: ("pair_fp64_kernel", 15, 24.0), 2: ("pair_sym_fp64_kernel", 10, 16.0),
                 4: ("pair_sym_fp64_kernel<EQM>", 9, 15.0), 5: ("pair_cross_fp64_kernel", 54, 85.0),
                 6: ("pair_cross_fp64_kernel<BHX>", 59, 93.0), 7: ("small_path_kernel", 15, 24.0),
-                8: ("pair_cross_sym_kernel", 38, 62.0), 9: ("pair_cross_sym_kernel<BHX>", 42, 68.0)}
+                8: ("pair_cross_sym_kernel", 38, 62.0), 9: ("pair_cross_sym_kernel<BHX>", 42, 68.0),
+                10: ("pair_cross_sym_kernel<EQM>", 37, 60.0), 11: ("pair_cross_sym_kernel<BHX, EQM>", 40, 65.0)}
 SMS, FP64_LANES_PER_SM = 148, 64
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed `ncu --set full`
 # captures (per launch, cold L2: ncu flushes the caches before every replay), keyed by (variant, N_s); each entry names the

@@ -73,12 +73,12 @@ extern "C" {
                                    its O(N^2) sums are fused into an fp64 pair kernel that also produces the Newtonian
                                    star-star term, its O(N) parts go into the epilogue.  From 6144 stars on that kernel
                                    evaluates every UNORDERED pair once for both stars (38 FP64 instructions per ordered
-                                   pair), below every ordered pair (54); PN_OPT_PAIR_KERNEL = PN_PAIR_SYMMETRIC /
+                                   pair, 37 with equal masses), below every ordered pair (54); PN_OPT_PAIR_KERNEL = PN_PAIR_SYMMETRIC /
                                    PN_PAIR_TILED forces either.  PN_CROSS_STAR | PN_CROSS_BH: also [a_1]_Cross, Eq. 2.3
                                    (PAPER.md:51-57), the second NEXT row -- the paper's full limited-1PN force (one more
                                    O(N^2) sum per star in the same kernel, 42 / 59 instructions per pair; the rest is O(N)).
                                    Applies to pn_accel and pn_step; pn_energy is Eq. 2.7 either way.  The Cross path is fp64
-                                   only: while it is on, PN_OPT_PAIR_PRECISION and PN_OPT_EQUAL_MASS have no effect. */
+                                   only: while it is on, PN_OPT_PAIR_PRECISION has no effect. */
 #define PN_CROSS_STAR 1
 #define PN_CROSS_BH 2
 

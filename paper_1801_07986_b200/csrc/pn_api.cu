@@ -417,17 +417,22 @@ int launch_pair(pn_ctx* c, int set, cudaStream_t st, bool timed)
     const bool mask = (c->eps2 == 0.0);
     if (c->cross) {  // NEXT-1: star-star Newtonian + pair part of [a_i]_Cross in one ordered-pair pass (fp64)
         const int nb = c->np / kNT;
-        cross_prep_kernel<kNT><<<nb, kNT, 0, st>>>(c->jrec[set], c->v[set], c->bh[set], c->crec, c->cblk, c->n_stars, c->np, c->GM);
+        const bool ceqm = cross_sym(c) && c->equal_mass && c->eqm_opt;  // equal-mass form of the symmetric Cross kernel
+        cross_prep_kernel<kNT><<<nb, kNT, 0, st>>>(c->jrec[set], c->v[set], c->bh[set], c->crec, c->cblk, c->n_stars, c->np, c->GM,
+                                                  ceqm ? 1.0 / c->gm_eq : 1.0);
         cross_sum_kernel<<<1, 256, 0, st>>>(c->cblk, nb, c->csum);
         const double GM4 = 4.0 * c->GM;
         if (cross_sym(c)) {  // every unordered pair once
             const int items = c->c_G * (c->c_G + 1) / 2;
-            if (c->cross & PN_CROSS_BH)
-                pair_cross_sym_kernel<kCrossSymMinB, true><<<items, 32, kCrossSymSmemBytes<true>, st>>>(c->crec, c->part6, c->np, c->c_T, c->c_m,
-                                                                                                         c->eps2, GM4);
+            const bool bhx = (c->cross & PN_CROSS_BH) != 0;
+#define PN_LAUNCH_CSYM(B, E)                                                                                                          \
+    pair_cross_sym_kernel<kCrossSymMinB, B, E><<<items, 32, kCrossSymSmemBytes<B>, st>>>(c->crec, c->part6, c->np, c->c_T, c->c_m, c->eps2, \
+                                                                                         GM4, c->gm_eq)
+            if (bhx)
+                ceqm ? PN_LAUNCH_CSYM(true, true) : PN_LAUNCH_CSYM(true, false);
             else
-                pair_cross_sym_kernel<kCrossSymMinB, false><<<items, 32, kCrossSymSmemBytes<false>, st>>>(c->crec, c->part6, c->np, c->c_T, c->c_m,
-                                                                                                           c->eps2, GM4);
+                ceqm ? PN_LAUNCH_CSYM(false, true) : PN_LAUNCH_CSYM(false, false);
+#undef PN_LAUNCH_CSYM
         } else {
             dim3 grid(c->np / (kCrossI * kNT), c->c_split);
             if (c->cross & PN_CROSS_BH)
@@ -816,8 +821,10 @@ int pn_set_option(pn_ctx* c, int key, int value)
                 c->c_T = c->np / kCrossSymU;
                 c->c_m = (c->c_T + kCrossSymMaxGroups - 1) / kCrossSymMaxGroups;
                 c->c_G = (c->c_T + c->c_m - 1) / c->c_m;
-                PN_CUDA(c, cudaFuncSetAttribute(pair_cross_sym_kernel<kCrossSymMinB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCrossSymSmemBytes<true>));
-                PN_CUDA(c, cudaFuncSetAttribute(pair_cross_sym_kernel<kCrossSymMinB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCrossSymSmemBytes<false>));
+                PN_CUDA(c, cudaFuncSetAttribute(pair_cross_sym_kernel<kCrossSymMinB, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCrossSymSmemBytes<true>));
+                PN_CUDA(c, cudaFuncSetAttribute(pair_cross_sym_kernel<kCrossSymMinB, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCrossSymSmemBytes<true>));
+                PN_CUDA(c, cudaFuncSetAttribute(pair_cross_sym_kernel<kCrossSymMinB, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCrossSymSmemBytes<false>));
+                PN_CUDA(c, cudaFuncSetAttribute(pair_cross_sym_kernel<kCrossSymMinB, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kCrossSymSmemBytes<false>));
                 PN_CUDA(c, dalloc(&c->crec, np));
                 PN_CUDA(c, dalloc(&c->cblk, (np / kNT) * kCrossSums));
                 PN_CUDA(c, dalloc(&c->csum, kCrossSums));
@@ -1073,7 +1080,8 @@ int pn_get_pair_config(pn_ctx* c, int32_t* cfg)
     if (c->cross && cross_sym(c)) {
         cfg[0] = 32, cfg[1] = kCrossSymI, cfg[2] = kCrossSymU, cfg[3] = c->c_G;
         cfg[4] = c->c_G * (c->c_G + 1) / 2, cfg[5] = c->np;
-        cfg[6] = (c->cross & PN_CROSS_BH) ? 42 : 38, cfg[7] = (c->cross & PN_CROSS_BH) ? 9 : 8;
+        const bool bhx = (c->cross & PN_CROSS_BH) != 0, ceqm = c->equal_mass && c->eqm_opt;
+        cfg[6] = bhx ? (ceqm ? 40 : 42) : (ceqm ? 37 : 38), cfg[7] = (bhx ? 9 : 8) + (ceqm ? 2 : 0);  // 10 / 11: equal-mass form
         return PN_OK;
     }
     if (c->cross) {

@@ -41,11 +41,20 @@ def test_cross_accel_parity_sizes(n_stars, terms):
         p = inputs.plummer_bh(n_stars, seed=700 + n_stars, c=20.0)  # a small c makes the 1PN terms 25 x larger than at c = 100
     ref = Oracle(p.mass, p.G, p.c, p.softening, terms=terms).accel(p.pos, p.vel)
     hot = Oracle(p.mass, p.G, p.c, p.softening).accel(p.pos, p.vel)
+    from paper_1801_07986_b200 import binding
+
     with _pn_cross(p, terms) as pn:
         sym = n_stars >= 6144
-        assert pn.pn_get_pair_config()["variant"] == ((9 if sym else 6) if terms & CROSS_BH else (8 if sym else 5))
+        # symmetric kernel: 10 / 11 in its equal-mass form (these Plummer sets), 8 / 9 in the general form; ordered pairs: 5 / 6
+        assert pn.pn_get_pair_config()["variant"] == ((11 if sym else 6) if terms & CROSS_BH else (10 if sym else 5))
         acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
         again = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
+        if sym:  # the same set through the general-mass form
+            pn.pn_set_option(binding.PN_OPT_EQUAL_MASS, 0)
+            assert pn.pn_get_pair_config()["variant"] == (9 if terms & CROSS_BH else 8)
+            general = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
+            assert rel_err_rows(general, ref).max() <= TOL_ACC
+            assert rel_err_rows(general, acc).max() <= 1e-13
     assert rel_err_rows(acc, ref).max() <= TOL_ACC
     assert np.array_equal(acc, again)  # fixed-order sums
     if n_stars >= 2:  # the Cross term is really there (with one star only the O(m_i) self line is left)
