@@ -296,7 +296,8 @@ cudaError_t prepare_small(pn_ctx* c)
     c->small_IW = std::min(kSmallMaxIW, std::max(1, (c->n_stars + warps - 1) / warps));
     c->small_blocks = (c->n_stars + 4 * c->small_IW - 1) / (4 * c->small_IW);
     if (c->small_blocks > c->n_sm) return cudaSuccess;  // one block per SM: every block must be resident
-    const int smem = c->np * (int)sizeof(JRec);
+    // the attribute belongs to the kernel, not to the context: always the largest size any context may ask of it
+    const int smem = ((kSmallMaxStars + 255) / 256 * 256) * (int)sizeof(JRec);
     for (int mode = 0; mode < 2; ++mode)
         for (int mask = 0; mask < 2; ++mask) {
             const void* fn = mode ? small_kernel<MODE_RK4>(c->small_IW, mask != 0) : small_kernel<MODE_ACCEL>(c->small_IW, mask != 0);

@@ -124,3 +124,17 @@ def test_two_small_contexts_on_two_streams():
             pn.pn_destroy()
     for (x, v), (xr, vr) in zip(got, ref):
         assert np.array_equal(x, xr) and np.array_equal(v, vr)
+
+
+def test_small_contexts_of_different_sizes_share_a_kernel():
+    """Two contexts whose sizes map to the same kernel instance (IW = 2) but need different amounts of shared memory: the
+    second pn_create must not lower the first one's limit."""
+    from paper_1801_07986_b200 import PN
+
+    big, small = inputs.plummer_bh(1180, seed=51, dt=1e-3), inputs.plummer_bh(600, seed=52, dt=1e-3)
+    with PN(big.mass, big.G, big.c, big.softening) as a, PN(small.mass, small.G, small.c, small.softening) as b:
+        assert a.pn_get_pair_config()["i_per_thread"] == b.pn_get_pair_config()["i_per_thread"] == 2
+        for pn, p in ((a, big), (b, small), (a, big)):
+            acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
+            ref = Oracle(p.mass, p.G, p.c, p.softening).accel(p.pos, p.vel)
+            assert rel_err_rows(acc, ref).max() <= TOL_ACC
