@@ -2,11 +2,15 @@
 // Product code: shares nothing with oracle/.  Citations: /root/reference/PAPER.md:<line>.
 //
 // Kernels, in the order of this file (DESIGN.md section 6 has the roofline of each):
-//   S1  pair_fp64_kernel          star-star Newtonian, every ordered pair, tiled (N_s < 3072, PN_PAIR_TILED)
-//       pair_sym_fp64_kernel      the same, every unordered pair once (Newton's third law), general / equal-mass form
-//       pair_cross_fp64_kernel    NEXT-1/2: S1 + the O(N^2) sums of the Cross terms, Eqs. 2.6 and 2.3 (cross_prep/sum: O(N))
-//       pair_fp32_kernel, pair_sym_fp32_kernel   fp32-pair / fp64-accumulate variant (split_kernel: two-float records)
+//   S1  pair_fp64_kernel          star-star Newtonian, every ordered pair, tiled (PN_PAIR_TILED)
+//       pair_sym_fp64_kernel      the same, every unordered pair once (Newton's third law), general / equal-mass form; the
+//                                 j-side sums travel through the lanes of a warp in Gray-code order (N_s >= 3072)
+//       pair_cross_fp64_kernel, pair_cross_sym_kernel   NEXT-1/2: S1 + the O(N^2) sums of the Cross terms, Eqs. 2.6 and 2.3, on
+//                                 ordered / unordered pairs (cross_prep/sum: O(N))
+//       pair_fp32_kernel, pair_sym_fp32_kernel   fp32-pair / fp64-accumulate variant (packed f32x2 arithmetic; split kernels:
+//                                 two-float records)
 //   S2-S4  epilogue_kernel        partial-sum reduction, BH <-> star Newtonian + 1PN, a_1 reduction, fused RK4 stage update
+//   S1-S4  small_path_kernel      N_s < 3072: a whole pn_step call (or one pn_accel) in ONE cooperative launch
 //   S5  energy_prep / energy_pair / energy_final   Eq. 2.7, compensated
 //   NEXT-3  momentum_prep / momentum_pair / momentum_final   Eq. 2.8, compensated
 //   pack / unpack (AoS <-> internal layout)
@@ -17,7 +21,7 @@
 //   double v[3][NP]     : stage velocity, SoA
 //   double x0/v0[3][NP] : state at the beginning of the RK4 step;  double sx/sv[3][NP] : weighted sum of k's
 //   double part[S][3][NP]: partial star-star accelerations, one slot per j-chunk (tiled) or j-group (symmetric), each entry
-//                         written by exactly one block; summed in fixed order by the epilogue (6 or 7 components per slot
+//                         written by exactly one block; summed in fixed order by the epilogue (7 or 8 components per slot
 //                         in Cross mode)
 //   BhState             : the massive object's stage state, step state, k-sums (a handful of doubles)
 #pragma once
