@@ -88,7 +88,7 @@ extern "C" {
 
 /* PN_OPT_PAIR_KERNEL values (either pair precision) */
 #define PN_PAIR_AUTO 0      /* symmetric for N - 1 >= 3072 stars (unit tiles of 128 stars, 512 from 36000 stars on).  Below
-                               (fp64, no Cross terms): the small-system path -- ONE cooperative kernel launch runs a whole
+                               (fp64; with the Cross terms: up to 1279 stars): the small-system path -- ONE cooperative kernel launch runs a whole
                                pn_step call (every stage of every step) or one pn_accel, every ordered pair, 15 instructions;
                                it needs a device with cooperative launch and as many SMs as blocks (else: tiled) */
 #define PN_PAIR_TILED 1     /* every ordered pair (i, j): 15 FP64 (18 FP32) instructions per ordered pair */

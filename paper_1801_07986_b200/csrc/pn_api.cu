@@ -63,6 +63,7 @@ struct pn_ctx {
     double* small_part = nullptr;      // [2][4 small_blocks][3] per-warp partials of a_1
     unsigned int* small_bar = nullptr; // [2]: arrival counter of the grid barrier, give-up flag (small_check)
     bool small_used = false;           // a small-path launch since the last check
+    XVRec* small_xv = nullptr;         // [2][np] exchanged stage state of the small-system path with the Cross terms
     unsigned int small_bar_base = 0;   // its value when the next launch starts
 
     // device buffers.  Two stage sets: [0] integrator state, [1] scratch for pn_accel.
@@ -192,6 +193,12 @@ bool use_small(const pn_ctx* c)
     return c->small_ok && c->kernel_opt == PN_PAIR_AUTO && c->precision == PN_FP64 && !c->cross;
 }
 
+// ... and with the Cross terms up to kSmallCrossMaxStars stars (the per-star Cross records of every star must fit in shared memory)
+bool use_small_cross(const pn_ctx* c)
+{
+    return c->small_ok && c->small_xv && c->kernel_opt == PN_PAIR_AUTO && c->cross && c->n_stars <= kSmallCrossMaxStars;
+}
+
 bool use_eqm(const pn_ctx* c) { return c->equal_mass && c->eqm_opt && use_sym(c) && !use_small(c); }
 
 // kernels of the pair stage of one force evaluation (the epilogue is counted by the callers)
@@ -237,6 +244,8 @@ const void* small_kernel(int iw, bool mask)
     }
 }
 
+int small_launch_common(pn_ctx* c, const void* fn, void** args, size_t smem, int64_t n_eval);
+
 // one cooperative launch: mode MODE_RK4 runs nsteps classical RK4 steps on the integrator state (stage set 0, with stage
 // set 1 as the second position buffer), MODE_ACCEL one force evaluation on stage set 1
 int launch_small(pn_ctx* c, int mode, double dt, int64_t nsteps, double* acc_out)
@@ -256,8 +265,14 @@ int launch_small(pn_ctx* c, int mode, double dt, int64_t nsteps, double* acc_out
     a.bar_base = c->small_bar_base;
     const bool mask = (c->eps2 == 0.0);
     const void* fn = (mode == MODE_RK4) ? small_kernel<MODE_RK4>(c->small_IW, mask) : small_kernel<MODE_ACCEL>(c->small_IW, mask);
-    const size_t smem = (size_t)c->np * sizeof(JRec);
     void* args[] = {&a};
+    const size_t smem = (size_t)c->np * sizeof(JRec);
+    return small_launch_common(c, fn, args, smem, (mode == MODE_RK4) ? 4 * nsteps : 1);
+}
+
+// one cooperative launch of a small-system kernel; on success the host's copy of the barrier counter moves on
+int small_launch_common(pn_ctx* c, const void* fn, void** args, size_t smem, int64_t n_eval)
+{
     // blocks of two grids that both spin at their own barrier must never share the device half and half: cooperative launches
     // of this process run one after the other (each waits for the event the previous one recorded, on whatever stream)
     static std::mutex g_small_mu;
@@ -279,9 +294,46 @@ int launch_small(pn_ctx* c, int mode, double dt, int64_t nsteps, double* acc_out
     PN_CUDA(c, e);
     PN_CUDA(c, cudaEventRecord(chain, c->stream));
     c->small_used = true;
-    const int64_t n_eval = (mode == MODE_RK4) ? 4 * nsteps : 1;
     c->small_bar_base += (unsigned int)((uint64_t)n_eval * (uint64_t)c->small_blocks);  // modulo 2^32, like the counter
     return PN_OK;
+}
+
+template <int MODE, bool BHX>
+const void* small_cross_kernel_ptr(int iw)
+{
+    switch (iw) {
+        case 1: return reinterpret_cast<const void*>(small_cross_kernel<MODE, 1, BHX>);
+        case 2: return reinterpret_cast<const void*>(small_cross_kernel<MODE, 2, BHX>);
+        default: return reinterpret_cast<const void*>(small_cross_kernel<MODE, 3, BHX>);
+    }
+}
+
+const void* small_cross_fn(int mode, int iw, bool bhx)
+{
+    if (mode == MODE_RK4) return bhx ? small_cross_kernel_ptr<MODE_RK4, true>(iw) : small_cross_kernel_ptr<MODE_RK4, false>(iw);
+    return bhx ? small_cross_kernel_ptr<MODE_ACCEL, true>(iw) : small_cross_kernel_ptr<MODE_ACCEL, false>(iw);
+}
+
+// the same with the Cross terms (PN_OPT_CROSS_TERMS): small_cross_kernel
+int launch_small_cross(pn_ctx* c, int mode, double dt, int64_t nsteps, double* acc_out)
+{
+    SmallCrossArgs a;
+    const int set = (mode == MODE_RK4) ? 0 : 1;
+    a.jrec_in = c->jrec[set], a.jrec_out = c->jrec[0];
+    a.v = c->v[set];
+    a.x0 = c->x0, a.v0 = c->v0, a.sx = c->sx, a.sv = c->sv;
+    a.bh = c->bh[set];
+    a.xv = c->small_xv;
+    a.bh_part = c->small_part;
+    a.bar = c->small_bar;
+    a.acc_out = acc_out;
+    a.n_stars = c->n_stars, a.np = c->np;
+    a.GM = c->GM, a.inv_c2 = c->inv_c2, a.eps2 = c->eps2, a.dt = dt;
+    a.nsteps = nsteps;
+    a.bar_base = c->small_bar_base;
+    void* args[] = {&a};
+    return small_launch_common(c, small_cross_fn(mode, c->small_IW, (c->cross & PN_CROSS_BH) != 0), args,
+                               (size_t)c->np * kSmallCrossBytesPerStar, (mode == MODE_RK4) ? 4 * nsteps : 1);
 }
 
 // sizes the small-system path and checks that the device can run it (cooperative launch, shared memory, residency)
@@ -762,7 +814,7 @@ int pn_destroy(pn_ctx* c)
     cudaFree(c->part), cudaFree(c->bh_part), cudaFree(c->ticket), cudaFree(c->prm);
     cudaFree(c->io_pos), cudaFree(c->io_vel), cudaFree(c->io_acc);
     cudaFree(c->crec), cudaFree(c->cblk), cudaFree(c->csum), cudaFree(c->part6), cudaFree(c->blk_mom);
-    cudaFree(c->small_part), cudaFree(c->small_bar);
+    cudaFree(c->small_part), cudaFree(c->small_bar), cudaFree(c->small_xv);
     cudaFree(c->frec), cudaFree(c->fpair), cudaFree(c->erec), cudaFree(c->blk_prep), cudaFree(c->blk_pair), cudaFree(c->d_energy);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     cudaGetLastError();
@@ -830,6 +882,23 @@ int pn_set_option(pn_ctx* c, int key, int value)
                 PN_CUDA(c, dalloc(&c->cblk, (np / kNT) * kCrossSums));
                 PN_CUDA(c, dalloc(&c->csum, kCrossSums));
                 PN_CUDA(c, dalloc(&c->part6, (size_t)std::max(c->c_split, c->c_G) * 8 * np));
+            }
+            if (value && c->small_ok && c->n_stars <= kSmallCrossMaxStars && !c->small_xv) {  // small-system path with the Cross terms
+                const size_t np = c->np;
+                for (int mode = 0; mode < 2; ++mode)
+                    for (int bhx = 0; bhx < 2; ++bhx)
+                        PN_CUDA(c, cudaFuncSetAttribute(small_cross_fn(mode, c->small_IW, bhx != 0), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                        ((kSmallCrossMaxStars + 255) / 256 * 256) * kSmallCrossBytesPerStar));
+                std::vector<XVRec> h(2 * np);  // pad entries are never written by the kernel: far away, at rest, for good
+                for (XVRec& r : h) r.x = r.y = r.z = kPadPos, r.vx = r.vy = r.vz = 0.0;
+                XVRec* xv = nullptr;
+                PN_CUDA(c, dalloc(&xv, 2 * np));
+                cudaError_t e = cudaMemcpy(xv, h.data(), h.size() * sizeof(XVRec), cudaMemcpyHostToDevice);
+                if (e != cudaSuccess) {
+                    cudaFree(xv);
+                    PN_CUDA(c, e);
+                }
+                c->small_xv = xv;
             }
             c->cross = value;
             destroy_graphs(c);
@@ -905,8 +974,8 @@ int pn_accel(pn_ctx* c, const double* pos, const double* vel, double* acc)
     const int grid_pack = (c->n_stars + 255) / 256;
     pack_kernel<<<grid_pack, 256, 0, c->stream>>>(pos, vel, c->jrec[1], c->v[1], nullptr, nullptr, c->bh[1], c->n_stars, c->np, 0);
     PN_CUDA(c, cudaGetLastError());
-    if (use_small(c)) {
-        const int rc = launch_small(c, MODE_ACCEL, 0.0, 0, acc);
+    if (use_small(c) || use_small_cross(c)) {
+        const int rc = c->cross ? launch_small_cross(c, MODE_ACCEL, 0.0, 0, acc) : launch_small(c, MODE_ACCEL, 0.0, 0, acc);
         if (rc == PN_OK) {
             c->n_launch += 2;
             return PN_OK;
@@ -947,8 +1016,8 @@ int pn_step(pn_ctx* c, double dt, int64_t nsteps)
     if (nsteps < 0) return fail(c, PN_EINVAL, "pn_step: nsteps must be >= 0");
     if (!c->have_state) return fail(c, PN_ESTATE, "pn_step: no state set (call pn_set_state first)");
     if (nsteps == 0) return PN_OK;
-    if (use_small(c)) {  // every stage of every step in one cooperative launch (PN_OPT_USE_GRAPH / PN_OPT_TIME_PAIR do not apply)
-        const int rc = launch_small(c, MODE_RK4, dt, nsteps, nullptr);
+    if (use_small(c) || use_small_cross(c)) {  // every stage of every step in one cooperative launch (PN_OPT_USE_GRAPH / PN_OPT_TIME_PAIR do not apply)
+        const int rc = c->cross ? launch_small_cross(c, MODE_RK4, dt, nsteps, nullptr) : launch_small(c, MODE_RK4, dt, nsteps, nullptr);
         if (rc == PN_OK) {
             c->n_launch += 1;
             return PN_OK;
@@ -1076,6 +1145,12 @@ int pn_get_pair_config(pn_ctx* c, int32_t* cfg)
     if (!cfg) return fail(c, PN_EINVAL, "pn_get_pair_config: null pointer");
     if (use_small(c)) {
         cfg[0] = kSmallNT, cfg[1] = c->small_IW, cfg[2] = 32, cfg[3] = 1, cfg[4] = c->small_blocks, cfg[5] = c->np, cfg[6] = 15, cfg[7] = 7;
+        return PN_OK;
+    }
+    if (use_small_cross(c)) {  // 12 / 13: the small-system path with the Cross terms (ordered pairs: 54 / 59 instructions)
+        const bool bhx = (c->cross & PN_CROSS_BH) != 0;
+        cfg[0] = kSmallNT, cfg[1] = c->small_IW, cfg[2] = 32, cfg[3] = 1, cfg[4] = c->small_blocks, cfg[5] = c->np;
+        cfg[6] = bhx ? 59 : 54, cfg[7] = bhx ? 13 : 12;
         return PN_OK;
     }
     if (c->cross && cross_sym(c)) {

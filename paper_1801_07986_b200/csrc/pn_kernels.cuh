@@ -1356,6 +1356,64 @@ __device__ __forceinline__ void block_sum3(double& a, double& b, double& c, doub
 //       k_x = v_stage, k_v = a;  st 0: s = k;  st 1, 2: s += 2k;  next stage state = y0 + {dt/2, dt/2, dt} k;
 //       st 3: y0 += dt/6 (s + k), next stage state = y0.
 // ---------------------------------------------------------------------------------------------------------
+// S2 + S3 (+ the O(N) parts of the Cross terms) for one star: x = x_i1 = x_i - x_1, vel = v_i, gm = G m_i, ss = the star's O(N^2)
+// sums (a^SS; CROSS: + X (3), S, and U for CROSS = 2), csum = P (3), Q1, Q3, W (3).  Returns a_i in a and the star's share of
+// a_1 in b.  Used by epilogue_kernel and by the small-system kernels.
+template <int CROSS>
+__device__ __forceinline__ void star_physics(double gm, const double (&x)[3], const double (&vel)[3], const double* ss,
+                                             const double* __restrict__ csum, double GM, double inv_c2, double (&a)[3], double (&b)[3])
+{
+    const double r2 = x[0] * x[0] + x[1] * x[1] + x[2] * x[2];
+    const double r = sqrt(r2);
+    const double inv_r = 1.0 / r;
+    const double inv_r3 = inv_r * inv_r * inv_r;
+    const double v2 = vel[0] * vel[0] + vel[1] * vel[1] + vel[2] * vel[2];
+    const double vx = vel[0] * x[0] + vel[1] * x[1] + vel[2] * x[2];
+    const double GMr = GM * inv_r;
+    // star <- BH: -GM x/r^3 + (1/c^2)(GM/r^3)[(4GM/r - v^2) x + 4 (v.x) v]
+    const double cs = GM * inv_r3;
+    const double fx = -1.0 + inv_c2 * (4.0 * GMr - v2);
+    const double fv = inv_c2 * 4.0 * vx;
+    // BH <- star (x_1j = -x): (G m/r^3){ x - (1/c^2)[(5GM/r - 2v^2 + 3/2 (v.x)^2/r^2) x + 3 (v.x) v] }
+    const double cb = gm * inv_r3;
+    const double gx = 1.0 - inv_c2 * (5.0 * GMr - 2.0 * v2 + 1.5 * vx * vx * inv_r * inv_r);
+    const double gv = -inv_c2 * 3.0 * vx;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) a[k] = ss[k] + cs * (fx * x[k] + fv * vel[k]);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) b[k] = cb * (gx * x[k] + gv * vel[k]);
+    if (CROSS) {
+        // [a_i]_Cross = L0 + the O(N) parts of L1, L3, L4 (global sums minus this star's own term) + pair part
+        const double P[3] = {csum[0] - gm * vel[0], csum[1] - gm * vel[1], csum[2] - gm * vel[2]};
+        const double Q1 = csum[3] - gm * inv_r, Q3 = csum[4] - gm * inv_r3;
+        const double W[3] = {csum[5] - gm * x[0] * inv_r3, csum[6] - gm * x[1] * inv_r3, csum[7] - gm * x[2] * inv_r3};
+        const double vP = vel[0] * P[0] + vel[1] * P[1] + vel[2] * P[2];
+        const double xP = x[0] * P[0] + x[1] * P[1] + x[2] * P[2];
+        // coefficient of x_i1: L0 (5 G m_i GM / r^4 - 4 G m_i v^2 / r^3) + L1 (GM/r^3)(5/4 Q1 + r^2/4 Q3) - L4 4 (v.P)/r^3
+        // + the pair part of L1, S / r^3 (S = sum_j G m_j (4 GM / rho_ij - GM rho_ij^2 / (4 r_j1^3)), 7th component)
+        const double kx = inv_r3 * (5.0 * gm * GMr - 4.0 * gm * v2 + GM * (1.25 * Q1 + 0.25 * r2 * Q3) - 4.0 * vP + ss[6]);
+        // coefficient of v_i: L0 7 G m_i (v.x)/r^3 + L4 3 (P.x)/r^3
+        const double kv = inv_r3 * (7.0 * gm * vx + 3.0 * xP);
+        const double kp = 4.0 * vx * inv_r3;  // L4: + 4 (v_i.x_i1) P / r^3
+        const double kw = 3.5 * GM * inv_r;   // L3: + (7/2) GM W / r_i1
+#pragma unroll
+        for (int k = 0; k < 3; ++k) a[k] += inv_c2 * (ss[3 + k] + kx * x[k] + kv * vel[k] + kp * P[k] + kw * W[k]);
+        if (CROSS == 2) {
+            // this star's share of [a_1]_Cross (x_1j = -x): T0 + T1 along x, T2 along a_j^SS, T3 with the FULL sum P
+            const double Pf[3] = {csum[0], csum[1], csum[2]};
+            const double vPf = vel[0] * Pf[0] + vel[1] * Pf[1] + vel[2] * Pf[2];
+            const double xPf = x[0] * Pf[0] + x[1] * Pf[1] + x[2] * Pf[2];
+            const double gr3 = gm * inv_r3, g_M = gr3 / GM;
+            const double tx = -(4.0 * gm * gr3 * inv_r + gr3 * (4.0 * Q1 + ss[CROSS == 2 ? 7 : 0])) + 4.0 * g_M * vPf;  // times x
+            const double tP = -3.0 * g_M * vx;       // times P
+            const double tv = -4.0 * g_M * xPf;      // times v_j
+            const double ta = 3.5 * gm * inv_r;      // times a_j^SS
+#pragma unroll
+            for (int k = 0; k < 3; ++k) b[k] += inv_c2 * (tx * x[k] + tP * Pf[k] + tv * vel[k] + ta * ss[k]);
+        }
+    }
+}
+
 struct EpiArgs {
     JRec* jrec;           // stage positions (x, y, z updated in RK4 mode)
     double* v;            // [3][NP] stage velocity
@@ -1434,58 +1492,9 @@ __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
         const JRec rec = A.jrec[i];
         const double x[3] = {rec.x - A.bh->xs[0], rec.y - A.bh->xs[1], rec.z - A.bh->xs[2]};  // x_i1 = x_i - x_1
         vel[0] = A.v[i], vel[1] = A.v[np + i], vel[2] = A.v[2 * np + i];
-        const double r2 = x[0] * x[0] + x[1] * x[1] + x[2] * x[2];
-        const double r = sqrt(r2);
-        const double inv_r = 1.0 / r;
-        const double inv_r3 = inv_r * inv_r * inv_r;
-        const double v2 = vel[0] * vel[0] + vel[1] * vel[1] + vel[2] * vel[2];
-        const double vx = vel[0] * x[0] + vel[1] * x[1] + vel[2] * x[2];
-        const double GMr = A.GM * inv_r;
-        // star <- BH: -GM x/r^3 + (1/c^2)(GM/r^3)[(4GM/r - v^2) x + 4 (v.x) v]
-        const double cs = A.GM * inv_r3;
-        const double fx = -1.0 + A.inv_c2 * (4.0 * GMr - v2);
-        const double fv = A.inv_c2 * 4.0 * vx;
-        // BH <- star (x_1j = -x): (G m/r^3){ x - (1/c^2)[(5GM/r - 2v^2 + 3/2 (v.x)^2/r^2) x + 3 (v.x) v] }
-        const double cb = rec.gm * inv_r3;
-        const double gx = 1.0 - A.inv_c2 * (5.0 * GMr - 2.0 * v2 + 1.5 * vx * vx * inv_r * inv_r);
-        const double gv = -A.inv_c2 * 3.0 * vx;
-#pragma unroll
-        for (int k = 0; k < 3; ++k) a[k] = ss[k] + cs * (fx * x[k] + fv * vel[k]);
-        b0 = cb * (gx * x[0] + gv * vel[0]);
-        b1 = cb * (gx * x[1] + gv * vel[1]);
-        b2 = cb * (gx * x[2] + gv * vel[2]);
-        if (CROSS) {
-            // [a_i]_Cross = L0 + the O(N) parts of L1, L3, L4 (global sums minus this star's own term) + pair part
-            const double P[3] = {A.csum[0] - rec.gm * vel[0], A.csum[1] - rec.gm * vel[1], A.csum[2] - rec.gm * vel[2]};
-            const double Q1 = A.csum[3] - rec.gm * inv_r, Q3 = A.csum[4] - rec.gm * inv_r3;
-            const double W[3] = {A.csum[5] - rec.gm * x[0] * inv_r3, A.csum[6] - rec.gm * x[1] * inv_r3,
-                                 A.csum[7] - rec.gm * x[2] * inv_r3};
-            const double vP = vel[0] * P[0] + vel[1] * P[1] + vel[2] * P[2];
-            const double xP = x[0] * P[0] + x[1] * P[1] + x[2] * P[2];
-            // coefficient of x_i1: L0 (5 G m_i GM / r^4 - 4 G m_i v^2 / r^3) + L1 (GM/r^3)(5/4 Q1 + r^2/4 Q3) - L4 4 (v.P)/r^3
-            // + the pair part of L1, S / r^3 (S = sum_j G m_j (4 GM / rho_ij - GM rho_ij^2 / (4 r_j1^3)), 7th component)
-            const double kx = inv_r3 * (5.0 * rec.gm * GMr - 4.0 * rec.gm * v2 + A.GM * (1.25 * Q1 + 0.25 * r2 * Q3) - 4.0 * vP + ss[6]);
-            // coefficient of v_i: L0 7 G m_i (v.x)/r^3 + L4 3 (P.x)/r^3
-            const double kv = inv_r3 * (7.0 * rec.gm * vx + 3.0 * xP);
-            const double kp = 4.0 * vx * inv_r3;       // L4: + 4 (v_i.x_i1) P / r^3
-            const double kw = 3.5 * A.GM * inv_r;      // L3: + (7/2) GM W / r_i1
-#pragma unroll
-            for (int k = 0; k < 3; ++k) a[k] += A.inv_c2 * (ss[3 + k] + kx * x[k] + kv * vel[k] + kp * P[k] + kw * W[k]);
-            if (CROSS == 2) {
-                // this star's share of [a_1]_Cross (x_1j = -x): T0 + T1 along x, T2 along a_j^SS, T3 with the FULL sum P
-                const double Pf[3] = {A.csum[0], A.csum[1], A.csum[2]};
-                const double vPf = vel[0] * Pf[0] + vel[1] * Pf[1] + vel[2] * Pf[2];
-                const double xPf = x[0] * Pf[0] + x[1] * Pf[1] + x[2] * Pf[2];
-                const double gr3 = rec.gm * inv_r3, g_M = gr3 / A.GM;
-                const double tx = -(4.0 * rec.gm * gr3 * inv_r + gr3 * (4.0 * Q1 + ss[CROSS == 2 ? 7 : 0])) + 4.0 * g_M * vPf;  // times x
-                const double tP = -3.0 * g_M * vx;                                                             // times P
-                const double tv = -4.0 * g_M * xPf;                                                            // times v_j
-                const double ta = 3.5 * rec.gm * inv_r;                                                        // times a_j^SS
-                b0 += A.inv_c2 * (tx * x[0] + tP * Pf[0] + tv * vel[0] + ta * ss[0]);
-                b1 += A.inv_c2 * (tx * x[1] + tP * Pf[1] + tv * vel[1] + ta * ss[1]);
-                b2 += A.inv_c2 * (tx * x[2] + tP * Pf[2] + tv * vel[2] + ta * ss[2]);
-            }
-        }
+        double bb[3];
+        star_physics<CROSS>(rec.gm, x, vel, ss, A.csum, A.GM, A.inv_c2, a, bb);
+        b0 = bb[0], b1 = bb[1], b2 = bb[2];
     }
 
     double hh = 0, dt = 0;
@@ -1754,26 +1763,10 @@ __global__ void __launch_bounds__(kSmallNT, 1) small_path_kernel(SmallArgs A)
         if (own) {
             const JRec rec = sj[my];
             const double x[3] = {rec.x - sbh.xs[0], rec.y - sbh.xs[1], rec.z - sbh.xs[2]};  // x_i1 = x_i - x_1
-            const double r2 = x[0] * x[0] + x[1] * x[1] + x[2] * x[2];
-            const double r = sqrt(r2);
-            const double inv_r = 1.0 / r;
-            const double inv_r3 = inv_r * inv_r * inv_r;
-            const double v2 = vs[0] * vs[0] + vs[1] * vs[1] + vs[2] * vs[2];
-            const double vx = vs[0] * x[0] + vs[1] * x[1] + vs[2] * x[2];
-            const double GMr = A.GM * inv_r;
-            const double cs = A.GM * inv_r3;
-            const double fx = -1.0 + A.inv_c2 * (4.0 * GMr - v2);
-            const double fv = A.inv_c2 * 4.0 * vx;
-            const double cb = gm_me * inv_r3;
-            const double gx = 1.0 - A.inv_c2 * (5.0 * GMr - 2.0 * v2 + 1.5 * vx * vx * inv_r * inv_r);
-            const double gv = -A.inv_c2 * 3.0 * vx;
             const double ss[3] = {s0, s1, s2};
-            double a[3];
-#pragma unroll
-            for (int k = 0; k < 3; ++k) a[k] = ss[k] + cs * (fx * x[k] + fv * vs[k]);
-            b0 = cb * (gx * x[0] + gv * vs[0]);
-            b1 = cb * (gx * x[1] + gv * vs[1]);
-            b2 = cb * (gx * x[2] + gv * vs[2]);
+            double a[3], bb[3];
+            star_physics<0>(gm_me, x, vs, ss, nullptr, A.GM, A.inv_c2, a, bb);
+            b0 = bb[0], b1 = bb[1], b2 = bb[2];
             if (MODE == MODE_ACCEL) {
                 double* o = A.acc_out + 3 * (size_t)(my + 1);
                 o[0] = a[0], o[1] = a[1], o[2] = a[2];
@@ -1828,6 +1821,270 @@ __global__ void __launch_bounds__(kSmallNT, 1) small_path_kernel(SmallArgs A)
             for (int k = 0; k < 3; ++k) {
                 const size_t q = (size_t)k * np + my;
                 A.v[q] = vs[k], A.x0[q] = x0[k], A.v0[q] = v0[k], A.sx[q] = sx[k], A.sv[q] = sv[k];
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// The small-system path with the Cross terms (Eqs. 2.6 and 2.3; N_s <= kSmallCrossMaxStars): the same one-launch scheme as
+// small_path_kernel.  What the blocks exchange per evaluation is the stage position AND velocity of every star (48 B, two
+// buffers by evaluation parity); from them every block builds, for itself and in the same order, the per-star records of the
+// Cross kernels (CRec) and the eight global sums P, Q1, Q3, W in shared memory -- redundant O(N) work instead of a second grid
+// barrier.  Every ordered pair (cross_pair, j != i by index), lanes share out the j-stars, 7 or 8 sums per i-star.
+// ---------------------------------------------------------------------------------------------------------
+struct __align__(16) XVRec {
+    double x, y, z, vx, vy, vz;  // stage position and velocity of a star
+};
+static_assert(sizeof(XVRec) == 48, "XVRec must be 48 bytes");
+
+struct SmallCrossArgs {
+    const JRec* jrec_in;  // positions of the state the launch starts from (and G m of every star)
+    JRec* jrec_out;       // MODE_RK4: the integrator's stage records, positions written back at the end
+    double* v;            // [3][np] stage velocity (read at the start, MODE_RK4: written at the end)
+    double *x0, *v0, *sx, *sv;
+    BhState* bh;
+    XVRec* xv;            // [2][np]: evaluation e >= 1 reads set e & 1, evaluation e writes set (e + 1) & 1
+    double* bh_part;      // [2][warps of the grid][3]
+    unsigned int* bar;
+    double* acc_out;
+    int n_stars, np;
+    double GM, inv_c2, eps2, dt;
+    long long nsteps;
+    unsigned int bar_base;
+};
+
+constexpr int kSmallCrossMaxStars = 1279;                                   // np <= 1280
+constexpr int kSmallCrossBytesPerStar = (int)(sizeof(XVRec) + sizeof(CRec) + 8);  // staged exchange record + CRec + G m
+
+template <int MODE, int IW, bool BHX>
+__global__ void __launch_bounds__(kSmallNT, 1) small_cross_kernel(SmallCrossArgs A)
+{
+    constexpr int CROSS = BHX ? 2 : 1;
+    constexpr int NW = kSmallNT / 32;
+    extern __shared__ double2 small_smem[];
+    const int np = A.np;
+    XVRec* sxv = reinterpret_cast<XVRec*>(small_smem);                    // [np] this evaluation's stage state of every star
+    CRec* scr = reinterpret_cast<CRec*>(small_smem + 3 * (size_t)np);     // [np] Cross records
+    double* sgm = reinterpret_cast<double*>(small_smem + 10 * (size_t)np); // [np] G m
+    __shared__ double red[kCrossSums][NW];
+    __shared__ double red3[3 * NW];
+    __shared__ double scsum[kCrossSums];
+    __shared__ BhState sbh;
+    __shared__ __align__(8) unsigned long long fill_bar;
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int gw = blockIdx.x * NW + w;
+    const int i0 = gw * IW;
+    const int my = i0 + lane;
+    const bool own = (lane < IW) && (my < A.n_stars);
+    const double GM4 = 4.0 * A.GM;
+    unsigned int target = A.bar_base;
+
+    double x0[3] = {0, 0, 0}, v0[3] = {0, 0, 0}, sx[3] = {0, 0, 0}, sv[3] = {0, 0, 0};
+    if (own && MODE == MODE_RK4) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const size_t q = (size_t)k * np + my;
+            x0[k] = A.x0[q], v0[k] = A.v0[q], sx[k] = A.sx[q], sv[k] = A.sv[q];
+        }
+    }
+    for (int q = tid; q < np; q += kSmallNT) {  // G m of every star; evaluation 0's stage state straight from the caller's arrays
+        const JRec r = A.jrec_in[q];
+        sgm[q] = r.gm;
+        XVRec o;
+        o.x = r.x, o.y = r.y, o.z = r.z;
+        o.vx = A.v[q], o.vy = A.v[np + q], o.vz = A.v[2 * (size_t)np + q];
+        sxv[q] = o;
+    }
+    if (tid == 0) {
+        sbh = *A.bh;
+        mbar_init(&fill_bar, 1);
+    }
+    __syncthreads();
+
+    const int n_part = (int)gridDim.x * NW;
+    auto finish_bh = [&](long long e) {
+        const int stage = (int)(e & 3);
+        const double* part = A.bh_part + (size_t)(e & 1) * 3 * n_part;
+        double c0 = 0, c1 = 0, c2 = 0;
+        for (int q = tid; q < n_part; q += kSmallNT) {
+            c0 += __ldcg(part + 3 * q), c1 += __ldcg(part + 3 * q + 1), c2 += __ldcg(part + 3 * q + 2);
+        }
+        __syncthreads();
+        block_sum3<kSmallNT>(c0, c1, c2, red3);
+        if (tid == 0) {
+            const double a1[3] = {c0, c1, c2};
+            if (MODE == MODE_ACCEL) {
+                if (blockIdx.x == 0) A.acc_out[0] = a1[0], A.acc_out[1] = a1[1], A.acc_out[2] = a1[2];
+            } else {
+                const double dt = A.dt, hh = (stage == 2) ? dt : 0.5 * dt;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const double kx = sbh.vs[k], kv = a1[k];
+                    if (stage == 3) {
+                        sbh.x0[k] += dt / 6.0 * (sbh.sx[k] + kx);
+                        sbh.v0[k] += dt / 6.0 * (sbh.sv[k] + kv);
+                        sbh.xs[k] = sbh.x0[k], sbh.vs[k] = sbh.v0[k];
+                    } else {
+                        if (stage == 0) {
+                            sbh.sx[k] = kx, sbh.sv[k] = kv;
+                        } else {
+                            sbh.sx[k] += 2.0 * kx, sbh.sv[k] += 2.0 * kv;
+                        }
+                        sbh.xs[k] = sbh.x0[k] + hh * kx;
+                        sbh.vs[k] = sbh.v0[k] + hh * kv;
+                    }
+                }
+            }
+        }
+    };
+
+    const long long n_eval = (MODE == MODE_RK4) ? 4 * A.nsteps : 1;
+    double xs_my[3] = {0, 0, 0}, vs_my[3] = {0, 0, 0};  // the own star's stage state after the last update
+    for (long long ev = 0; ev < n_eval; ++ev) {
+        const int stage = (int)(ev & 3);
+        if (ev > 0) {
+            if (tid == 0) bulk_copy_g2s(sxv, A.xv + (size_t)(ev & 1) * np, (unsigned int)(np * sizeof(XVRec)), &fill_bar);
+            finish_bh(ev - 1);
+            mbar_wait(&fill_bar, (unsigned int)((ev - 1) & 1));
+        }
+        __syncthreads();
+
+        // per-star records of the Cross kernels and the eight global sums, every block for itself in the same order
+        {
+            double sums[kCrossSums] = {0, 0, 0, 0, 0, 0, 0, 0};
+            for (int q = tid; q < np; q += kSmallNT) {
+                const XVRec s = sxv[q];
+                const double gm = sgm[q];
+                CRec o;
+                o.x = s.x, o.y = s.y, o.z = s.z, o.gm = gm;
+                o.vx = o.vy = o.vz = o.a5 = o.b = o.wx = o.wy = o.wz = o.rj2 = o.kap = 0.0;
+                if (q < A.n_stars) {
+                    const double d[3] = {s.x - sbh.xs[0], s.y - sbh.xs[1], s.z - sbh.xs[2]};  // x_j1
+                    const double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+                    const double inv_r = 1.0 / sqrt(r2);
+                    const double inv_r3 = inv_r * inv_r * inv_r;
+                    o.vx = s.vx, o.vy = s.vy, o.vz = s.vz;
+                    o.a5 = A.GM * 1.25 * inv_r, o.b = A.GM * 0.25 * inv_r3, o.rj2 = r2;
+                    o.kap = 4.0 * A.GM * inv_r + (s.vx * s.vx + s.vy * s.vy + s.vz * s.vz);
+                    const double wv[3] = {gm * d[0] * inv_r3, gm * d[1] * inv_r3, gm * d[2] * inv_r3};
+                    o.wx = -3.5 * A.GM * wv[0], o.wy = -3.5 * A.GM * wv[1], o.wz = -3.5 * A.GM * wv[2];
+                    sums[0] += gm * s.vx, sums[1] += gm * s.vy, sums[2] += gm * s.vz;
+                    sums[3] += gm * inv_r, sums[4] += gm * inv_r3;
+                    sums[5] += wv[0], sums[6] += wv[1], sums[7] += wv[2];
+                }
+                scr[q] = o;
+            }
+#pragma unroll
+            for (int q = 0; q < kCrossSums; ++q) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) sums[q] += __shfl_down_sync(0xffffffffu, sums[q], o);
+                if (lane == 0) red[q][w] = sums[q];
+            }
+            __syncthreads();
+            if (tid < kCrossSums) {
+                double t = 0;
+                for (int q = 0; q < NW; ++q) t += red[tid][q];
+                scsum[tid] = t;
+            }
+            __syncthreads();
+        }
+
+        // every ordered pair (i, j != i) of this warp's IW i-stars: lane l takes j = l, l + 32, ...
+        double xi[IW][3], vi[IW][3], ri2[IW], kapi[IW];
+        CrossAcc acc[IW];
+#pragma unroll
+        for (int k = 0; k < IW; ++k) {
+            const CRec c = scr[min(i0 + k, np - 1)];
+            xi[k][0] = c.x, xi[k][1] = c.y, xi[k][2] = c.z, vi[k][0] = c.vx, vi[k][1] = c.vy, vi[k][2] = c.vz;
+            ri2[k] = c.rj2, kapi[k] = c.kap;
+            cross_acc_zero(acc[k]);
+        }
+        {
+            CrossAcc dummy;
+            cross_acc_zero(dummy);
+            const double zero3[3] = {0, 0, 0};
+#pragma unroll 2
+            for (int jq = lane; jq < np; jq += 32) {
+                const CRec r = scr[jq];
+#pragma unroll
+                for (int k = 0; k < IW; ++k)
+                    cross_pair<false, BHX, false>(r, xi[k], vi[k], ri2[k], kapi[k], 0.0, 0.0, 0.0, zero3, acc[k], dummy, A.eps2, GM4, jq == i0 + k);
+            }
+        }
+        double ss[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#pragma unroll
+        for (int k = 0; k < IW; ++k) {
+            double t[8] = {acc[k].n[0], acc[k].n[1], acc[k].n[2], acc[k].X[0], acc[k].X[1], acc[k].X[2], acc[k].S, BHX ? acc[k].U : 0.0};
+#pragma unroll
+            for (int c = 0; c < (BHX ? 8 : 7); ++c) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) t[c] += __shfl_xor_sync(0xffffffffu, t[c], o);
+                if (lane == k) ss[c] = t[c];
+            }
+        }
+
+        double b[3] = {0, 0, 0};
+        if (own) {
+            const XVRec me = sxv[my];
+            const double x[3] = {me.x - sbh.xs[0], me.y - sbh.xs[1], me.z - sbh.xs[2]};  // x_i1
+            const double vel[3] = {me.vx, me.vy, me.vz};
+            double a[3];
+            star_physics<CROSS>(sgm[my], x, vel, ss, scsum, A.GM, A.inv_c2, a, b);
+            if (MODE == MODE_ACCEL) {
+                double* o = A.acc_out + 3 * (size_t)(my + 1);
+                o[0] = a[0], o[1] = a[1], o[2] = a[2];
+            } else {
+                const double dt = A.dt, hh = (stage == 2) ? dt : 0.5 * dt;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const double kx = vel[k], kv = a[k];
+                    if (stage == 3) {
+                        x0[k] = x0[k] + dt / 6.0 * (sx[k] + kx);
+                        v0[k] = v0[k] + dt / 6.0 * (sv[k] + kv);
+                        xs_my[k] = x0[k], vs_my[k] = v0[k];
+                    } else {
+                        if (stage == 0) {
+                            sx[k] = kx, sv[k] = kv;
+                        } else {
+                            sx[k] += 2.0 * kx, sv[k] += 2.0 * kv;
+                        }
+                        xs_my[k] = x0[k] + hh * kx;
+                        vs_my[k] = v0[k] + hh * kv;
+                    }
+                }
+                XVRec o;
+                o.x = xs_my[0], o.y = xs_my[1], o.z = xs_my[2], o.vx = vs_my[0], o.vy = vs_my[1], o.vz = vs_my[2];
+                A.xv[(size_t)((ev + 1) & 1) * np + my] = o;  // the next evaluation's stage state, for every block
+            }
+        }
+        {
+            double p0 = 0, p1 = 0, p2 = 0;
+#pragma unroll
+            for (int k = 0; k < IW; ++k) {
+                p0 += __shfl_sync(0xffffffffu, b[0], k);
+                p1 += __shfl_sync(0xffffffffu, b[1], k);
+                p2 += __shfl_sync(0xffffffffu, b[2], k);
+            }
+            if (lane == 0) {
+                double* bp = A.bh_part + (size_t)(ev & 1) * 3 * n_part + 3 * (size_t)gw;
+                bp[0] = p0, bp[1] = p1, bp[2] = p2;
+            }
+        }
+        target += gridDim.x;
+        small_grid_barrier(A.bar, target);
+    }
+    finish_bh(n_eval - 1);
+    __syncthreads();
+    if (MODE == MODE_RK4) {
+        if (blockIdx.x == 0 && tid == 0) *A.bh = sbh;
+        if (own) {
+            JRec* g = A.jrec_out + my;
+            g->x = xs_my[0], g->y = xs_my[1], g->z = xs_my[2];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const size_t q = (size_t)k * np + my;
+                A.v[q] = vs_my[k], A.x0[q] = x0[k], A.v0[q] = v0[k], A.sx[q] = sx[k], A.sv[q] = sv[k];
             }
         }
     }

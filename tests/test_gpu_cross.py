@@ -33,7 +33,7 @@ def _pn_cross(p, terms=CROSS_STAR):
 @pytest.mark.parametrize("terms", TERMS)
 # from 6144 stars on the Cross terms run in the symmetric kernel (every unordered pair once, variant 8 / 9): 64-star unit
 # tiles in up to 128 groups of m tiles (m = 1 up to 8192 stars, 2 up to 16384, 3 at 20000)
-@pytest.mark.parametrize("n_stars", [1, 2, 3, 129, 1023, 4099, 6143, 6144, 8200, 13001, 16383, 20000])
+@pytest.mark.parametrize("n_stars", [1, 2, 3, 129, 592, 593, 1023, 1185, 1279, 1280, 4099, 6143, 6144, 8200, 13001, 16383, 20000])
 def test_cross_accel_parity_sizes(n_stars, terms):
     if n_stars <= 3:
         p = inputs.random_small(n_stars, seed=700 + n_stars, M=1.0, m_scale=1e-2, c=10.0, softening=1e-3, bh_moving=True)
@@ -44,11 +44,19 @@ def test_cross_accel_parity_sizes(n_stars, terms):
     from paper_1801_07986_b200 import binding
 
     with _pn_cross(p, terms) as pn:
-        sym = n_stars >= 6144
-        # symmetric kernel: 10 / 11 in its equal-mass form (these Plummer sets), 8 / 9 in the general form; ordered pairs: 5 / 6
-        assert pn.pn_get_pair_config()["variant"] == ((11 if sym else 6) if terms & CROSS_BH else (10 if sym else 5))
+        sym, small = n_stars >= 6144, n_stars <= 1279
+        # symmetric kernel: 10 / 11 in its equal-mass form (these Plummer sets), 8 / 9 in the general form; ordered pairs: 5 / 6;
+        # up to 1279 stars the small-system path (one cooperative launch per call): 12 / 13
+        bhx = bool(terms & CROSS_BH)
+        assert pn.pn_get_pair_config()["variant"] == ((13 if bhx else 12) if small else ((11 if bhx else 10) if sym else (6 if bhx else 5)))
         acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
         again = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
+        if small:  # the same set through the multi-kernel path (ordered-pair kernel)
+            pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, binding.PN_PAIR_TILED)
+            assert pn.pn_get_pair_config()["variant"] == (6 if bhx else 5)
+            tiled = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
+            assert rel_err_rows(tiled, ref).max() <= TOL_ACC
+            pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, binding.PN_PAIR_AUTO)
         if sym:  # the same set through the general-mass form
             pn.pn_set_option(binding.PN_OPT_EQUAL_MASS, 0)
             assert pn.pn_get_pair_config()["variant"] == (9 if terms & CROSS_BH else 8)
@@ -87,7 +95,7 @@ def test_cross_accel_parity_other_inputs(gen, terms):
         [[0, 1, p.N - 1], np.sort(np.random.default_rng(3).choice(np.arange(2, p.N - 1), 1500, replace=False))])
     ref = Oracle(p.mass, p.G, p.c, p.softening, terms=terms).accel_rows(p.pos, p.vel, rows)
     with _pn_cross(p, terms) as pn:
-        assert (pn.pn_get_pair_config()["variant"] >= 8) == gen.endswith("_sym")
+        assert (pn.pn_get_pair_config()["variant"] in (8, 9, 10, 11)) == gen.endswith("_sym")
         acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
     assert np.isfinite(acc).all()
     assert rel_err_rows(acc[rows], ref).max() <= TOL_ACC
@@ -106,7 +114,7 @@ def test_cross_symmetric_and_ordered_kernels_agree_and_track_the_oracle(terms):
         with PN(p.mass, p.G, p.c, p.softening) as pn:
             pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, kernel)  # before the Cross option: it sizes the Cross buffers
             pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, terms)
-            assert (pn.pn_get_pair_config()["variant"] >= 8) == (kernel == binding.PN_PAIR_AUTO)
+            assert (pn.pn_get_pair_config()["variant"] in (8, 9, 10, 11)) == (kernel == binding.PN_PAIR_AUTO)
             acc[kernel] = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
             pn.pn_set_state_host(p.pos, p.vel)
             pn.pn_step(p.dt, 3)
@@ -133,9 +141,11 @@ def test_cross_switch_off_restores_the_hot_path_bitwise_and_is_deterministic():
     assert np.array_equal(a0, a1) and np.array_equal(c1, c2) and not np.array_equal(a0, c1)
 
 
+@pytest.mark.parametrize("kernel", ["auto", "tiled"])
 @pytest.mark.parametrize("terms", TERMS)
-def test_cross_rk4_trajectory_tracks_oracle(terms):
-    """pn_step with the Cross terms (graph and plain launches) against the oracle's RK4 with the same terms."""
+def test_cross_rk4_trajectory_tracks_oracle(terms, kernel):
+    """pn_step with the Cross terms against the oracle's RK4 with the same terms.  auto: 600 stars take the small-system
+    path (one cooperative launch for the 20 steps); tiled: the multi-kernel path, as a CUDA graph and as plain launches."""
     from paper_1801_07986_b200 import binding
 
     p = inputs.plummer_bh(600, seed=13, c=20.0, dt=1e-3)
@@ -144,6 +154,9 @@ def test_cross_rk4_trajectory_tracks_oracle(terms):
     out = []
     for use_graph in (1, 0):
         with _pn_cross(p, terms) as pn:
+            if kernel == "tiled":
+                pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, binding.PN_PAIR_TILED)
+            assert pn.pn_get_pair_config()["variant"] == ((6 if terms & CROSS_BH else 5) if kernel == "tiled" else (13 if terms & CROSS_BH else 12))
             pn.pn_set_option(binding.PN_OPT_USE_GRAPH, use_graph)
             pn.pn_set_state_host(p.pos, p.vel)
             pn.pn_step(p.dt, 20)
