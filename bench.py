@@ -44,7 +44,9 @@ PAIR_KERNELS = {0: ("pair_fp64_kernel", 15, 24.0), 2: ("pair_sym_fp64_kernel", 1
                 4: ("pair_sym_fp64_kernel<EQM>", 9, 15.0), 5: ("pair_cross_fp64_kernel", 54, 85.0),
                 6: ("pair_cross_fp64_kernel<BHX>", 59, 93.0), 7: ("small_path_kernel", 15, 24.0),
                 8: ("pair_cross_sym_kernel", 38, 62.0), 9: ("pair_cross_sym_kernel<BHX>", 42, 68.0),
-                10: ("pair_cross_sym_kernel<EQM>", 37, 60.0), 11: ("pair_cross_sym_kernel<BHX, EQM>", 40, 65.0)}
+                10: ("pair_cross_sym_kernel<EQM>", 37, 60.0), 11: ("pair_cross_sym_kernel<BHX, EQM>", 40, 65.0),
+                12: ("small_cross_kernel", 54, 85.0), 13: ("small_cross_kernel<BHX>", 59, 93.0)}
+ONE_LAUNCH_PER_STEP = (7, 12, 13)  # small-system path: the launch is the whole RK4 step
 SMS, FP64_LANES_PER_SM = 148, 64
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed `ncu --set full`
 # captures (per launch, cold L2: ncu flushes the caches before every replay), keyed by (variant, N_s); each entry names the
@@ -498,7 +500,7 @@ def run_ours(args) -> None:
         kname, instr, exec_flops = PAIR_KERNELS[cfg["variant"]]
         assert instr == cfg["fp64_instr_per_pair"]
         pairs_per_launch = p.pairs_per_eval
-        if cfg["variant"] == 7:  # one launch = one whole RK4 step (4 force evaluations): its time is the step's
+        if cfg["variant"] in ONE_LAUNCH_PER_STEP:  # one launch = one whole RK4 step (4 force evaluations): its time is the step's
             pair_avg_ms, pair_n, pairs_per_launch = ms_steps / K, K, 4 * p.pairs_per_eval
         kernel_pairs_per_s = pairs_per_launch / (pair_avg_ms * 1e-3) if pair_n else None
         achieved = kernel_pairs_per_s * 2 * instr / 1e12 if pair_n else None
@@ -512,8 +514,8 @@ def run_ours(args) -> None:
                           f"FMA (2 flops) = FP64-pipe issue-slot utilisation; peak = {SMS} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x "
                           f"{sm_max:.0f} MHz (clocks.max.sm; no measured fp64 peak in MEASURED_PEAKS.json)",
             "pairs_per_launch": pairs_per_launch, "avg_launch_ms": pair_avg_ms, "launches_timed": pair_n,
-            "launches_in_timed_steps": K if cfg["variant"] == 7 else 4 * K,
-            "pair_kernel_share_of_steps": (1.0 if cfg["variant"] == 7 else 4 * K * pair_avg_ms / ms_steps) if ms_steps else None,
+            "launches_in_timed_steps": K if cfg["variant"] in ONE_LAUNCH_PER_STEP else 4 * K,
+            "pair_kernel_share_of_steps": (1.0 if cfg["variant"] in ONE_LAUNCH_PER_STEP else 4 * K * pair_avg_ms / ms_steps) if ms_steps else None,
             "kernel_pairs_per_s": kernel_pairs_per_s,
             "frac_at_sampled_clock": (achieved / (peak_tflops * clocks["sm_mhz"] / sm_max)) if achieved and clocks.get("sm_mhz") else None,
             "executed_flops_frac": (kernel_pairs_per_s * exec_flops / 1e12 / peak_tflops) if achieved else None,
