@@ -28,6 +28,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 namespace pn {
 
 struct __align__(16) JRec {
@@ -2285,34 +2287,42 @@ __global__ void __launch_bounds__(NT) energy_pair_kernel(const ERec* __restrict_
         }
         __syncthreads();
         const int j0 = jt * TJ;
+        // the i < j mask is needed inside the diagonal tile only: two loop bodies, so that the 127 of 128 tile pairs off the
+        // diagonal carry no compare / select per pair (two-register non-FP64 instructions cost FP64 operand bandwidth)
+        auto walk_tile = [&](auto diag) {
 #pragma unroll 1
-        for (int jb = 0; jb < TJ; jb += kEGroup) {
-            // kEGroup terms are added plainly (their sum is tiny next to the running total), then the group sum
-            // goes into the compensated accumulator: one TwoSum per kEGroup pairs instead of one per pair
-            double g = 0.0;
+            for (int jb = 0; jb < TJ; jb += kEGroup) {
+                // kEGroup terms are added plainly (their sum is tiny next to the running total), then the group sum
+                // goes into the compensated accumulator: one TwoSum per kEGroup pairs instead of one per pair
+                double g = 0.0;
 #pragma unroll
-            for (int u = 0; u < kEGroup; ++u) {
-                const int jj = jb + u;
-                const ERec r = sj[jj];
-                const double dx = me.x - r.x, dy = me.y - r.y, dz = me.z - r.z;  // x_ij
-                const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
-                const double y0 = rsqrt_seed(r2);
-                const double t2 = y0 * y0;
-                const double e = fma(-r2, t2, 1.0);
-                const double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1/rho to full fp64 accuracy
-                const double vv = fma(me.vx, r.vx, fma(me.vy, r.vy, me.vz * r.vz));
-                const double xvi = fma(dx, me.vx, fma(dy, me.vy, dz * me.vz));
-                const double xvj = fma(dx, r.vx, fma(dy, r.vy, dz * r.vz));
-                // q = -1 + (1/c^2)[w_i + w_j - 7/2 v_i.v_j - 1/2 (x_ij.v_i)(x_ij.v_j)/rho^2]; me.w, r.w carry the 1/c^2
-                double q = wi1 + r.w;
-                q = fma(-c35, vv, q);
-                q = fma(-c05, (xvi * xvj) * (y * y), q);
-                double term = (r.gm * y) * q;
-                term = (j0 + jj <= i) ? 0.0 : term;  // i < j only (false only inside the diagonal tile)
-                g += term;
+                for (int u = 0; u < kEGroup; ++u) {
+                    const int jj = jb + u;
+                    const ERec r = sj[jj];
+                    const double dx = me.x - r.x, dy = me.y - r.y, dz = me.z - r.z;  // x_ij
+                    const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+                    const double y0 = rsqrt_seed(r2);
+                    const double t2 = y0 * y0;
+                    const double e = fma(-r2, t2, 1.0);
+                    const double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1/rho to full fp64 accuracy
+                    const double vv = fma(me.vx, r.vx, fma(me.vy, r.vy, me.vz * r.vz));
+                    const double xvi = fma(dx, me.vx, fma(dy, me.vy, dz * me.vz));
+                    const double xvj = fma(dx, r.vx, fma(dy, r.vy, dz * r.vz));
+                    // q = -1 + (1/c^2)[w_i + w_j - 7/2 v_i.v_j - 1/2 (x_ij.v_i)(x_ij.v_j)/rho^2]; me.w, r.w carry the 1/c^2
+                    double q = wi1 + r.w;
+                    q = fma(-c35, vv, q);
+                    q = fma(-c05, (xvi * xvj) * (y * y), q);
+                    double term = (r.gm * y) * q;
+                    if (decltype(diag)::value) term = (j0 + jj <= i) ? 0.0 : term;  // i < j only
+                    g += term;
+                }
+                two_sum_acc(h_hi, h_lo, g);
             }
-            two_sum_acc(h_hi, h_lo, g);
-        }
+        };
+        if (it == jt)
+            walk_tile(std::true_type{});
+        else
+            walk_tile(std::false_type{});
         if (++jt == n_tiles) {  // next row of the list: the next i-tile, starting at its diagonal pair
             close_row();
             ++it, jt = it;
@@ -2445,29 +2455,35 @@ __global__ void __launch_bounds__(NT) momentum_pair_kernel(const ERec* __restric
         }
         __syncthreads();
         const int j0 = jt * TJ;
+        auto walk_tile = [&](auto diag) {  // the i < j mask inside the diagonal tile only (see energy_pair_kernel)
 #pragma unroll 1
-        for (int jb = 0; jb < TJ; jb += kGroup) {
-            double g[3] = {0, 0, 0};
+            for (int jb = 0; jb < TJ; jb += kGroup) {
+                double g[3] = {0, 0, 0};
 #pragma unroll
-            for (int u = 0; u < kGroup; ++u) {
-                const int jj = jb + u;
-                const ERec r = sj[jj];
-                const double dx = me.x - r.x, dy = me.y - r.y, dz = me.z - r.z;  // x_ij
-                const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
-                const double y0 = rsqrt_seed(r2);
-                const double e = fma(-r2, y0 * y0, 1.0);
-                double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1 / rho
-                y = (j0 + jj <= i) ? 0.0 : y;  // i < j only (also keeps the self pair's 1/0 out when eps = 0)
-                const double ux = me.vx + r.vx, uy = me.vy + r.vy, uz = me.vz + r.vz;
-                const double ud = fma(ux, dx, fma(uy, dy, uz * dz)) * (y * y);
-                const double c = r.gm * y;
-                g[0] = fma(c, fma(ud, dx, ux), g[0]);
-                g[1] = fma(c, fma(ud, dy, uy), g[1]);
-                g[2] = fma(c, fma(ud, dz, uz), g[2]);
+                for (int u = 0; u < kGroup; ++u) {
+                    const int jj = jb + u;
+                    const ERec r = sj[jj];
+                    const double dx = me.x - r.x, dy = me.y - r.y, dz = me.z - r.z;  // x_ij
+                    const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+                    const double y0 = rsqrt_seed(r2);
+                    const double e = fma(-r2, y0 * y0, 1.0);
+                    double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1 / rho
+                    if (decltype(diag)::value) y = (j0 + jj <= i) ? 0.0 : y;  // i < j only (also keeps the self pair's 1/0 out when eps = 0)
+                    const double ux = me.vx + r.vx, uy = me.vy + r.vy, uz = me.vz + r.vz;
+                    const double ud = fma(ux, dx, fma(uy, dy, uz * dz)) * (y * y);
+                    const double c = r.gm * y;
+                    g[0] = fma(c, fma(ud, dx, ux), g[0]);
+                    g[1] = fma(c, fma(ud, dy, uy), g[1]);
+                    g[2] = fma(c, fma(ud, dz, uz), g[2]);
+                }
+#pragma unroll
+                for (int k = 0; k < 3; ++k) two_sum_acc(hi[k], lo[k], g[k]);
             }
-#pragma unroll
-            for (int k = 0; k < 3; ++k) two_sum_acc(hi[k], lo[k], g[k]);
-        }
+        };
+        if (it == jt)
+            walk_tile(std::true_type{});
+        else
+            walk_tile(std::false_type{});
         if (++jt == n_tiles) {
             close_row();
             ++it, jt = it;
