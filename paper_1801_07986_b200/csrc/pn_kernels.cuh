@@ -644,39 +644,51 @@ __global__ void __launch_bounds__(NT, MINB) pair_cross_fp64_kernel(const CRec* _
         if (t + 1 < t_end) fill(buf ^ 1, t + 1);
         const CRec* tile = sj[buf];
         const int j0 = t * TJ;
+        // j != i by index (with eps > 0 the self term does not cancel in these sums): only a tile that overlaps the block's own
+        // i range can hold a self pair, so all other tiles run a body without the compare and the two selects per pair
+        auto walk_tile = [&](auto masked) {
 #pragma unroll 2
-        for (int jj = 0; jj < TJ; ++jj) {
-            const CRec r = tile[jj];
+            for (int jj = 0; jj < TJ; ++jj) {
+                const CRec r = tile[jj];
 #pragma unroll
-            for (int k = 0; k < I; ++k) {
-                const bool self = (j0 + jj == ii[k]);  // j != i in every sum of Eq. 2.6 (eps > 0 does not cancel it here)
-                const double dx = xi[k] - r.x, dy = yi[k] - r.y, dz = zi[k] - r.z;  // x_ij
-                const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
-                const double y0 = rsqrt_seed(r2);
-                const double e = fma(-r2, y0 * y0, 1.0);
-                double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1 / rho to full fp64 accuracy
-                y = self ? 0.0 : y;
-                const double gm = self ? 0.0 : r.gm;
-                const double y2 = y * y;
-                const double s = gm * (y2 * y);  // G m_j / rho^3
-                nx[k] = fma(-s, dx, nx[k]), ny[k] = fma(-s, dy, ny[k]), nz[k] = fma(-s, dz, nz[k]);
-                const double ux = vxi[k] - r.vx, uy = vyi[k] - r.vy, uz = vzi[k] - r.vz;  // v_ij
-                const double uu = fma(ux, ux, fma(uy, uy, uz * uz));
-                const double vjx = fma(r.vx, dx, fma(r.vy, dy, r.vz * dz));
-                const double vix = fma(vxi[k], dx, fma(vyi[k], dy, vzi[k] * dz));
-                double g = fma(r2 - ri2[k], r.b, r.a5) + kapi[k];
-                g = fma(-2.0, uu, g);
-                g = fma(1.5, (vjx * vjx) * y2, g);
-                const double sg = s * g;
-                ax[k] = fma(sg, dx, ax[k]), ay[k] = fma(sg, dy, ay[k]), az[k] = fma(sg, dz, az[k]);
-                S[k] = fma(gm, fma(-r2, r.b, GM4 * y), S[k]);
-                Yx[k] = fma(y, r.wx, Yx[k]), Yy[k] = fma(y, r.wy, Yy[k]), Yz[k] = fma(y, r.wz, Yz[k]);
-                const double h = s * fma(4.0, vix, -3.0 * vjx);
-                H[k] += h;
-                Vx[k] = fma(h, r.vx, Vx[k]), Vy[k] = fma(h, r.vy, Vy[k]), Vz[k] = fma(h, r.vz, Vz[k]);
-                if (BHX) U[k] = fma(gm * y, fma((ri2[k] - r.rj2) * y2, 0.25, 1.25), U[k]);
+                for (int k = 0; k < I; ++k) {
+                    const double dx = xi[k] - r.x, dy = yi[k] - r.y, dz = zi[k] - r.z;  // x_ij
+                    const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+                    const double y0 = rsqrt_seed(r2);
+                    const double e = fma(-r2, y0 * y0, 1.0);
+                    double y = fma(y0 * e, fma(e, 0.375, 0.5), y0);  // 1 / rho to full fp64 accuracy
+                    double gm = r.gm;
+                    if (decltype(masked)::value) {
+                        const bool self = (j0 + jj == ii[k]);
+                        y = self ? 0.0 : y;
+                        gm = self ? 0.0 : gm;
+                    }
+                    const double y2 = y * y;
+                    const double s = gm * (y2 * y);  // G m_j / rho^3
+                    nx[k] = fma(-s, dx, nx[k]), ny[k] = fma(-s, dy, ny[k]), nz[k] = fma(-s, dz, nz[k]);
+                    const double ux = vxi[k] - r.vx, uy = vyi[k] - r.vy, uz = vzi[k] - r.vz;  // v_ij
+                    const double uu = fma(ux, ux, fma(uy, uy, uz * uz));
+                    const double vjx = fma(r.vx, dx, fma(r.vy, dy, r.vz * dz));
+                    const double vix = fma(vxi[k], dx, fma(vyi[k], dy, vzi[k] * dz));
+                    double g = fma(r2 - ri2[k], r.b, r.a5) + kapi[k];
+                    g = fma(-2.0, uu, g);
+                    g = fma(1.5, (vjx * vjx) * y2, g);
+                    const double sg = s * g;
+                    ax[k] = fma(sg, dx, ax[k]), ay[k] = fma(sg, dy, ay[k]), az[k] = fma(sg, dz, az[k]);
+                    S[k] = fma(gm, fma(-r2, r.b, GM4 * y), S[k]);
+                    Yx[k] = fma(y, r.wx, Yx[k]), Yy[k] = fma(y, r.wy, Yy[k]), Yz[k] = fma(y, r.wz, Yz[k]);
+                    const double h = s * fma(4.0, vix, -3.0 * vjx);
+                    H[k] += h;
+                    Vx[k] = fma(h, r.vx, Vx[k]), Vy[k] = fma(h, r.vy, Vy[k]), Vz[k] = fma(h, r.vz, Vz[k]);
+                    if (BHX) U[k] = fma(gm * y, fma((ri2[k] - r.rj2) * y2, 0.25, 1.25), U[k]);
+                }
             }
-        }
+        };
+        const int i_lo = blockIdx.x * (I * NT);
+        if (j0 + TJ > i_lo && j0 < i_lo + I * NT)
+            walk_tile(std::true_type{});
+        else
+            walk_tile(std::false_type{});
         __syncthreads();
     }
     double* out = part + (size_t)blockIdx.y * NC * np;
