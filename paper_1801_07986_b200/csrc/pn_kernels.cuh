@@ -706,6 +706,9 @@ __global__ void __launch_bounds__(NT, MINB) pair_cross_fp64_kernel(const CRec* _
 // ---- the symmetric form: every unordered pair once.  One-warp blocks, I = 2 i-stars per lane, unit tiles of U = 64 stars,
 // the work-item / slot scheme of pair_sym_fp64_kernel (block (A <= B) of a triangular grid over G groups of m tiles: row
 // sums to slot B, column sums to slot A, one writer per (slot, star), nothing zeroed, no atomics).
+#ifndef PN_CROSS_STEPS
+#define PN_CROSS_STEPS 8
+#endif
 constexpr int kCrossSymI = 2;
 constexpr int kCrossSymU = 32 * kCrossSymI;
 template <bool BHX>
@@ -805,7 +808,7 @@ __device__ __forceinline__ void cp_async16(void* dst_smem, const void* src)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-template <int MINB, bool BHX, bool EQM>
+template <int MINB, bool BHX, bool EQM, int CSTEPS = PN_CROSS_STEPS>
 __global__ void __launch_bounds__(32, MINB) pair_cross_sym_kernel(const CRec* __restrict__ crec, double* __restrict__ part /* [G][NC][np] */,
                                                                   int np, int n_tiles, int m, double eps2, double GM4, double gm_eq)
 {
@@ -889,16 +892,17 @@ __global__ void __launch_bounds__(32, MINB) pair_cross_sym_kernel(const CRec* __
                     CrossAcc b;
                     cross_acc_zero(b);
 #pragma unroll 1
-                    for (int c = 0; c < 4; ++c) {  // Gray-code walk in four chunks of 8 steps (see sym_unit_tile_gray)
-                        const int base = jb + (lane ^ ((c & 1 ? 12 : 0) ^ (c & 2 ? 24 : 0)));
-                        const int last_mask = (c & 1) ? 16 : 8;
+                    for (int c = 0; c < 32 / CSTEPS; ++c) {  // Gray-code walk in chunks of CSTEPS steps (see sym_unit_tile_gray)
+                        const int r0 = CSTEPS * c, r1 = r0 + CSTEPS - 1, r2 = (r0 + CSTEPS) & 31;  // g(r) = r ^ (r >> 1)
+                        const int base = jb + (lane ^ (r0 ^ (r0 >> 1)));
+                        const int last_mask = (r1 ^ (r1 >> 1)) ^ (r2 ^ (r2 >> 1));  // into the next chunk or, after step 31, home
 #pragma unroll
-                        for (int q = 0; q < 8; ++q) {
+                        for (int q = 0; q < CSTEPS; ++q) {
                             const CRec r = sj[base ^ (q ^ (q >> 1))];
 #pragma unroll
                             for (int k = 0; k < I; ++k)
                                 cross_pair<true, BHX, EQM>(r, xi[k], vi[k], ri2[k], kapi[k], gmi[k], a5i[k], bi[k], wi[k], acc[k], b, eps2, GM4, false);
-                            cross_acc_shfl<BHX>(b, (q + 1 < 8) ? ((q + 1) & -(q + 1)) : last_mask);
+                            cross_acc_shfl<BHX>(b, (q + 1 < CSTEPS) ? ((q + 1) & -(q + 1)) : last_mask);
                         }
                     }
                     store_acc(b, jb + lane);
