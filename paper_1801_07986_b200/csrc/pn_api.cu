@@ -156,10 +156,11 @@ enum { SYM_W1_U128 = 0, SYM_JS_U128 = 1, SYM_W4_U512 = 2 };
 
 void choose_sym(pn_ctx* c)
 {
-    // measured with the Gray-code walk (profiles/r2_ncu_summary.md section 4): one-warp blocks win only where 120 - 128 one-tile
-    // groups give 7260 - 8256 items of one 128 x 128 tile pair (N_s = 16383: 0.763 against 0.756); below and above (two-tile
-    // groups from 16385 stars on) the j-split form, whose items are a quarter as long; 512-star tiles from 36000 stars on
-    if (c->n_stars < 15360)
+    // measured with the Gray-code walk (profiles/r2_ncu_summary.md section 4): one-warp blocks win only right below 16384 stars,
+    // where 128 one-tile groups give 8256 items of one 128 x 128 tile pair (N_s = 16383: 0.772 against 0.758; at 15359 the
+    // j-split form is ahead again, 0.746 against 0.726); everywhere else below 36000 stars the j-split form, whose items are a
+    // quarter as long; 512-star tiles from 36000 stars on
+    if (c->n_stars < 16000)
         c->sym_kind = SYM_JS_U128;
     else if (c->n_stars <= 16384)
         c->sym_kind = SYM_W1_U128;
