@@ -524,6 +524,7 @@ def run_ours(args) -> None:
             "frac_of_measured_dfma": (achieved / dfma_peak) if achieved and dfma_peak else None,
         }
         bar = bar_leg(args, stream, flush, local, peak_tflops, sm_max) if (world == 1 and args.workload == "config2" and not args.cross and not args.no_bar) else None
+        small = small_leg(stream) if (world == 1 and args.workload == "config2" and not args.cross and not args.no_bar) else None
         base = cpu_baseline(p, terms=cross_mask(args)) if not args.no_cpu_baseline else None
         line = {
             "metric": "fp64 pair-interactions/s", "value": value, "unit": "pair-interactions/s", "n_gpus": world,
@@ -537,12 +538,37 @@ def run_ours(args) -> None:
             "e2e": {"value": e2e_val, "unit": "pair-interactions/s", "h2d_bytes_per_step": 2 * p.N * 24,
                     "d2h_bytes_per_step": 2 * p.N * 24, "ms_per_step": 1e3 * e2e_m / K,
                     "api": "pn_set_state_host + pn_step + pn_get_state_host per step, pinned host buffers"},
-            "gpu_launches": launches, "roofline": roof, "bar": bar, "cpu_baseline": base,
+            "gpu_launches": launches, "roofline": roof, "bar": bar, "config1": small, "cpu_baseline": base,
         }
         print(json.dumps(line), flush=True)
     pn.pn_destroy()
     if world > 1:
         dist.destroy_process_group()
+
+
+def small_leg(stream, steps: int = 200) -> dict:
+    """BASELINE.json configs[0] (N = 1+1023), the small-system path: one pn_step(dt, steps) call = one cooperative launch."""
+    import torch
+
+    from paper_1801_07986_b200 import PN
+
+    p = make_problem("config1")
+    pn = PN(p.mass, p.G, p.c, p.softening, stream=stream)
+    cfg = pn.pn_get_pair_config()
+    pn.pn_set_state(torch.from_numpy(p.pos).cuda(), torch.from_numpy(p.vel).cuda())
+    pn.pn_step(p.dt, 8)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    pn.pn_step(p.dt, steps)
+    b.record(stream)
+    torch.cuda.synchronize()
+    ms = a.elapsed_time(b) / steps
+    launches = pn.pn_get_launch_count()
+    pn.pn_destroy()
+    return {"workload": p.name, "N": p.N, "pair_config": cfg, "steps": steps, "ms_per_step": ms, "steps_per_s": 1e3 / ms,
+            "pairs_per_s": 4 * p.pairs_per_eval / (ms * 1e-3), "launches_for_all_steps": launches - 2,
+            "note": "one cooperative launch runs all steps (small_path_kernel); round 1: 0.0462 ms per step with 8 launches per step"}
 
 
 def bar_leg(args, stream, flush, local, peak_tflops, sm_max, steps: int = 3) -> dict:
