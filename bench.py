@@ -745,7 +745,7 @@ def main():
     ap.add_argument("--kmin", type=int, default=10)
     ap.add_argument("--kmax", type=int, default=20)
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50, help="timed RK4 steps (default: the 50 steps BASELINE.json configs[1] states)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config2")
