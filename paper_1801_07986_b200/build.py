@@ -19,7 +19,7 @@ CSRC = PKG / "csrc"
 INCLUDE = PKG.parent / "include"
 LIB = PKG / "libpn.so"
 SOURCES = [CSRC / "pn_api.cu"]
-HEADERS = [CSRC / "pn_kernels.cuh", INCLUDE / "pn.h"]
+HEADERS = sorted(CSRC.glob("*.cuh")) + [INCLUDE / "pn.h"]
 BENCH_LIB = PKG / "libpn_bench.so"  # roofline-denominator probes for bench.py; not linked into or loaded by the product
 BENCH_SOURCES = [CSRC / "pn_bench.cu"]
 BENCH_HEADERS = [INCLUDE / "pn_bench.h"]

@@ -1,4 +1,4 @@
-"""Combinatorics behind the symmetric pair kernels (paper_1801_07986_b200/csrc/pn_kernels.cuh), checked on the CPU.
+"""Combinatorics behind the symmetric pair kernels (paper_1801_07986_b200/csrc/pn_pair_fp64.cuh, pn_pair_cross.cuh, pn_energy.cuh), checked on the CPU.
 
 The kernels let the j-side sums of a 32-star sub-group travel through the lanes of a warp in Gray-code order: at step r lane l
 works on j-star l ^ g(r), g(r) = r ^ (r >> 1), and after the step the sums move with a butterfly shuffle (lane l receives from
