@@ -1,7 +1,8 @@
 // pn_kernels.cuh -- sm_100a kernels of the limited-1PN hot path (arXiv:1801.07986).
 // Product code: shares nothing with oracle/.  Citations: /root/reference/PAPER.md:<line>.
 //
-// Kernels, in the order of this file (DESIGN.md section 6 has the roofline of each):
+// Kernels (DESIGN.md section 6 has the roofline of each); the parts are included at the end of this file, in this order:
+//   pn_common.cuh, pn_pair_fp64.cuh, pn_pair_cross.cuh, pn_pair_fp32.cuh, pn_epilogue.cuh, pn_small.cuh, pn_energy.cuh
 //   S1  pair_fp64_kernel          star-star Newtonian, every ordered pair, tiled (PN_PAIR_TILED)
 //       pair_sym_fp64_kernel      the same, every unordered pair once (Newton's third law), general / equal-mass form; the
 //                                 j-side sums travel through the lanes of a warp in Gray-code order (N_s >= 3072)
