@@ -17,6 +17,11 @@ using namespace pn;
 
 namespace {
 
+// threads per epilogue block: 32 stars x (threads / 32) warps that share the partial-sum slots.  8 warps for the hot path: at
+// N_s = 16383 the 50 MB of partials come out of L2 and the read is bound by bytes in flight (RK4 step 0.706 -> 0.692 ms;
+// 12 and 16 warps and 2 slots per thread in flight are slower, 4 warps x 8 slots equal); no difference once they stream from HBM.
+constexpr int kEpiNT = 256;
+constexpr int kEpiNTCross = 128;  // 7 - 8 components per slot: 4 warps measure 0.6 % ahead
 constexpr int kNT = 128;        // threads per block of the pair / energy / epilogue kernels
 constexpr int kTJ = 128;        // j records per shared-memory tile
 constexpr int kGraphBatch = 16; // RK4 steps captured in the batched graph
@@ -564,11 +569,11 @@ int enqueue_rk4_step(pn_ctx* c, cudaStream_t st, bool timed)
         int rc = launch_pair(c, 0, st, timed && (c->time_pair != 2 || stage == 0));
         if (rc) return rc;
         if (c->cross & PN_CROSS_BH)
-            epilogue_kernel<MODE_RK4, kNT, 2><<<grid, kNT, 0, st>>>(a, stage);
+            epilogue_kernel<MODE_RK4, kEpiNTCross, 2><<<grid, kEpiNTCross, 0, st>>>(a, stage);
         else if (c->cross)
-            epilogue_kernel<MODE_RK4, kNT, 1><<<grid, kNT, 0, st>>>(a, stage);
+            epilogue_kernel<MODE_RK4, kEpiNTCross, 1><<<grid, kEpiNTCross, 0, st>>>(a, stage);
         else
-            epilogue_kernel<MODE_RK4, kNT, 0><<<grid, kNT, 0, st>>>(a, stage);
+            epilogue_kernel<MODE_RK4, kEpiNT, 0><<<grid, kEpiNT, 0, st>>>(a, stage);
         PN_CUDA(c, cudaGetLastError());
     }
     return PN_OK;
@@ -986,11 +991,11 @@ int pn_accel(pn_ctx* c, const double* pos, const double* vel, double* acc)
     if (int rc = launch_pair(c, 1, c->stream, c->time_pair != 0)) return rc;
     const EpiArgs a = epi_args(c, 1, acc);
     if (c->cross & PN_CROSS_BH)
-        epilogue_kernel<MODE_ACCEL, kNT, 2><<<c->np / kEpiStars, kNT, 0, c->stream>>>(a, 0);
+        epilogue_kernel<MODE_ACCEL, kEpiNTCross, 2><<<c->np / kEpiStars, kEpiNTCross, 0, c->stream>>>(a, 0);
     else if (c->cross)
-        epilogue_kernel<MODE_ACCEL, kNT, 1><<<c->np / kEpiStars, kNT, 0, c->stream>>>(a, 0);
+        epilogue_kernel<MODE_ACCEL, kEpiNTCross, 1><<<c->np / kEpiStars, kEpiNTCross, 0, c->stream>>>(a, 0);
     else
-        epilogue_kernel<MODE_ACCEL, kNT, 0><<<c->np / kEpiStars, kNT, 0, c->stream>>>(a, 0);
+        epilogue_kernel<MODE_ACCEL, kEpiNT, 0><<<c->np / kEpiStars, kEpiNT, 0, c->stream>>>(a, 0);
     PN_CUDA(c, cudaGetLastError());
     c->n_launch += 2 + kernels_per_eval(c);
     return PN_OK;

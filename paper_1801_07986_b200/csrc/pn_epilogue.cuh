@@ -126,7 +126,6 @@ __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
 {
     constexpr int NW = NT / 32;
     constexpr int NC = CROSS == 2 ? 8 : (CROSS ? 7 : 3);
-    static_assert(NW == 4, "the fixed-order cross-warp sum below is written for 4 warps");
     __shared__ double red[3 * NW];
     __shared__ double wsum[NW][NC][kEpiStars];
     __shared__ bool is_last;
@@ -164,7 +163,12 @@ __global__ void __launch_bounds__(NT) epilogue_kernel(EpiArgs A, int stage)
     __syncthreads();
     if (w == 0) {
 #pragma unroll
-        for (int k = 0; k < NC; ++k) ss[k] = ((wsum[0][k][lane] + wsum[1][k][lane]) + wsum[2][k][lane]) + wsum[3][k][lane];
+        for (int k = 0; k < NC; ++k) {
+            double t = wsum[0][k][lane];
+#pragma unroll
+            for (int q = 1; q < NW; ++q) t += wsum[q][k][lane];  // fixed order: warp 0, 1, ...
+            ss[k] = t;
+        }
     }
     const bool live = (w == 0) && (i < A.n_stars);
 
