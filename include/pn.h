@@ -39,6 +39,7 @@
 #ifndef PN_H_
 #define PN_H_
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -145,6 +146,36 @@ int pn_get_pair_config(pn_ctx* ctx, int32_t* cfg_host); /* 8 ints: threads/block
                                                            4 fp64 symmetric, equal-mass form,
                                                            5 fp64 ordered pairs with the Cross terms of Eq. 2.6,
                                                            6 the same with the O(N^2) sum of Eq. 2.3) */
+
+/* The one entry point for callers that cannot allocate device memory (paper_1801_07986_b200/csrc/pn_noalloc.cu).
+ * Every other call needs a pn_ctx, and pn_create obtains its work buffers with cudaMalloc.  That rules the library out
+ * for a program whose own pool already owns (nearly) all of the GPU's memory or that runs under a fixed memory quota --
+ * a further cudaMalloc fails there -- and for a time-critical loop that cannot accept the device-wide stall of
+ * cudaMalloc / cudaFree.  This call needs no context and never calls cudaMalloc, cudaFree or an allocating library
+ * routine.
+ *
+ * Computes a_1, the acceleration of the massive object from all stars, Eqs. 2.1 + 2.2 -- the same
+ * quantity as row 0 of pn_accel's output on the hot path -- and writes its three components to a1_dev.
+ *   N            bodies, 2 <= N <= 1 + PN_NOALLOC_MAX_STARS; PN_EINVAL with a message beyond (nothing is launched)
+ *   masses_dev   N device doubles, masses_dev[0] = M; NOT validated (they stay on the device): NaN / negative values propagate
+ *   pos_dev, vel_dev   device, fp64, row-major [N][3], body 0 first; vel_dev[0] (v_1) is not used (reading R7)
+ *   G > 0 finite; c > 0, +inf for the Newtonian limit
+ *   a1_dev       3 device doubles, written by the kernel
+ *   cuda_stream  a cudaStream_t (NULL: the legacy default stream); the call is asynchronous on it
+ *   errbuf_host / errbuf_len   optional host buffer that receives the error text (pn_last_error does not cover this call)
+ * All pointers belong to the caller and are used only during the call's stream-ordered work.
+ *
+ * The kernel's scratch memory (one partial sum per thread block + a block counter) is a fixed 98 560-byte array inside
+ * the library image: every GPU on which the process uses libpn.so holds it until the process exits, and its size is
+ * what limits N.  The FIRST call on each device looks up that array's device address (cudaGetSymbolAddress, with that
+ * device current), which may load the library's code onto the device: make it during start-up, before any stream
+ * capture.  Later calls on that device enqueue one 256-byte memset (the counter must start at zero; the array keeps
+ * the previous call's contents) and one kernel.  All calls on a device share the array: calls that overlap on the GPU
+ * (different streams, threads or contexts without ordering between them) race and give wrong results -- keep them on
+ * one stream or order them with events. */
+#define PN_NOALLOC_MAX_STARS (1 << 20)
+int pn_bh_accel_noalloc(int64_t N, const double* masses_dev, const double* pos_dev, const double* vel_dev, double G, double c,
+                        double* a1_dev, void* cuda_stream, char* errbuf_host, size_t errbuf_len);
 
 const char* pn_last_error(pn_ctx* ctx); /* ctx may be NULL: last error of a failed pn_create in this thread */
 const char* pn_version(void);

@@ -11,7 +11,7 @@ from . import inputs  # noqa: F401
 
 
 def __getattr__(name):
-    if name in ("PN", "PNError", "load_library", "pn_version"):
+    if name in ("PN", "PNError", "load_library", "pn_version", "pn_bh_accel_noalloc"):
         from . import binding
 
         return getattr(binding, name)

@@ -26,8 +26,9 @@ EXPORTS = (
     "pn_create", "pn_destroy", "pn_set_stream", "pn_set_option", "pn_set_state", "pn_get_state",
     "pn_set_state_host", "pn_get_state_host", "pn_accel", "pn_accel_host", "pn_step", "pn_energy", "pn_momentum",
     "pn_get_launch_count", "pn_get_pair_time", "pn_get_pair_config", "pn_last_error",
-    "pn_version",
+    "pn_version", "pn_bh_accel_noalloc",
 )
+PN_NOALLOC_MAX_STARS = 1 << 20
 
 _lib = None
 
@@ -67,6 +68,7 @@ def load_library() -> ctypes.CDLL:
     lib.pn_last_error.argtypes = [vp]
     lib.pn_last_error.restype = ctypes.c_char_p
     lib.pn_version.argtypes = []
+    lib.pn_bh_accel_noalloc.argtypes = [i64, vp, vp, vp, dbl, dbl, vp, vp, ctypes.c_char_p, ctypes.c_size_t]
     lib.pn_version.restype = ctypes.c_char_p
     for name in EXPORTS:
         if name not in ("pn_last_error", "pn_version"):
@@ -105,6 +107,35 @@ def _host_ptr(a, n: int, name: str) -> int:
             and a.is_contiguous():
         return a.data_ptr()
     raise TypeError(f"{name} must be a host float64 array/tensor of shape ({n}, 3)")
+
+
+def pn_bh_accel_noalloc(masses, pos, vel, G: float, c: float, a1, stream=None):
+    """a_1 (Eqs. 2.1 + 2.2) through the library's one entry point that allocates no device memory.
+
+    It exists for callers that cannot call cudaMalloc -- their own pool owns the GPU's memory, they run under a memory
+    quota, or they sit in a loop that cannot take cudaMalloc's device-wide stall -- so it needs no PN context and the
+    CALLER supplies every tensor, the output included: masses (N,), pos and vel (N, 3), a1 (3,), all contiguous CUDA
+    float64.  At most PN_NOALLOC_MAX_STARS = 2**20 stars (the library's fixed scratch array); PNError(PN_EINVAL) beyond.
+    Asynchronous on `stream` (default: torch's current stream).  The first call on a device does a one-time set-up and
+    should come before any stream capture; calls that overlap on the GPU share the scratch array and race (pn.h).
+    Marshalling only: this function creates no tensor."""
+    import torch
+
+    lib = load_library()
+    n = int(masses.shape[0]) if hasattr(masses, "shape") and len(masses.shape) == 1 else -1
+    for t, shape, name in ((masses, (n,), "masses"), (a1, (3,), "a1")):
+        if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float64 or tuple(t.shape) != shape \
+                or not t.is_contiguous():
+            raise TypeError(f"{name} must be a contiguous CUDA float64 tensor of shape {shape}")
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    handle = getattr(stream, "cuda_stream", stream)
+    err = ctypes.create_string_buffer(512)
+    rc = lib.pn_bh_accel_noalloc(n, masses.data_ptr(), _dev_ptr(pos, n, "pos"), _dev_ptr(vel, n, "vel"), float(G), float(c),
+                                 a1.data_ptr(), ctypes.c_void_p(int(handle)), err, len(err))
+    if rc != PN_OK:
+        raise PNError(rc, err.value.decode())
+    return a1
 
 
 class PN:

@@ -18,7 +18,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 INCLUDE = PKG.parent / "include"
 LIB = PKG / "libpn.so"
-SOURCES = [CSRC / "pn_api.cu"]
+SOURCES = [CSRC / "pn_api.cu", CSRC / "pn_noalloc.cu"]
 HEADERS = sorted(CSRC.glob("*.cuh")) + [INCLUDE / "pn.h"]
 BENCH_LIB = PKG / "libpn_bench.so"  # roofline-denominator probes for bench.py; not linked into or loaded by the product
 BENCH_SOURCES = [CSRC / "pn_bench.cu"]
