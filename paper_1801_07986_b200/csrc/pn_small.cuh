@@ -28,6 +28,7 @@ struct SmallArgs {
     BhState* bh;
     double* bh_part;     // [2][warps of the grid][3]: evaluation e writes set e & 1
     unsigned int* bar;   // [2]: arrival counter of the grid barrier (monotonic; bar_base = its value at launch), give-up flag
+    unsigned int* host_flag;  // mapped host word, set together with the give-up flag: the host sees it without a copy
     double* acc_out;     // MODE_ACCEL: [N][3]
     int n_stars, np;
     double GM, inv_c2, eps2, dt;
@@ -63,23 +64,37 @@ constexpr int kSmallNT = 128;  // threads per block of small_path_kernel (one wa
 
 // ctr[0]: arrivals (monotonic); ctr[1]: set if a wait ever gave up.  The wait is bounded (about half a minute of polling) so
 // that a broken invariant -- blocks not all resident, a counter out of step with the host's copy -- ends in an error the host
-// reports (pn_api.cu: small_check) instead of a hung device.
-__device__ __forceinline__ void small_grid_barrier(unsigned int* ctr, unsigned int target)
+// reports (pn_api.cu: small_check) instead of a hung device.  The bound holds for the whole LAUNCH, not per barrier: a waiting
+// block also looks at the give-up flag (every 1024 polls), and the barrier returns false to every thread of a block that gave
+// up or saw the flag; the kernels then return at once, without another barrier and without writing any state back.
+__device__ __forceinline__ bool small_grid_barrier(unsigned int* ctr, unsigned int target, unsigned int* s_abort /* shared */,
+                                                   unsigned int* host_flag /* mapped host memory */)
 {
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();  // this block's global writes are visible before its arrival is
         atomicAdd(ctr, 1u);
-        unsigned int seen, polls = 0;
-        do {
+        unsigned int seen, polls = 0, abort = 0;
+        for (;;) {
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(ctr) : "memory");
-            if (++polls == (1u << 26)) {
+            if ((int)(seen - target) >= 0) break;
+            ++polls;
+            if ((polls & 1023u) == 0) {
+                asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(abort) : "l"(ctr + 1) : "memory");
+                if (abort) break;  // another block gave up: it will never arrive
+            }
+            if (polls == (1u << 26)) {
                 atomicExch(ctr + 1, 1u);
+                *reinterpret_cast<volatile unsigned int*>(host_flag) = 1u;  // the next API call on the context reports it
+                __threadfence_system();
+                abort = 1;
                 break;
             }
-        } while ((int)(seen - target) < 0);
+        }
+        *s_abort = abort;
     }
     __syncthreads();
+    return *s_abort == 0;
 }
 
 template <int MODE, int IW, int JU, bool MASK>
@@ -90,6 +105,7 @@ __global__ void __launch_bounds__(kSmallNT, 1) small_path_kernel(SmallArgs A)
     __shared__ double red[3 * (kSmallNT / 32)];
     __shared__ BhState sbh;
     __shared__ __align__(8) unsigned long long fill_bar;  // completion of the bulk copy of the stage records
+    __shared__ unsigned int bar_abort;                    // small_grid_barrier: this block gave up / saw the give-up flag
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
     const int np = A.np;
     const int gw = blockIdx.x * (kSmallNT / 32) + w;     // warp of the grid
@@ -238,7 +254,7 @@ __global__ void __launch_bounds__(kSmallNT, 1) small_path_kernel(SmallArgs A)
         }
         // (D) everything of this evaluation is in global memory before anyone starts the next one
         target += gridDim.x;
-        small_grid_barrier(A.bar, target);
+        if (!small_grid_barrier(A.bar, target, &bar_abort, A.host_flag)) return;  // timed out: the host reports it (small_check)
     }
     finish_bh(n_eval - 1);
     __syncthreads();
@@ -275,6 +291,7 @@ struct SmallCrossArgs {
     XVRec* xv;            // [2][np]: evaluation e >= 1 reads set e & 1, evaluation e writes set (e + 1) & 1
     double* bh_part;      // [2][warps of the grid][3]
     unsigned int* bar;
+    unsigned int* host_flag;  // as in SmallArgs
     double* acc_out;
     int n_stars, np;
     double GM, inv_c2, eps2, dt;
@@ -300,6 +317,7 @@ __global__ void __launch_bounds__(kSmallNT, 1) small_cross_kernel(SmallCrossArgs
     __shared__ double scsum[kCrossSums];
     __shared__ BhState sbh;
     __shared__ __align__(8) unsigned long long fill_bar;
+    __shared__ unsigned int bar_abort;
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
     const int gw = blockIdx.x * NW + w;
     const int i0 = gw * IW;
@@ -500,7 +518,7 @@ __global__ void __launch_bounds__(kSmallNT, 1) small_cross_kernel(SmallCrossArgs
             }
         }
         target += gridDim.x;
-        small_grid_barrier(A.bar, target);
+        if (!small_grid_barrier(A.bar, target, &bar_abort, A.host_flag)) return;  // timed out: the host reports it (small_check)
     }
     finish_bh(n_eval - 1);
     __syncthreads();
