@@ -28,6 +28,11 @@
  *     so calls on one context must not run concurrently -- one stream at a time, one host thread at a
  *     time.  pn_set_stream orders the new stream after everything already enqueued on the old one.
  *     Use one context per stream for concurrent work.
+   - Small-system path (PN_PAIR_AUTO, fewer than 3072 stars): its one-launch kernels synchronise their blocks with a grid
+     barrier whose wait is bounded; a launch that gives up (about half a minute; it cannot happen while every block is
+     resident) leaves invalid results.  Calls that synchronise report it at once (PN_ECUDA); callers that only use the
+     asynchronous calls learn of it from the NEXT pn_set_state / pn_get_state / pn_accel / pn_step on the context, which
+     look at a word in mapped host memory that the kernel sets (no copy, no synchronisation in the normal case).
  *   - A context belongs to the CUDA device that was current in pn_create; every later call must be made
  *     with that device current (PN_EINVAL otherwise; pn_destroy switches to it by itself).
  *   - Size limit: 2 <= N <= 2^24 bodies (PN_EINVAL beyond; star indices and tile counts are 32-bit, the
@@ -106,7 +111,12 @@ int pn_create(pn_ctx** out, int64_t N, const double* masses_host, double G, doub
 int pn_destroy(pn_ctx* ctx); /* synchronises, frees everything; NULL is allowed */
 
 int pn_set_stream(pn_ctx* ctx, void* cuda_stream); /* a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); the new
-                                                      stream waits for the work already enqueued on the old one */
+                                                      stream waits for the work already enqueued on the old one.  The OLD
+                                                      stream must still exist at this call: switch first, destroy it afterwards
+                                                      (the CUDA runtime does not validate a destroyed handle -- recording on one
+                                                      crashed inside the driver when tried on a B200).  If the runtime does
+                                                      report an error for the old stream, the call waits for the whole device
+                                                      instead and still switches */
 int pn_set_option(pn_ctx* ctx, int key, int value);
 
 /* Integrator state (x, v) of all N bodies.  [N][3] each. */
@@ -138,7 +148,9 @@ int pn_momentum(pn_ctx* ctx, double* P_host);
 int pn_get_launch_count(pn_ctx* ctx, int64_t* n_kernels_host);          /* kernels launched (graph nodes count) */
 int pn_get_pair_time(pn_ctx* ctx, double* ms_total_host, int64_t* n_launches_host, int reset); /* PN_OPT_TIME_PAIR: sum of
                                                                             the bracketed pair-stage times and their count
-                                                                            since the last reset; synchronises the stream */
+                                                                            since the last reset; synchronises the stream.
+                                                                            On the small-system path (PN_PAIR_AUTO) there is
+                                                                            no separate pair stage: both come back 0 */
 int pn_get_pair_config(pn_ctx* ctx, int32_t* cfg_host); /* 8 ints: threads/block, i per thread, j-tile, partial-sum
                                                            slots (j-splits / groups), grid blocks, padded N_s, pipe
                                                            instructions per ordered pair, variant (0 fp64 tiled,

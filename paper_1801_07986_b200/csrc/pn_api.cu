@@ -67,6 +67,7 @@ struct pn_ctx {
     int small_ok = 0, small_IW = 0, small_blocks = 0;
     double* small_part = nullptr;      // [2][4 small_blocks][3] per-warp partials of a_1
     unsigned int* small_bar = nullptr; // [2]: arrival counter of the grid barrier, give-up flag (small_check)
+    unsigned int* small_host_flag = nullptr; // mapped host word the kernel sets when it gives up (small_poll: no copy, no sync)
     bool small_used = false;           // a small-path launch since the last check
     XVRec* small_xv = nullptr;         // [2][np] exchanged stage state of the small-system path with the Cross terms
     unsigned int small_bar_base = 0;   // its value when the next launch starts
@@ -264,6 +265,7 @@ int launch_small(pn_ctx* c, int mode, double dt, int64_t nsteps, double* acc_out
     a.bh = c->bh[set];
     a.bh_part = c->small_part;
     a.bar = c->small_bar;
+    a.host_flag = c->small_host_flag;
     a.acc_out = acc_out;
     a.n_stars = c->n_stars, a.np = c->np;
     a.GM = c->GM, a.inv_c2 = c->inv_c2, a.eps2 = c->eps2, a.dt = dt;
@@ -332,6 +334,7 @@ int launch_small_cross(pn_ctx* c, int mode, double dt, int64_t nsteps, double* a
     a.xv = c->small_xv;
     a.bh_part = c->small_part;
     a.bar = c->small_bar;
+    a.host_flag = c->small_host_flag;
     a.acc_out = acc_out;
     a.n_stars = c->n_stars, a.np = c->np;
     a.GM = c->GM, a.inv_c2 = c->inv_c2, a.eps2 = c->eps2, a.dt = dt;
@@ -365,6 +368,10 @@ cudaError_t prepare_small(pn_ctx* c)
     e = dalloc(&c->small_part, 2 * 3 * (size_t)4 * c->small_blocks);
     if (e == cudaSuccess) e = dalloc(&c->small_bar, 2);
     if (e == cudaSuccess) e = cudaMemset(c->small_bar, 0, 2 * sizeof(unsigned int));
+    if (e == cudaSuccess && !c->small_host_flag) {
+        e = cudaHostAlloc(reinterpret_cast<void**>(&c->small_host_flag), sizeof(unsigned int), cudaHostAllocMapped);
+        if (e == cudaSuccess) *c->small_host_flag = 0;
+    }
     if (e == cudaSuccess) c->small_ok = 1;
     return e;
 }
@@ -666,10 +673,22 @@ int small_check(pn_ctx* c)
     PN_CUDA(c, cudaMemcpy(&flag, c->small_bar + 1, sizeof flag, cudaMemcpyDeviceToHost));
     if (!flag) return PN_OK;
     cudaMemset(c->small_bar, 0, 2 * sizeof(unsigned int));
+    if (c->small_host_flag) *reinterpret_cast<volatile unsigned int*>(c->small_host_flag) = 0;
     c->small_bar_base = 0;
     c->small_ok = 0;
-    return fail(c, PN_ECUDA, "small-system path: a grid barrier timed out (the results of the last pn_step / pn_accel are invalid); "
-                             "the context uses the multi-kernel path from now on");
+    return fail(c, PN_ECUDA, "small-system path: a grid barrier timed out (the results of the last pn_step / pn_accel are invalid, set the "
+                             "state again); the context uses the multi-kernel path from now on");
+}
+
+// Device-only callers (pn_step, then pn_accel or pn_get_state with their own stream synchronisation) never reach small_check.
+// The kernel that gives up also sets a word in mapped host memory; every asynchronous entry point looks at it first (a plain
+// host read: no copy, no synchronisation), so a failed launch is reported by the NEXT call on the context at the latest.
+int small_poll(pn_ctx* c)
+{
+    if (!c->small_host_flag || !*reinterpret_cast<volatile unsigned int*>(c->small_host_flag)) return PN_OK;
+    PN_CUDA(c, cudaStreamSynchronize(c->stream));  // the launch that gave up drains within the barrier's bound
+    c->small_used = true;
+    return small_check(c);
 }
 
 }  // namespace
@@ -821,6 +840,7 @@ int pn_destroy(pn_ctx* c)
     cudaFree(c->io_pos), cudaFree(c->io_vel), cudaFree(c->io_acc);
     cudaFree(c->crec), cudaFree(c->cblk), cudaFree(c->csum), cudaFree(c->part6), cudaFree(c->blk_mom);
     cudaFree(c->small_part), cudaFree(c->small_bar), cudaFree(c->small_xv);
+    if (c->small_host_flag) cudaFreeHost(c->small_host_flag);
     cudaFree(c->frec), cudaFree(c->fpair), cudaFree(c->erec), cudaFree(c->blk_prep), cudaFree(c->blk_pair), cudaFree(c->d_energy);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     cudaGetLastError();
@@ -836,8 +856,17 @@ int pn_set_stream(pn_ctx* c, void* s)
     if (ns != c->stream) {
         // pn_accel and pn_step share the context's scratch (partial sums, the a_1 block partials and their ticket):
         // work already enqueued on the old stream must finish before anything enqueued on the new one touches it
-        PN_CUDA(c, cudaEventRecord(c->stream_ev, c->stream));
-        PN_CUDA(c, cudaStreamWaitEvent(ns, c->stream_ev, 0));
+        // If the runtime rejects the old stream (e.g. a handle it recognises as invalid), everything on the device is waited
+        // for instead and the context moves to the new stream all the same.  This is no licence to destroy the old stream
+        // first: the runtime does not validate a destroyed handle (cudaEventRecord on one crashed in the driver when tried);
+        // pn.h asks callers to switch first and destroy afterwards.
+        cudaError_t e = cudaEventRecord(c->stream_ev, c->stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(ns, c->stream_ev, 0);
+        if (e != cudaSuccess) {
+            cudaGetLastError();  // clear it: not this call's failure
+            c->stream = ns;      // never stay bound to a dead handle
+            PN_CUDA(c, cudaDeviceSynchronize());
+        }
         c->stream = ns;
     }
     return PN_OK;
@@ -927,6 +956,7 @@ int pn_set_option(pn_ctx* c, int key, int value)
 int pn_set_state(pn_ctx* c, const double* pos, const double* vel)
 {
     if (int rc = check_ctx(c)) return rc;
+    if (int rc = small_poll(c)) return rc;  // a small-system launch that gave up since the last call
     if (!pos || !vel) return fail(c, PN_EINVAL, "pn_set_state: null pointer");
     const int grid = (c->n_stars + 255) / 256;
     pack_kernel<<<grid, 256, 0, c->stream>>>(pos, vel, c->jrec[0], c->v[0], c->x0, c->v0, c->bh[0], c->n_stars, c->np, 1);
@@ -939,6 +969,7 @@ int pn_set_state(pn_ctx* c, const double* pos, const double* vel)
 int pn_get_state(pn_ctx* c, double* pos, double* vel)
 {
     if (int rc = check_ctx(c)) return rc;
+    if (int rc = small_poll(c)) return rc;  // a small-system launch that gave up since the last call
     if (!pos || !vel) return fail(c, PN_EINVAL, "pn_get_state: null pointer");
     if (!c->have_state) return fail(c, PN_ESTATE, "pn_get_state: no state set");
     const int grid = (c->n_stars + 255) / 256;
@@ -976,6 +1007,7 @@ int pn_get_state_host(pn_ctx* c, double* pos, double* vel)
 int pn_accel(pn_ctx* c, const double* pos, const double* vel, double* acc)
 {
     if (int rc = check_ctx(c)) return rc;
+    if (int rc = small_poll(c)) return rc;  // a small-system launch that gave up since the last call
     if (!pos || !vel || !acc) return fail(c, PN_EINVAL, "pn_accel: null pointer");
     const int grid_pack = (c->n_stars + 255) / 256;
     pack_kernel<<<grid_pack, 256, 0, c->stream>>>(pos, vel, c->jrec[1], c->v[1], nullptr, nullptr, c->bh[1], c->n_stars, c->np, 0);
@@ -1018,6 +1050,7 @@ int pn_accel_host(pn_ctx* c, const double* pos, const double* vel, double* acc)
 int pn_step(pn_ctx* c, double dt, int64_t nsteps)
 {
     if (int rc = check_ctx(c)) return rc;
+    if (int rc = small_poll(c)) return rc;  // a small-system launch that gave up since the last call
     if (!std::isfinite(dt)) return fail(c, PN_EINVAL, "pn_step: dt must be finite");
     if (nsteps < 0) return fail(c, PN_EINVAL, "pn_step: nsteps must be >= 0");
     if (!c->have_state) return fail(c, PN_ESTATE, "pn_step: no state set (call pn_set_state first)");

@@ -359,3 +359,4 @@ def test_state_errors_and_bad_arguments():
             pn.pn_set_option(99, 0)
         with pytest.raises(TypeError):
             pn.pn_accel(torch.zeros(5, 3, dtype=torch.float64, device="cuda"), _dev(p.vel))
+
