@@ -54,15 +54,28 @@ SMS, FP64_LANES_PER_SM = 148, 64
 NCU_DRAM_BYTES_PER_PAIR_LAUNCH = {
     (4, 16383): (826624 + 185856, "profiles/r2_ncu_summary.md section 6 (r2_bench_c2, pair_sym_fp64_kernel<4,1,12,0,1,0,8,16>, round-2 build)"),
     (4, 65535): (3268864 + 142611968, "profiles/r2_ncu_summary.md section 6 (r2_bench_c3, pair_sym_fp64_kernel<4,4,3,0,1,0,8,16>, round-2 build)"),
-    (8, 16383): (1872384 + 62415872, "profiles/r2_ncu_summary.md section 8 (r2_cross_sym, pair_cross_sym_kernel<8,0>, before the cp.async prefetch)"),
 }
 
 
-def algorithmic_bytes_per_pair_launch(cfg: dict) -> dict:
-    """What one launch of the star-star kernel has to move: every j record once (48 B per padded star) and the partial
-    sums it hands to the epilogue (24 B per star and slot)."""
-    npad, slots = cfg["padded_stars"], cfg["j_splits"]
-    return {"jrec_read": 48 * npad, "partial_sums_written": 24 * slots * npad, "total": 48 * npad + 24 * slots * npad}
+def algorithmic_bytes_per_pair_launch(cfg: dict):
+    """What one launch of the star-star kernel has to move by design, keyed on the kernel variant: every j record once and
+    the partial sums it hands to the epilogue.  fp64 / fp32-pair hot path (variants 0 - 4): 48 B JRec per padded star, 3
+    doubles per star and slot.  Cross kernels (5, 6, 8 - 11): 112 B CRec per padded star, 7 doubles per star and slot (a^SS,
+    X, S), 8 with the sum U of Eq. 2.3 (variants 6, 9, 11).  Small-system path (7, 12, 13): no partial sums in global memory
+    and no separate pair launch -- null."""
+    v, npad, slots = cfg["variant"], cfg["padded_stars"], cfg["j_splits"]
+    if v in ONE_LAUNCH_PER_STEP:
+        return None
+    if v in (0, 1, 2, 3, 4):
+        rec, comps = 48, 3
+    elif v in (5, 8, 10):
+        rec, comps = 112, 7
+    elif v in (6, 9, 11):
+        rec, comps = 112, 8
+    else:
+        return None
+    return {"record_bytes": rec, "sum_components": comps, "jrec_read": rec * npad, "partial_sums_written": 8 * comps * slots * npad,
+            "total": rec * npad + 8 * comps * slots * npad}
 
 
 _BENCH_LIB = None

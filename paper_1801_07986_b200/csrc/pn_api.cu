@@ -156,7 +156,7 @@ constexpr int kSymMaxGroups = 128;  // partial-sum slots of the symmetric kernel
 
 // Symmetric (Newton's third law) kernel variants, by problem size (measured on a B200, profiles/r2_ncu_summary.md): the
 // j-split form (4 warps share one 128 x 128 unit-tile pair: work items a quarter as long) where the grid is small,
-// one-warp blocks around N_s = 16384, 512-star unit tiles (4 warps, 128 i-stars each) from 40000 stars on, where the
+// one-warp blocks around N_s = 16384, 512-star unit tiles (4 warps, 128 i-stars each) from 36000 stars on, where the
 // tile prologue and flush weigh least.
 enum { SYM_W1_U128 = 0, SYM_JS_U128 = 1, SYM_W4_U512 = 2 };
 

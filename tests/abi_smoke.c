@@ -67,7 +67,9 @@ int main(void)
     /* the star has moved along its nearly circular orbit (a = -0.97 instead of -1); E stays put up to the orders the
        limited 1PN equations drop (c = 10, m / M = 1e-3: DESIGN.md reading R8), so this is a sanity bound, not parity */
     if (!(x[1][1] > 0.099 && x[1][1] < 0.101 && x[1][0] < 1.0 && x[1][0] > 0.99) || !close_to(e1, e0, 1e-2, 0) ||
-        launches < 8) { /* N = 2 takes the small-system path: the 100 steps are ONE cooperative launch */
+        launches < 8) { /* kernels of the whole program, not of pn_step: N = 2 takes the small-system path, where the 100 steps
+                           are ONE cooperative launch; with pack + accel (2), pack (1), two energies (3 each) and unpack (1)
+                           that makes 11.  The bound only says that every call really launched kernels */
         fprintf(stderr, "after 100 steps: x = (%.17g, %.17g), E = %.17g (E0 %.17g), launches %lld\n", x[1][0], x[1][1], e1, e0,
                 (long long)launches);
         pn_destroy(ctx);

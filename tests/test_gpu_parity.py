@@ -79,8 +79,10 @@ def test_accel_parity_other_distributions(gen):
 
 
 # both fp64 star-star kernels at every size class: the tiled one (ordered pairs) and the symmetric one (unordered
-# pairs applied to both stars) in its three unit-tile variants (U = 64: N_s < 12288, 128: < 49152, 512 above),
-# with one group per tile (m = 1) and several (9000 -> T = 144, m = 2; 20000 -> T = 157, m = 2, ragged last group)
+# pairs applied to both stars) in the forms choose_sym (pn_api.cu) picks by size: the j-split form on 128-star unit tiles
+# (below 16000 stars and from 16385 to 35999), one-warp blocks on 128-star tiles (16000 ... 16384), 512-star tiles from
+# 36000 stars on (test_gpu_fullsize.py covers those), with one group per tile (m = 1) and several (20000 -> T = 157,
+# m = 2, ragged last group)
 # "symmetric" on equal-mass stars takes the equal-mass form (variant 4: rho^-3 d accumulated, G m applied at the flush);
 # "symmetric_general" switches that off (variant 2), which is also what unequal masses get.
 @pytest.mark.parametrize("kernel", ["tiled", "symmetric", "symmetric_general"])
