@@ -37,8 +37,10 @@
  * NEXT rows (Cross terms, Eqs. 2.3 and 2.6; momentum, Eq. 2.8): residual orders lam^3 / lam^2 / lam^3 against the full
  * EIH acceleration and momentum, hand values for two bodies, bit-identity with the hot path at c = inf and for massless
  * stars, two-body finite-mass periastron advance 6 pi G (M + m) / (c^2 a (1 - e^2)) and energy conservation.
- * Parity unpinned: the softening convention inside the 1PN star-star energy bracket, the Cross terms and the
- * momentum (every star-star r_ij -> rho_ij, n_ij -> x_ij / rho_ij, reading R9) -- exact at eps = 0, a convention otherwise.
+ * Softening inside the 1PN star-star energy bracket, the Cross terms and the momentum (every star-star r_ij -> rho_ij,
+ * the r_ij^2 numerators and n_ij -> x_ij / rho_ij included, reading R9) is a convention the paper does not fix (exact at
+ * eps = 0).  That the convention is APPLIED at every occurrence is pinned by hand values at eps^2 = 11 (rho_AB = 6):
+ * tests/golden/n3_345_softened.txt (energy) and n3_345_softened_cross.txt (Eqs. 2.6, 2.3, 2.8, worked line by line).
  */
 #include <math.h>
 #include <stdint.h>

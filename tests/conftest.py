@@ -30,9 +30,11 @@ def load_golden(name: str) -> dict:
         key, *vals = line.split()
         out[key] = np.array([_num(v) for v in vals], dtype=np.float64)
     n = out["mass"].shape[0]
-    for k in ("pos", "vel", "acc", "acc_newton"):
+    for k in ("pos", "vel", "acc", "acc_newton", "acc_cross_star", "acc_cross_full"):
         if k in out:
             out[k] = out[k].reshape(n, 3)
+    if "cross_star" in out:  # [a_i]_Cross of the stars only (bodies 1 .. N-1)
+        out["cross_star"] = out["cross_star"].reshape(n - 1, 3)
     for k in ("G", "c", "eps", "eps2", "energy", "energy_newton"):
         if k in out:
             out[k] = float(out[k][0])

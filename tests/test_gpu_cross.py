@@ -165,3 +165,26 @@ def test_cross_rk4_trajectory_tracks_oracle(terms, kernel):
     assert np.array_equal(x, x2) and np.array_equal(v, v2)
     assert max(rel_err_rows(x, xr).max(), rel_err_rows(v, vr).max()) <= 1e-11
     assert rel_err_rows(v, vh).max() > 1e-9  # and it is not the hot-path trajectory
+
+
+@pytest.mark.parametrize("kernel", ["auto", "tiled", "symmetric"])
+def test_cross_hand_values_softened_345_on_gpu(kernel):
+    """tests/golden/n3_345_softened_cross.txt (Eqs. 2.6 + 2.3 with rho_AB = 6, worked by hand) straight through the C-ABI:
+    the small-system kernel, the ordered-pair kernel and the symmetric kernel each soften every star-star distance."""
+    from paper_1801_07986_b200 import PN, binding
+    from tests.conftest import load_golden
+
+    g = load_golden("n3_345_softened_cross.txt")
+    opt = {"auto": binding.PN_PAIR_AUTO, "tiled": binding.PN_PAIR_TILED, "symmetric": binding.PN_PAIR_SYMMETRIC}[kernel]
+    for terms, key in ((CROSS_STAR, "acc_cross_star"), (CROSS_STAR | CROSS_BH, "acc_cross_full")):
+        with PN(g["mass"], g["G"], g["c"], g["eps"]) as pn:
+            pn.pn_set_option(binding.PN_OPT_CROSS_TERMS, terms)
+            pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, opt)
+            acc = pn.pn_accel(_dev(g["pos"]), _dev(g["vel"])).cpu().numpy()
+        assert rel_err_rows(acc, g[key]).max() <= 1e-14, (kernel, key)
+        # the Cross part by itself is 1e-4 of a_i here: it must be right to 1e-10 of its own size
+        hot = load_golden("n3_345_softened.txt")["acc"]
+        cr = (acc - hot) * g["c"] ** 2
+        np.testing.assert_allclose(cr[1:], g["cross_star"], rtol=0, atol=1e-10 * np.abs(g["cross_star"]).max())
+        if terms & CROSS_BH:
+            np.testing.assert_allclose(cr[0], g["cross_bh"], rtol=0, atol=1e-9 * np.abs(g["cross_bh"]).max())

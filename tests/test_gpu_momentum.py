@@ -54,3 +54,15 @@ def test_momentum_is_conserved_better_with_the_cross_terms():
             pn.pn_step(p.dt, 50)
             drift[terms] = np.abs(pn.pn_momentum() - P0).max()
     assert drift[3] < 0.5 * drift[0]  # measured: 4.8e-8 against 2.4e-7 (what is left is the dropped star-star 1PN terms, R8)
+
+
+def test_momentum_hand_value_softened_345_on_gpu():
+    """Eq. 2.8 of the softened 3-4-5 system, worked by hand (tests/golden/n3_345_softened_cross.txt), through the C-ABI."""
+    from paper_1801_07986_b200 import PN
+    from tests.conftest import load_golden
+
+    g = load_golden("n3_345_softened_cross.txt")
+    with PN(g["mass"], g["G"], g["c"], g["eps"]) as pn:
+        pn.pn_set_state_host(g["pos"], g["vel"])
+        P = pn.pn_momentum()
+    np.testing.assert_allclose(P, g["momentum"], rtol=1e-14, atol=0)

@@ -518,6 +518,34 @@ def test_cross_terms_hand_values_two_bodies():
     np.testing.assert_allclose(a[1] - hot[1], [5.75e-5, 0.0, 0.0], rtol=1e-12, atol=1e-18)
 
 
+def test_cross_terms_and_momentum_hand_values_softened_345():
+    """The eps > 0 branch of Eqs. 2.6, 2.3 and 2.8 (reading R9: every star-star distance softened, the r_ij^2 numerators and
+    n_ij included): tests/golden/n3_345_softened_cross.txt, worked by hand in exact fractions (rho_AB = 6).  One unsoftened
+    occurrence of r_ij in cross_star, cross_bh or oracle_momentum moves a value here by 1e-3 ... 1e-1 of itself."""
+    from oracle.pn_oracle import CROSS_BH, CROSS_STAR
+    from tests.conftest import load_golden, rel_err_rows
+
+    g = load_golden("n3_345_softened_cross.txt")
+    args = (g["mass"], g["G"], g["c"], g["eps"])
+    hot = Oracle(*args).accel(g["pos"], g["vel"])
+    star = Oracle(*args, terms=CROSS_STAR).accel(g["pos"], g["vel"])
+    full = Oracle(*args, terms=CROSS_STAR | CROSS_BH).accel(g["pos"], g["vel"])
+    assert rel_err_rows(star, g["acc_cross_star"]).max() <= 1e-14
+    assert rel_err_rows(full, g["acc_cross_full"]).max() <= 1e-14
+    # the Cross terms by themselves (1e-2 ... 1e-4 of the acceleration): difference to the hot path, times c^2
+    c2 = g["c"] ** 2
+    np.testing.assert_allclose((star[1:] - hot[1:]) * c2, g["cross_star"], rtol=0, atol=1e-12 * np.abs(g["cross_star"]).max())
+    np.testing.assert_allclose((full[0] - hot[0]) * c2, g["cross_bh"], rtol=0, atol=1e-11 * np.abs(g["cross_bh"]).max())
+    np.testing.assert_array_equal(star[0], hot[0])
+    P = Oracle(*args).momentum(g["pos"], g["vel"])
+    np.testing.assert_allclose(P, g["momentum"], rtol=1e-14, atol=0)
+    # and the softening matters at the level the pin resolves: eps = 0 changes every one of these values
+    full0 = Oracle(g["mass"], g["G"], g["c"], 0.0, terms=CROSS_STAR | CROSS_BH).accel(g["pos"], g["vel"])
+    hot0 = Oracle(g["mass"], g["G"], g["c"], 0.0).accel(g["pos"], g["vel"])
+    assert np.abs((full0 - hot0) - (full - hot)).max() * c2 > 1e-2 * np.abs(g["cross_star"]).max()
+    assert np.abs(Oracle(g["mass"], g["G"], g["c"], 0.0).momentum(g["pos"], g["vel"]) - P).max() > 1e-9
+
+
 # ------------------------------------------------------------------ symmetries every term must respect
 def _rotation(seed):
     rng = np.random.default_rng(seed)
