@@ -80,10 +80,36 @@ def test_config4_full_size_fp32_variant():
     _check_sampled(inputs.config(4), 128, precision=binding.PN_FP32_PAIR, tol=TOL_FP32)
 
 
-@pytest.mark.parametrize("k", [10, 14, 17, 20])
-def test_config5_sweep_sampled_rows(k):
-    """k = 20 is the largest size of the sweep (N = 2^20: 3.2 GB of partial sums, 16 unit tiles per group)."""
-    _check_sampled(inputs.uniform_ball_bh(k), 256 if k < 20 else 64)
+_C5_REF = {}  # k -> (problem, rows, oracle rows): one size at a time, shared by the two precisions
+
+
+def _config5_ref(k):
+    if k not in _C5_REF:
+        _C5_REF.clear()
+        p = inputs.uniform_ball_bh(k)
+        rows = np.arange(p.N, dtype=np.int64) if k <= 14 else _sample_rows(p, 4096)
+        _C5_REF[k] = (p, rows, Oracle(p.mass, p.G, p.c, p.softening).accel_rows(p.pos, p.vel, rows))
+    return _C5_REF[k]
+
+
+@pytest.mark.parametrize("precision", ["fp64", "fp32pair"])
+@pytest.mark.parametrize("k", list(range(10, 21)))
+def test_config5_sweep_every_size_both_precisions(k, precision):
+    """BASELINE.json config 5 as stated: one force evaluation at N = 1 + (2^k - 1) for EVERY k = 10 ... 20 (uniform ball,
+    Gaussian velocities, seed k), in the fp64 path and in the fp32-pair / fp64-accumulate variant, in the launch configuration
+    bench.py --sweep times (automatic kernel choice).  Every row against the long-double oracle up to k = 14, a seeded
+    4096-row subset (each row against ALL j) above; k = 20: 3.2 GB of partial sums, 16 unit tiles per group."""
+    from paper_1801_07986_b200 import PN, binding
+
+    p, rows, ref = _config5_ref(k)
+    with PN(p.mass, p.G, p.c, p.softening) as pn:
+        if precision == "fp32pair":
+            pn.pn_set_option(binding.PN_OPT_PAIR_PRECISION, binding.PN_FP32_PAIR)
+        acc = pn.pn_accel(_dev(p.pos), _dev(p.vel)).cpu().numpy()
+        cfg = pn.pn_get_pair_config()
+    assert np.isfinite(acc).all()
+    err = rel_err_rows(acc[rows], ref)
+    assert err.max() <= (TOL_ACC if precision == "fp64" else TOL_FP32), (k, precision, cfg, float(err.max()))
 
 
 def test_large_n_offsets_beyond_32_bits():
