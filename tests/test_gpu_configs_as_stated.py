@@ -1,4 +1,8 @@
-"""BASELINE.json configs 3 and 4 run AS STATED through the CUDA path, against the long-double oracle.
+"""BASELINE.json configs 2, 3 and 4 run AS STATED through the CUDA path, against the long-double oracle.
+
+config 2 (configs[1], the metric's config): N = 1+16383 Plummer + BH 0.1, dt = 1e-4, all 50 steps: trajectory and 1PN
+    energy after every step against the oracle's 50-step run (tests/golden/config2_digest.npz, 128 rows per step; the
+    full run with 2048 rows + the final state in tests/cache/ when present), same script as config 3.
 
 config 3 (configs[2]): N = 1+65535 Bahcall-Wolf cusp, dt = 1e-5, 20 steps, "1PN energy drift tracked": the GPU trajectory
     and E after every step against the oracle's full-size 20-step run (3.4e11 long-double pair visits + 21 O(N^2)
@@ -31,16 +35,57 @@ def _dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-def load_config3_reference(p):
-    """The oracle's 20-step run of config 3: the full cache if it is there, else the committed subset of the same run."""
+def load_traj_reference(p, name):
+    """The oracle's run of a config as stated: the full cache if it is there, else the committed subset of the same run."""
     key = ref_key(p)
-    for path in (CACHE / "config3_traj.npz", GOLDEN / "config3_digest.npz"):
+    for path in (CACHE / f"{name}_traj.npz", GOLDEN / f"{name}_digest.npz"):
         if path.exists():
             z = np.load(path)
             if str(z["key"]) == key:
                 return {k: z[k] for k in z.files}, path.name
-    pytest.fail("no oracle reference for config 3 matches oracle/pn_oracle.c and the seeded inputs: "
-                "run `python tests/make_fullsize_refs.py --only config3` (about 1.5 h of host time)")
+    pytest.fail(f"no oracle reference for {name} matches oracle/pn_oracle.c and the seeded inputs: "
+                f"run `python tests/make_fullsize_refs.py --only {name}` (config 3: about 1.5 h of host time, config 2: 0.5 h)")
+
+
+def load_config3_reference(p):
+    return load_traj_reference(p, "config3")
+
+
+def _run_as_stated(p, ref, variant):
+    """pn_step one step at a time; after every step the sampled rows of (x, v) and the drift against the oracle's."""
+    from paper_1801_07986_b200 import PN
+
+    rows, E = ref["rows"], ref["E"]
+    assert E.shape == (p.nsteps + 1,) and ref["x_rows"].shape[:2] == (p.nsteps, rows.size)
+    with PN(p.mass, p.G, p.c, p.softening) as pn:
+        assert pn.pn_get_pair_config()["variant"] == variant  # the kernel bench.py times at this size
+        pn.pn_set_state_host(p.pos, p.vel)
+        e0 = pn.pn_energy()
+        assert e0 == pytest.approx(E[0], rel=1e-13)
+        worst_traj = worst_drift = 0.0
+        for s in range(p.nsteps):
+            pn.pn_step(p.dt, 1)
+            x, v = pn.pn_get_state_host()
+            worst_traj = max(worst_traj, rel_err_rows(x[rows], ref["x_rows"][s]).max(),
+                             rel_err_rows(v[rows], ref["v_rows"][s]).max())
+            d_gpu = (pn.pn_energy() - e0) / abs(e0)
+            d_ref = (E[s + 1] - E[0]) / abs(E[0])
+            worst_drift = max(worst_drift, abs(d_gpu - d_ref))
+        if "x_final" in ref:  # the cache holds every row of the final state
+            worst_traj = max(worst_traj, rel_err_rows(x, ref["x_final"]).max(), rel_err_rows(v, ref["v_final"]).max())
+    return worst_traj, worst_drift, d_ref
+
+
+def test_config2_full_size_50_steps():
+    """The metric's configuration exactly as BASELINE.json states it: 50 RK4 steps at N = 1+16383, every step compared."""
+    p = inputs.config(2)
+    ref, source = load_traj_reference(p, "config2")
+    assert p.nsteps == 50
+    worst_traj, worst_drift, d_last = _run_as_stated(p, ref, variant=4)
+    print(f"config 2 ({source}): oracle drift after 50 steps {d_last:.3e}, worst trajectory error {worst_traj:.2e}, "
+          f"worst drift difference {worst_drift:.2e}")
+    assert worst_traj <= TOL_TRAJ
+    assert worst_drift <= TOL_DRIFT
 
 
 def load_config4_energy(p):
