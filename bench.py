@@ -14,6 +14,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -266,7 +267,9 @@ class NvmlSampler:
         bits = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
         reasons = sorted(nm for nm, b in bits.items() if any(r[2] & b for r in rows))
         return {"sm_mhz": float(np.median([r[1] for r in rows])) if rows else None, "sm_max_mhz": float(smax),
-                "power_w_max": max((r[3] for r in rows), default=None), "samples": len(rows), "reasons": reasons,
+                "sm_mhz_min": float(min(r[1] for r in rows)) if rows else None,
+                "power_w_max": max((r[3] for r in rows), default=None),
+                "power_w_mean": float(np.mean([r[3] for r in rows])) if rows else None, "samples": len(rows), "reasons": reasons,
                 "source": "nvml, 2 ms poll during the timed region"}
 
 
@@ -501,8 +504,12 @@ def run_ours(args) -> None:
 
     # ---------------- max over ranks, whole-job aggregate
     pairs_per_step = 4 * p.pairs_per_eval
-    ms_total_m, ms_steps_m, e2e_m, ms_graph_m = max_over_ranks([ms_total, ms_steps, e2e_s, ms_graph], world, "cuda")
-    value = whole_job_rate(world, K, pairs_per_step, ms_total_m * 1e-3)
+    ms_total_m, ms_steps_m, e2e_m, ms_graph_m, ms_energy_m = max_over_ranks([ms_total, ms_steps, e2e_s, ms_graph, ms_energy], world, "cuda")
+    # `value` must not depend on --steps: the timed region holds K steps and 2 energy evaluations, the workload as stated
+    # (BASELINE.json: p.nsteps steps, E at the start and at the end) holds 2 per p.nsteps steps.  One step is therefore charged
+    # its own measured time plus 2 / p.nsteps of a measured energy evaluation, whatever K was; the raw sums are reported too.
+    ms_step_charged = ms_steps_m / K + (ms_energy_m / 2) * (2.0 / p.nsteps)
+    value = whole_job_rate(world, 1, pairs_per_step, ms_step_charged * 1e-3)
     e2e_val = whole_job_rate(world, K, pairs_per_step, e2e_m)
 
     if rank == 0:
@@ -537,21 +544,26 @@ def run_ours(args) -> None:
             "frac_of_measured_dfma": (achieved / dfma_peak) if achieved and dfma_peak else None,
         }
         bar = bar_leg(args, stream, flush, local, peak_tflops, sm_max, dfma_peak) if (world == 1 and args.workload == "config2" and not args.cross and not args.no_bar) else None
+        sustained = ([sustained_leg(w, stream, local, peak_tflops, args.sustain_s) for w in ("config2", "config3")]
+                     if (world == 1 and args.workload == "config2" and not args.cross and not args.no_bar and args.sustain_s > 0) else None)
         small = small_leg(stream) if (world == 1 and args.workload == "config2" and not args.cross and not args.no_bar) else None
         base = cpu_baseline(p, terms=cross_mask(args)) if not args.no_cpu_baseline else None
         line = {
             "metric": "fp64 pair-interactions/s", "value": value, "unit": "pair-interactions/s", "n_gpus": world,
-            "steps": K, "warmup": W, "ms_per_step": ms_total_m / K, "higher_is_better": True, "scaling": "weak",
+            "steps": K, "warmup": W, "ms_per_step": ms_step_charged, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(p, args),
-            "steps_per_s": world * K / (ms_total_m * 1e-3), "rk4_only_ms_per_step": ms_steps_m / K,
-            "energy_ms_per_eval": ms_energy / 2, "graph_ms_per_step": ms_graph_m / K,
+            "steps_per_s": world / (ms_step_charged * 1e-3), "rk4_only_ms_per_step": ms_steps_m / K,
+            "energy_ms_per_eval": ms_energy_m / 2, "timed_region_ms": ms_total_m,
+            "value_definition": f"pairs of one RK4 step / (measured ms per step + 2/{p.nsteps} of a measured pn_energy): the workload as "
+                                f"stated has 2 energy evaluations per {p.nsteps} steps; independent of --steps",
+            "graph_ms_per_step": ms_graph_m / K,
             "graph_pairs_per_s": whole_job_rate(world, K, pairs_per_step, ms_graph_m * 1e-3),
             "energy_drift": (e_end - e_start) / abs(e_start), "pair_config": cfg,
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": "pair-interactions/s", "h2d_bytes_per_step": 2 * p.N * 24,
                     "d2h_bytes_per_step": 2 * p.N * 24, "ms_per_step": 1e3 * e2e_m / K,
                     "api": "pn_set_state_host + pn_step + pn_get_state_host per step, pinned host buffers"},
-            "gpu_launches": launches, "roofline": roof, "bar": bar, "config1": small, "cpu_baseline": base,
+            "gpu_launches": launches, "roofline": roof, "bar": bar, "sustained": sustained, "config1": small, "cpu_baseline": base,
         }
         print(json.dumps(line), flush=True)
     pn.pn_destroy()
@@ -582,6 +594,57 @@ def small_leg(stream, steps: int = 200) -> dict:
     return {"workload": p.name, "N": p.N, "pair_config": cfg, "steps": steps, "ms_per_step": ms, "steps_per_s": 1e3 / ms,
             "pairs_per_s": 4 * p.pairs_per_eval / (ms * 1e-3), "launches_for_all_steps": launches - 2,
             "note": "one cooperative launch runs all steps (small_path_kernel); round 1: 0.0462 ms per step with 8 launches per step"}
+
+
+def sustained_leg(workload: str, stream, local, peak_tflops, seconds: float) -> dict:
+    """>= `seconds` of back-to-back pn_step on the batched CUDA graph (what a production run does; PAPER.md:130 times
+    32-step runs, PAPER.md:172 runs 1.3 M steps), clocks / power / throttle reasons sampled over the whole leg, then -- with no
+    pause -- a short instrumented stretch (event-record nodes around the pair stage of the first force evaluation of every
+    step) for the pair kernel's in-graph fraction of the FP64 issue roofline under the same thermal state."""
+    import torch
+
+    from paper_1801_07986_b200 import PN, binding
+
+    p = make_problem(workload)
+    pn = PN(p.mass, p.G, p.c, p.softening, stream=stream)
+    cfg = pn.pn_get_pair_config()
+    kname, instr, exec_flops = PAIR_KERNELS[cfg["variant"]]
+    pn.pn_set_state(torch.from_numpy(p.pos).cuda(), torch.from_numpy(p.vel).cuda())
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    pn.pn_step(p.dt, 32)
+    b.record(stream)
+    torch.cuda.synchronize()
+    est = a.elapsed_time(b) / 32
+    steps = int(math.ceil(seconds * 1e3 / est / 16.0)) * 16
+    sampler = make_sampler(local)
+    sampler.start()
+    t0 = time.perf_counter()
+    a.record(stream)
+    pn.pn_step(p.dt, steps)
+    b.record(stream)
+    torch.cuda.synchronize()  # the option drops the captured graphs: not while they run (the rebuild idles the GPU for a few ms)
+    pn.pn_set_option(binding.PN_OPT_TIME_PAIR, 2)
+    n_inst = max(8, min(200, steps // 10))
+    pn.pn_step(p.dt, n_inst)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    clocks = sampler.stop(t0, t1)
+    ms = a.elapsed_time(b) / steps
+    pair_ms, pair_n = pn.pn_get_pair_time(reset=True)
+    pn.pn_destroy()
+    avg = pair_ms / max(1, pair_n)
+    rate = p.pairs_per_eval / (avg * 1e-3) if pair_n else None
+    return {"workload": p.name, "N": p.N, "kernel": kname, "steps": steps, "seconds": a.elapsed_time(b) * 1e-3, "ms_per_step": ms,
+            "steps_per_s": 1e3 / ms, "pairs_per_s": 4 * p.pairs_per_eval / (ms * 1e-3),
+            "step_frac": 4 * p.pairs_per_eval / (ms * 1e-3) * 2 * instr / 1e12 / peak_tflops,
+            "pair_stage": {"launches_timed": pair_n, "avg_launch_ms": avg, "kernel_pairs_per_s": rate,
+                           "frac": (rate * 2 * instr / 1e12 / peak_tflops) if rate else None,
+                           "executed_flops_frac": (rate * exec_flops / 1e12 / peak_tflops) if rate else None,
+                           "note": f"{n_inst} instrumented steps right after the sustained stretch (a few ms of graph rebuild in between)"},
+            "clocks": clocks,
+            "note": "batched CUDA graph (16 steps per launch), no L2 flush, no energy evaluation; step_frac = whole step against the "
+                    "pair kernel's issue roofline (epilogues and launch gaps count as loss)"}
 
 
 def bar_leg(args, stream, flush, local, peak_tflops, sm_max, dfma_peak=None, steps: int = 3) -> dict:
@@ -671,12 +734,73 @@ def run_sweep(args) -> None:
             pair_ms, n = pn.pn_get_pair_time(reset=True)
             pair_ms = pair_ms / n if n else ms  # small-system path: no separate pair stage, the evaluation is one launch
             tfl = p.pairs_per_eval * 2 * instr / (pair_ms * 1e-3) / 1e12
+            epi = None
+            cfg = pn.pn_get_pair_config()
+            if cross == 0 and prec == binding.PN_FP64 and cfg["variant"] not in ONE_LAUNCH_PER_STEP:
+                # the O(N) kernel of the hot path (fused S2 + S3 + S4 epilogue) inside captured RK4 steps: the interval between two
+                # bracketed pair stages.  Design bytes: the partial sums it reduces (24 B per star and slot) + the per-star state
+                # it reads and writes (stages 0 - 2: 216, 264, 264 B); algorithmic bytes: SURVEY.md 8(d), ~100 B per body.
+                dt = getattr(p, "dt", None) or 1e-4
+                pn.pn_set_state(pos, vel)
+                pn.pn_step(dt, 1)
+                pn.pn_get_pair_time(reset=True), pn.pn_get_epilogue_time(reset=True)
+                pn.pn_step(dt, 3)
+                e_ms, e_n = pn.pn_get_epilogue_time(reset=True)
+                pn.pn_get_pair_time(reset=True)
+                if e_n:
+                    t = e_ms / e_n * 1e-3
+                    design = 24 * cfg["j_splits"] * cfg["padded_stars"] + 248 * p.n_stars
+                    hbm = peaks.get("hbm_gbs", 6549.4)
+                    epi = {"kernel": "epilogue_kernel<MODE_RK4>", "intervals": e_n, "avg_ms": e_ms / e_n, "design_bytes": design,
+                           "algorithmic_bytes": 100 * p.N, "gbs_design": design / t / 1e9, "gbs_algorithmic": 100 * p.N / t / 1e9,
+                           "hbm_peak_gbs": hbm, "frac_of_hbm_design": design / t / 1e9 / hbm,
+                           "note": "interval between two bracketed pair stages of a captured RK4 step (one epilogue launch + its launch "
+                                   "gaps); L2-resident below N ~ 2^18, HBM-bound only at the largest sizes"}
             print(json.dumps({
                 "workload": name, "N": p.N, "precision": pname, "pairs": p.pairs_per_eval, "accel_ms": ms,
                 "accel_pairs_per_s": p.pairs_per_eval / (ms * 1e-3), "pair_kernel_ms": pair_ms,
                 "pair_kernel_pairs_per_s": p.pairs_per_eval / (pair_ms * 1e-3), "pipe_instr_per_pair": instr,
-                "roofline_frac": tfl / peak, "peak_tflops": peak, "pair_config": pn.pn_get_pair_config()}), flush=True)
+                "roofline_frac": tfl / peak, "peak_tflops": peak, "epilogue": epi, "pair_config": cfg}), flush=True)
         pn.pn_destroy()
+
+
+def run_variants(args) -> None:
+    """--variants: the table behind choose_sym's size thresholds (pn_api.cu): every form of the symmetric fp64 pair kernel
+    (PN_SYM_FORM = w1: one-warp blocks on 128-star tiles, js: four warps share one 128 x 128 tile pair, u512: 512-star tiles),
+    forced through the environment of pn_create, at sizes around the switch points; pair-stage time of one force evaluation,
+    median of 7.  One JSON line per (N, form); "auto" is what the library picks by itself."""
+    import torch
+
+    from paper_1801_07986_b200 import PN, binding, inputs
+
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream()
+    sm_max = load_peaks().get("sm_max_mhz", 1965.0)
+    peak64 = SMS * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    for n_stars in (4095, 8191, 12287, 15359, 16383, 20479, 32767, 36863, 49151, 65535, 131071):
+        p = inputs.plummer_bh(n_stars, seed=n_stars)
+        pos, vel = torch.from_numpy(p.pos).cuda(), torch.from_numpy(p.vel).cuda()
+        acc = torch.empty_like(pos)
+        for form in ("auto", "w1", "js", "u512"):
+            os.environ.pop("PN_SYM_FORM", None)
+            if form != "auto":
+                os.environ["PN_SYM_FORM"] = form
+            pn = PN(p.mass, p.G, p.c, p.softening, stream=stream)
+            os.environ.pop("PN_SYM_FORM", None)
+            pn.pn_set_option(binding.PN_OPT_PAIR_KERNEL, binding.PN_PAIR_SYMMETRIC)
+            pn.pn_set_option(binding.PN_OPT_TIME_PAIR, 1)
+            cfg = pn.pn_get_pair_config()
+            times = []
+            for r in range(9):
+                pn.pn_accel(pos, vel, acc)
+                ms, n = pn.pn_get_pair_time(reset=True)
+                if r >= 2:
+                    times.append(ms / n)
+            pn.pn_destroy()
+            ms = float(np.median(times))
+            print(json.dumps({"N": p.N, "form": form, "pair_kernel_ms": ms, "pair_kernel_pairs_per_s": p.pairs_per_eval / (ms * 1e-3),
+                              "roofline_frac": p.pairs_per_eval * 2 * cfg["fp64_instr_per_pair"] / (ms * 1e-3) / 1e12 / peak64,
+                              "pair_config": cfg}), flush=True)
 
 
 # PAPER.md:137-142, Table 3.2: elapsed seconds of 32 RK4 steps + energy at both ends, mean of 10 samples,
@@ -757,6 +881,7 @@ def run_cold_collapse(args) -> None:
 
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--variants", action="store_true", help="forms of the symmetric fp64 pair kernel around choose_sym's thresholds")
     ap.add_argument("--sweep", action="store_true", help="config-5 single-evaluation sweep (one JSON line per case)")
     ap.add_argument("--sweep-configs", action="store_true")
     ap.add_argument("--kmin", type=int, default=10)
@@ -767,6 +892,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sustain-s", type=float, default=2.0, help="length of each sustained leg (config 2 and config 3) in seconds; 0: skip")
     ap.add_argument("--no-bar", action="store_true", help="skip the short config-3 leg (the >= 70 %% bar's configuration)")
     ap.add_argument("--cross", nargs="?", const="star", default=None, choices=["star", "full"],
                     help="add the Cross terms (NEXT rows of the scope table): star = [a_i]_Cross, Eq. 2.6; "
@@ -788,6 +914,8 @@ def main():
         run_cold_collapse(args)
     elif args.paper_timing:
         run_paper_timing(args)
+    elif args.variants:
+        run_variants(args)
     elif args.sweep:
         run_sweep(args)
     elif args.impl == "reference":

@@ -151,6 +151,14 @@ int pn_get_pair_time(pn_ctx* ctx, double* ms_total_host, int64_t* n_launches_hos
                                                                             since the last reset; synchronises the stream.
                                                                             On the small-system path (PN_PAIR_AUTO) there is
                                                                             no separate pair stage: both come back 0 */
+int pn_get_epilogue_time(pn_ctx* ctx, double* ms_total_host, int64_t* n_intervals_host, int reset); /* PN_OPT_TIME_PAIR = 1 and
+                                                                            pn_step on its CUDA graph: sum and count of the intervals
+                                                                            from the end of one bracketed pair stage to the start
+                                                                            of the next one inside a step (3 per step) -- each is
+                                                                            one fused epilogue (S2 + S3 + S4, with the Cross terms
+                                                                            also their O(N) preparation kernels) plus the launch
+                                                                            gaps around it.  For the HBM figure of the O(N) kernels
+                                                                            at large N; 0 otherwise.  Synchronises the stream */
 int pn_get_pair_config(pn_ctx* ctx, int32_t* cfg_host); /* 8 ints: threads/block, i per thread, j-tile, partial-sum
                                                            slots (j-splits / groups), grid blocks, padded N_s, pipe
                                                            instructions per ordered pair, variant (0 fp64 tiled,

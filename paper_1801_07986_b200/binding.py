@@ -26,7 +26,7 @@ EXPORTS = (
     "pn_create", "pn_destroy", "pn_set_stream", "pn_set_option", "pn_set_state", "pn_get_state",
     "pn_set_state_host", "pn_get_state_host", "pn_accel", "pn_accel_host", "pn_step", "pn_energy", "pn_momentum",
     "pn_get_launch_count", "pn_get_pair_time", "pn_get_pair_config", "pn_last_error",
-    "pn_version", "pn_bh_accel_noalloc",
+    "pn_version", "pn_bh_accel_noalloc", "pn_get_epilogue_time",
 )
 PN_NOALLOC_MAX_STARS = 1 << 20
 
@@ -64,6 +64,7 @@ def load_library() -> ctypes.CDLL:
     lib.pn_momentum.argtypes = [vp, ctypes.POINTER(dbl)]
     lib.pn_get_launch_count.argtypes = [vp, ctypes.POINTER(i64)]
     lib.pn_get_pair_time.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(i64), ci]
+    lib.pn_get_epilogue_time.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(i64), ci]
     lib.pn_get_pair_config.argtypes = [vp, ctypes.POINTER(ctypes.c_int32)]
     lib.pn_last_error.argtypes = [vp]
     lib.pn_last_error.restype = ctypes.c_char_p
@@ -228,6 +229,11 @@ class PN:
     def pn_get_pair_time(self, reset: bool = True):
         ms, n = ctypes.c_double(0.0), ctypes.c_int64(0)
         _check(self._lib, self._ctx, self._lib.pn_get_pair_time(self._ctx, ctypes.byref(ms), ctypes.byref(n), int(reset)))
+        return ms.value, n.value
+
+    def pn_get_epilogue_time(self, reset: bool = True):
+        ms, n = ctypes.c_double(0.0), ctypes.c_int64(0)
+        _check(self._lib, self._ctx, self._lib.pn_get_epilogue_time(self._ctx, ctypes.byref(ms), ctypes.byref(n), int(reset)))
         return ms.value, n.value
 
     def pn_get_pair_config(self) -> dict:

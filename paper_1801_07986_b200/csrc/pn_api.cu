@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -107,6 +108,10 @@ struct pn_ctx {
     size_t ev_used = 0;
     double pair_ms_folded = 0;
     int64_t pair_n_folded = 0;
+    std::vector<char> ev_chain;   // per event pair: 1 = it follows the previous pair inside one captured RK4 step, so the time
+                                  // from that pair's stop to this pair's start is one epilogue (pn_get_epilogue_time)
+    double epi_ms_folded = 0;
+    int64_t epi_n_folded = 0;
 };
 
 namespace {
@@ -174,6 +179,13 @@ void choose_sym(pn_ctx* c)
         c->sym_kind = SYM_JS_U128;
     else
         c->sym_kind = SYM_W4_U512;
+    // diagnostics only (bench.py --variants: the table behind the thresholds above): PN_SYM_FORM=w1|js|u512 in the environment
+    // of pn_create forces a form.  The form fixes the padding and the buffer sizes, hence creation time and not pn_set_option.
+    if (const char* f = std::getenv("PN_SYM_FORM")) {
+        if (!std::strcmp(f, "w1")) c->sym_kind = SYM_W1_U128;
+        else if (!std::strcmp(f, "js")) c->sym_kind = SYM_JS_U128;
+        else if (!std::strcmp(f, "u512")) c->sym_kind = SYM_W4_U512;
+    }
     c->sym_I = 4;
     c->sym_W = (c->sym_kind == SYM_W1_U128) ? 1 : 4;
     c->sym_U = (c->sym_kind == SYM_W4_U512) ? 512 : 128;
@@ -454,7 +466,13 @@ int fold_events(pn_ctx* c)
         float ms = 0;
         PN_CUDA(c, cudaEventElapsedTime(&ms, c->ev[q], c->ev[q + 1]));
         c->pair_ms_folded += ms;
+        if (q / 2 < c->ev_chain.size() && c->ev_chain[q / 2]) {
+            PN_CUDA(c, cudaEventElapsedTime(&ms, c->ev[q - 1], c->ev[q]));
+            c->epi_ms_folded += ms;
+            c->epi_n_folded += 1;
+        }
     }
+    c->ev_chain.assign(c->ev_chain.size(), 0);
     c->pair_n_folded += (int64_t)(c->ev_used / 2);
     c->ev_used = 0;
     return PN_OK;
@@ -1091,6 +1109,11 @@ int pn_step(pn_ctx* c, double dt, int64_t nsteps)
             for (int q = 0; q < ne; ++q)
                 PN_CUDA(c, cudaGraphExecEventRecordNodeSetEvent(c->graphT, c->tnode[q], c->ev[c->ev_used + q]));
             PN_CUDA(c, cudaGraphLaunch(c->graphT, c->stream));
+            if (ne == 8) {  // four bracketed pair stages in one step: between two of them lies exactly one epilogue
+                const size_t base = c->ev_used / 2;
+                if (c->ev_chain.size() < base + 4) c->ev_chain.resize(base + 4, 0);
+                c->ev_chain[base] = 0, c->ev_chain[base + 1] = c->ev_chain[base + 2] = c->ev_chain[base + 3] = 1;
+            }
             c->ev_used += ne;
         }
         c->n_launch += 4 * (1 + kernels_per_eval(c)) * nsteps;
@@ -1175,6 +1198,17 @@ int pn_get_pair_time(pn_ctx* c, double* ms_total, int64_t* n_launches, int reset
     *ms_total = c->pair_ms_folded;
     *n_launches = c->pair_n_folded;
     if (reset) c->pair_ms_folded = 0, c->pair_n_folded = 0;
+    return PN_OK;
+}
+
+int pn_get_epilogue_time(pn_ctx* c, double* ms_total, int64_t* n_intervals, int reset)
+{
+    if (int rc = check_ctx(c)) return rc;
+    if (!ms_total || !n_intervals) return fail(c, PN_EINVAL, "pn_get_epilogue_time: null pointer");
+    if (int rc = fold_events(c)) return rc;
+    *ms_total = c->epi_ms_folded;
+    *n_intervals = c->epi_n_folded;
+    if (reset) c->epi_ms_folded = 0, c->epi_n_folded = 0;
     return PN_OK;
 }
 
